@@ -1,0 +1,214 @@
+"""CPU oracle for the client hot path of arxiv 2006.14726 -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  The product (paper_2006_14726_b200) never does, and
+this package never imports the product.  The arithmetic lives in splat_oracle.cpp
+(single-threaded C++, float32 with the op order of DESIGN.md sec. 3); this file
+only compiles it and marshals numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "splat_oracle.cpp"
+_LIB = _HERE / "libsplatoracle.so"
+_lib = None
+
+_vp = ctypes.c_void_p
+_i32 = ctypes.c_int
+_i64 = ctypes.c_int64
+
+
+def _cpu_has_fma() -> bool:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    return " fma " in (line + " ")
+    except OSError:
+        pass
+    return False
+
+
+def build(force: bool = False) -> Path:
+    """g++ -O2 -ffp-contract=off: the only fused multiply-adds are explicit fmaf().
+    -mfma (when the host has it) merely inlines fmaf(); the result is the same
+    correctly rounded value libm's fmaf() returns."""
+    stamp = _HERE / ".built_with_fma"
+    want_fma = _cpu_has_fma()
+    stale = (not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime
+             or (stamp.exists() and not want_fma))
+    if force or stale:
+        cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC"]
+        if want_fma:
+            cmd.append("-mfma")
+        cmd += [str(_SRC), "-o", str(_LIB)]
+        subprocess.run(cmd, check=True)
+        if want_fma:
+            stamp.write_text("1")
+        elif stamp.exists():
+            stamp.unlink()
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(str(_LIB))
+        L.oracle_pixel_ray.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp, _vp]
+        L.oracle_unproject.argtypes = [_vp, _vp, _i32, _i32, ctypes.c_float, _vp, _vp]
+        L.oracle_unproject.restype = _i64
+        L.oracle_bounds.argtypes = [_vp, _vp, _i64, _vp, _vp]
+        L.oracle_morton_point.argtypes = [_vp, _vp, _vp]
+        L.oracle_morton_point.restype = ctypes.c_uint64
+        L.oracle_compact_codes.argtypes = [_vp, _vp, _i64, _vp, _vp, _vp, _vp]
+        L.oracle_compact_codes.restype = _i64
+        L.oracle_sort.argtypes = [_vp, _i64, _vp]
+        L.oracle_tree.argtypes = [_vp, _i64, _vp, _vp, _vp]
+        L.oracle_refit.argtypes = [_vp, _vp, _i64, _vp]
+        L.oracle_ray_sphere.argtypes = [_vp, _vp, _vp, _vp]
+        L.oracle_ray_sphere.restype = _i32
+        L.oracle_composite.argtypes = [_i32, _vp, _vp, _vp, _vp]
+        L.oracle_composite.restype = _i32
+        L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+        L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+        _lib = L
+    return _lib
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _ptr(a):
+    return a.ctypes.data if a is not None else None
+
+
+# ------------------------------------------------------------------ single steps
+def pixel_ray(cam, W, H, x, y):
+    cam = _f32(cam)
+    d = np.empty(3, np.float32)
+    ln = np.empty(1, np.float32)
+    lib().oracle_pixel_ray(_ptr(cam), W, H, x, y, _ptr(d), _ptr(ln))
+    return d, float(ln[0])
+
+
+def unproject(depth, cam, W, H, r_scale):
+    depth, cam = _f32(depth).reshape(-1), _f32(cam)
+    assert depth.size == W * H
+    sphere = np.empty((W * H, 4), np.float32)
+    valid = np.empty(W * H, np.uint8)
+    n = lib().oracle_unproject(_ptr(depth), _ptr(cam), W, H, float(r_scale), _ptr(sphere), _ptr(valid))
+    return sphere, valid, int(n)
+
+
+def bounds(sphere, valid):
+    lo, hi = np.empty(3, np.float32), np.empty(3, np.float32)
+    lib().oracle_bounds(_ptr(sphere), _ptr(valid), sphere.shape[0], _ptr(lo), _ptr(hi))
+    return lo, hi
+
+
+def morton_point(c, lo, hi) -> int:
+    c, lo, hi = _f32(c), _f32(lo), _f32(hi)
+    return int(lib().oracle_morton_point(_ptr(c), _ptr(lo), _ptr(hi)))
+
+
+def compact_codes(sphere, valid, lo, hi, n):
+    ids = np.empty(n, np.uint32)
+    codes = np.empty(n, np.uint64)
+    lo, hi = _f32(lo), _f32(hi)
+    m = lib().oracle_compact_codes(_ptr(sphere), _ptr(valid), sphere.shape[0], _ptr(lo), _ptr(hi), _ptr(ids), _ptr(codes))
+    assert m == n
+    return ids, codes
+
+
+def sort_codes(codes):
+    codes = np.ascontiguousarray(codes, dtype=np.uint64)
+    order = np.empty(codes.size, np.uint32)
+    lib().oracle_sort(_ptr(codes), codes.size, _ptr(order))
+    return order
+
+
+def tree(sorted_codes):
+    sorted_codes = np.ascontiguousarray(sorted_codes, dtype=np.uint64)
+    n = sorted_codes.size
+    children = np.full((max(n - 1, 0), 2), -1, np.int32)
+    parents = np.full(max(2 * n - 1, 0), -2, np.int32)
+    ranges = np.full((max(n - 1, 0), 2), -1, np.int32)
+    lib().oracle_tree(_ptr(sorted_codes), n, _ptr(children), _ptr(parents), _ptr(ranges))
+    return children, parents, ranges
+
+
+def refit(sphere_sorted, children):
+    sphere_sorted = _f32(sphere_sorted)
+    n = sphere_sorted.shape[0]
+    aabbs = np.zeros((max(2 * n - 1, 0), 6), np.float32)
+    lib().oracle_refit(_ptr(sphere_sorted), _ptr(children), n, _ptr(aabbs))
+    return aabbs
+
+
+def ray_sphere(o, d, sphere4):
+    o, d, s = _f32(o), _f32(d), _f32(sphere4)
+    t = np.zeros(1, np.float32)
+    hit = lib().oracle_ray_sphere(_ptr(o), _ptr(d), _ptr(s), _ptr(t))
+    return bool(hit), float(t[0])
+
+
+def composite(t, ids, rgba):
+    t, rgba = _f32(t), _f32(rgba)
+    ids = np.ascontiguousarray(ids, dtype=np.uint32)
+    out = np.zeros(4, np.float32)
+    used = lib().oracle_composite(t.size, _ptr(t), _ptr(ids), _ptr(rgba), _ptr(out))
+    return out, int(used)
+
+
+# ------------------------------------------------------------------ whole path
+def build_scene(color, depth, cam, W, H, r_scale):
+    """O1..O7 on one 2.5D frame.  Returns a dict of numpy arrays (see keys below)."""
+    color = _f32(color).reshape(W * H, 4)
+    sphere, valid, n = unproject(depth, cam, W, H, r_scale)
+    lo, hi = bounds(sphere, valid)
+    ids, codes = compact_codes(sphere, valid, lo, hi, n)
+    order = sort_codes(codes)
+    sorted_ids = ids[order]
+    sorted_codes = codes[order]
+    sphere_sorted = np.ascontiguousarray(sphere[sorted_ids])
+    rgba_sorted = np.ascontiguousarray(color[sorted_ids])
+    children, parents, ranges = tree(sorted_codes)
+    aabbs = refit(sphere_sorted, children)
+    return dict(N=n, W=W, H=H, sphere=sphere, valid=valid, lo=lo, hi=hi, ids=ids, codes=codes, order=order,
+                sorted_ids=sorted_ids, sorted_codes=sorted_codes, sphere_sorted=sphere_sorted,
+                rgba_sorted=rgba_sorted, children=children, parents=parents, ranges=ranges, aabbs=aabbs)
+
+
+def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False):
+    """O8..O9.  mode 'brute' = L0 (definition), 'bvh' = L1 (walk of the oracle's tree).
+    pixels: optional int64 array of destination pixel indices (y*W2+x)."""
+    cam = _f32(cam)
+    n = scene["N"]
+    if pixels is not None:
+        pixels = np.ascontiguousarray(pixels, dtype=np.int64)
+        total = pixels.size
+    else:
+        total = W2 * H2
+    out = np.zeros((total, 4), np.float32)
+    used = np.zeros(total, np.int32)
+    sp, co, ids = scene["sphere_sorted"], scene["rgba_sorted"], scene["sorted_ids"]
+    if mode == "brute":
+        lib().oracle_render_brute(_ptr(sp), _ptr(co), _ptr(ids), n, _ptr(cam), W2, H2, _ptr(pixels), total,
+                                  _ptr(out), _ptr(used))
+    elif mode == "bvh":
+        lib().oracle_render_bvh(_ptr(sp), _ptr(co), _ptr(ids), n, _ptr(scene["children"]), _ptr(scene["aabbs"]),
+                                _ptr(cam), W2, H2, _ptr(pixels), total, _ptr(out), _ptr(used))
+    else:
+        raise ValueError(mode)
+    if pixels is None:
+        out = out.reshape(H2, W2, 4)
+        used = used.reshape(H2, W2)
+    return (out, used) if return_hits else out

@@ -1,0 +1,375 @@
+// oracle/splat_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, single-threaded CPU statement of what the client hot path of
+// arxiv 2006.14726 computes (2.5D frame -> sphere splats -> LBVH -> ray-traced,
+// front-to-back composited image).  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code
+// with the CUDA path (paper_2006_14726_b200/csrc) and neither includes the other.
+//
+// Precision: float32 with the operation order written out below.  The paper does
+// not fix a precision; the acceptance bar (BASELINE.json north_star) is *bit-exact*
+// Morton codes / permutation / topology / AABBs, and a sphere hit-or-miss is a
+// decision taken by floating point, so both sides take those decisions in the
+// kernel's precision (float32) with one stated op order (DESIGN.md sec. 3,
+// SURVEY.md sec. 8(c) O1..O9).  Compile with -ffp-contract=off: the only fused
+// multiply-adds are the explicit fmaf() calls.
+//
+// Parity pins (tests/test_oracle_*.py): closed-form single-sphere hit t, closed-form
+// alpha stack, identity-camera reprojection == source image bit-exactly, Morton codes
+// vs a bit loop and hand-worked values, sort == numpy stable argsort, top-down tree
+// == Karras' per-node construction (re-implemented in the test) on random and
+// duplicate-heavy keys and on a hand-worked 8-key example, BVH-walk renderer ==
+// brute-force renderer.  "Parity unpinned": only the conservative slab test used by
+// the BVH-walk renderer (any conservative test is correct; it is checked through
+// BVH-walk == brute force).
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Camera {  // PAPER.md:85 "the camera the buffers are associated with"
+  float e[3], R[3], U[3], F[3], tau;
+};
+
+Camera load_camera(const float* c13) {
+  Camera c;
+  for (int k = 0; k < 3; ++k) { c.e[k] = c13[k]; c.R[k] = c13[3 + k]; c.U[k] = c13[6 + k]; c.F[k] = c13[9 + k]; }
+  c.tau = c13[12];
+  return c;
+}
+
+// O1 (first half) -- primary ray through the centre of pixel (x, y); row 0 = top.
+// PAPER.md:63 sec. 4.1 "We march rays r = o + d t".  Returns the unit direction and
+// the length `len` of the un-normalised direction F + u R + v U.
+void pixel_ray(const Camera& c, int W, int H, int x, int y, float dhat[3], float* len_out) {
+  float nx = (float)(2 * x + 1 - W) / (float)W;
+  float ny = (float)(H - 2 * y - 1) / (float)H;
+  float ta = (c.tau * (float)W) / (float)H;
+  float u = nx * ta;
+  float v = ny * c.tau;
+  float d[3];
+  for (int k = 0; k < 3; ++k) d[k] = fmaf(v, c.U[k], fmaf(u, c.R[k], c.F[k]));
+  float len = sqrtf(fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0])));
+  for (int k = 0; k < 3; ++k) dhat[k] = d[k] / len;
+  *len_out = len;
+}
+
+// O2 -- k_r = r_scale * sqrt(1/2) * (2 tau / H): half-diagonal of a pixel at unit
+// view-axis depth (north_star: "radius is its one-pixel footprint at its depth";
+// by analogy with PAPER.md:69 "half the size of a voxel's diagonal").
+float radius_factor(const Camera& c, int H, float r_scale) {
+  const float SQRT_HALF = 0.70710678118654752440f;
+  return (r_scale * SQRT_HALF) * ((2.0f * c.tau) / (float)H);
+}
+
+// O3 -- PAPER.md:69: samples with zero radius never reach the client.
+bool depth_valid(float t) { return std::isfinite(t) && t > 0.0f; }
+
+// O4 -- 63-bit Morton code, 21 bit per axis, x in the highest slot of each triple.
+uint64_t morton63(const float c[3], const float lo[3], const float hi[3]) {
+  uint32_t q[3];
+  for (int k = 0; k < 3; ++k) {
+    float ext = hi[k] - lo[k];
+    if (ext > 0.0f) {
+      float s = ((c[k] - lo[k]) / ext) * 2097152.0f;
+      uint32_t v = (uint32_t)s;
+      q[k] = v < 2097151u ? v : 2097151u;
+    } else {
+      q[k] = 0;
+    }
+  }
+  uint64_t code = 0;
+  for (int i = 0; i < 21; ++i) {
+    code |= (uint64_t)((q[0] >> i) & 1u) << (3 * i + 2);
+    code |= (uint64_t)((q[1] >> i) & 1u) << (3 * i + 1);
+    code |= (uint64_t)((q[2] >> i) & 1u) << (3 * i);
+  }
+  return code;
+}
+
+// O8 -- ray / sphere entry point ("spheres that are represented as real quadrics",
+// PAPER.md:55), perpendicular-vector form (the b*b - c form misses
+// 9 % of the hits at these radii in float32).
+bool ray_sphere(const float o[3], const float d[3], const float s[4], float* t_out) {
+  float oc[3] = {s[0] - o[0], s[1] - o[1], s[2] - o[2]};
+  float b = fmaf(oc[2], d[2], fmaf(oc[1], d[1], oc[0] * d[0]));
+  float l[3];
+  for (int k = 0; k < 3; ++k) l[k] = fmaf(-b, d[k], oc[k]);
+  float l2 = fmaf(l[2], l[2], fmaf(l[1], l[1], l[0] * l[0]));
+  float disc = fmaf(s[3], s[3], -l2);
+  if (!(disc > 0.0f)) return false;  // tangent = miss
+  float t = b - sqrtf(disc);
+  if (!(t >= 0.0f)) return false;    // eye inside (or sphere behind): no contribution
+  *t_out = t;
+  return true;
+}
+
+struct Hit { float t; uint32_t id; uint32_t leaf; };
+bool hit_less(const Hit& a, const Hit& b) { return a.t < b.t || (a.t == b.t && a.id < b.id); }
+
+// O9 -- front-to-back premultiplied "over" of the hits in (t, id) order, stop once
+// A >= 0.99 (tested after each hit).  "no shading other than the constant sample
+// color".  Returns how many hits were composited.
+int composite(std::vector<Hit>& hits, const float* rgba /*[N][4], sorted order*/, float out[4]) {
+  std::sort(hits.begin(), hits.end(), hit_less);
+  float C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f;
+  int used = 0;
+  for (const Hit& h : hits) {
+    const float* col = rgba + 4 * (size_t)h.leaf;
+    float T = 1.0f - A;
+    for (int k = 0; k < 3; ++k) C[k] = fmaf(T, col[k], C[k]);
+    A = fmaf(T, col[3], A);
+    ++used;
+    if (A >= 0.99f) break;
+  }
+  out[0] = C[0]; out[1] = C[1]; out[2] = C[2]; out[3] = A;
+  return used;
+}
+
+// Conservative slab test for the BVH-walk renderer (unpinned on purpose): double
+// arithmetic on a box padded by far more than the float32 error of ray_sphere().
+bool ray_box_conservative(const float o[3], const float d[3], const float* box /*lo3,hi3*/) {
+  double m = 1.0;
+  for (int k = 0; k < 3; ++k) {
+    m = std::max(m, std::fabs((double)o[k]));
+    m = std::max(m, std::fabs((double)box[k]));
+    m = std::max(m, std::fabs((double)box[3 + k]));
+  }
+  double pad = 1e-4 * m;
+  double tn = -1e300, tf = 1e300;
+  for (int k = 0; k < 3; ++k) {
+    double lo = (double)box[k] - pad, hi = (double)box[3 + k] + pad;
+    if (d[k] == 0.0f) {
+      if (o[k] < lo || o[k] > hi) return false;
+      continue;
+    }
+    double a = (lo - o[k]) / d[k], b = (hi - o[k]) / d[k];
+    if (a > b) std::swap(a, b);
+    tn = std::max(tn, a);
+    tf = std::min(tf, b);
+  }
+  return tn <= tf && tf >= 0.0;
+}
+
+}  // namespace
+
+extern "C" {
+
+// ---- O1: unit ray direction of pixel (x, y) and the un-normalised length.
+void oracle_pixel_ray(const float* cam13, int W, int H, int x, int y, float* dhat3, float* len) {
+  Camera c = load_camera(cam13);
+  pixel_ray(c, W, H, x, y, dhat3, len);
+}
+
+// ---- O1..O3: Eq. 1 p = o + d t_i for every pixel, radius, validity.
+// sphere[p] = (cx, cy, cz, r) and valid[p]; entries of invalid pixels are zeroed.
+// Returns N = number of valid pixels.
+int64_t oracle_unproject(const float* depth, const float* cam13, int W, int H, float r_scale,
+                         float* sphere /*[P][4]*/, uint8_t* valid /*[P]*/) {
+  Camera c = load_camera(cam13);
+  float k_r = radius_factor(c, H, r_scale);
+  int64_t n = 0;
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      size_t p = (size_t)y * W + x;
+      float t = depth[p];
+      float* s = sphere + 4 * p;
+      if (!depth_valid(t)) { valid[p] = 0; s[0] = s[1] = s[2] = s[3] = 0.0f; continue; }
+      float dh[3], len;
+      pixel_ray(c, W, H, x, y, dh, &len);
+      for (int k = 0; k < 3; ++k) s[k] = fmaf(t, dh[k], c.e[k]);  // Eq. 1
+      float z = t / len;                                          // view-axis depth
+      s[3] = k_r * z;
+      valid[p] = 1;
+      ++n;
+    }
+  return n;
+}
+
+// ---- O4 (bounds): component-wise min / max of the valid centres.
+void oracle_bounds(const float* sphere, const uint8_t* valid, int64_t P, float* lo3, float* hi3) {
+  bool any = false;
+  for (int64_t p = 0; p < P; ++p) {
+    if (!valid[p]) continue;
+    const float* s = sphere + 4 * p;
+    if (!any) { for (int k = 0; k < 3; ++k) lo3[k] = hi3[k] = s[k]; any = true; continue; }
+    for (int k = 0; k < 3; ++k) { lo3[k] = fminf(lo3[k], s[k]); hi3[k] = fmaxf(hi3[k], s[k]); }
+  }
+  if (!any) for (int k = 0; k < 3; ++k) lo3[k] = hi3[k] = 0.0f;
+}
+
+uint64_t oracle_morton_point(const float* c3, const float* lo3, const float* hi3) { return morton63(c3, lo3, hi3); }
+
+// ---- O3 + O4: compaction in ascending pixel order; ids[n] = pixel index, codes[n].
+int64_t oracle_compact_codes(const float* sphere, const uint8_t* valid, int64_t P, const float* lo3,
+                             const float* hi3, uint32_t* ids /*[N]*/, uint64_t* codes /*[N]*/) {
+  int64_t n = 0;
+  for (int64_t p = 0; p < P; ++p) {
+    if (!valid[p]) continue;
+    ids[n] = (uint32_t)p;
+    codes[n] = morton63(sphere + 4 * p, lo3, hi3);
+    ++n;
+  }
+  return n;
+}
+
+// ---- O5: std::stable_sort by code over ids in ascending order == order by (code, id).
+// order[j] = compacted index of the j-th splat in sorted order.
+void oracle_sort(const uint64_t* codes, int64_t N, uint32_t* order) {
+  std::vector<uint32_t> idx((size_t)N);
+  for (int64_t i = 0; i < N; ++i) idx[i] = (uint32_t)i;
+  std::stable_sort(idx.begin(), idx.end(), [&](uint32_t a, uint32_t b) { return codes[a] < codes[b]; });
+  for (int64_t i = 0; i < N; ++i) order[i] = idx[i];
+}
+
+// ---- O6: top-down binary radix tree over the sorted codes (LBVH, PAPER.md:71
+// [LGS*09]), Karras numbering.  Node ids: internal j in [0, N-1) -> j, leaf i
+// (sorted position) -> (N-1) + i.  children[j] = {left id, right id};
+// parents[id] = internal index of the parent, -1 for the root;
+// ranges[j] = {first, last} sorted position covered by internal node j.
+void oracle_tree(const uint64_t* sorted_codes, int64_t N, int32_t* children /*[N-1][2]*/,
+                 int32_t* parents /*[2N-1]*/, int32_t* ranges /*[N-1][2]*/) {
+  if (N <= 0) return;
+  if (N == 1) { parents[0] = -1; return; }  // the single leaf is the root
+  struct Item { int64_t a, b; int32_t node; };
+  std::vector<Item> stack;
+  parents[0] = -1;
+  stack.push_back({0, N - 1, 0});
+  while (!stack.empty()) {
+    Item it = stack.back();
+    stack.pop_back();
+    int64_t a = it.a, b = it.b, gamma = a;
+    if (sorted_codes[a] != sorted_codes[b]) {
+      uint64_t diff = sorted_codes[a] ^ sorted_codes[b];
+      int m = 63;
+      while (!((diff >> m) & 1ull)) --m;             // highest differing bit
+      for (int64_t i = a; i <= b; ++i)               // last index whose bit m is 0
+        if (!((sorted_codes[i] >> m) & 1ull)) gamma = i;
+    } else {                                         // duplicates: split on the sorted position
+      uint32_t diff = (uint32_t)a ^ (uint32_t)b;
+      int m = 31;
+      while (!((diff >> m) & 1u)) --m;
+      for (int64_t i = a; i <= b; ++i)
+        if (!(((uint32_t)i >> m) & 1u)) gamma = i;
+    }
+    int32_t left, right;
+    if (gamma == a) left = (int32_t)(N - 1 + a);
+    else { left = (int32_t)gamma; stack.push_back({a, gamma, left}); }
+    if (gamma + 1 == b) right = (int32_t)(N - 1 + b);
+    else { right = (int32_t)(gamma + 1); stack.push_back({gamma + 1, b, right}); }
+    children[2 * (size_t)it.node] = left;
+    children[2 * (size_t)it.node + 1] = right;
+    parents[left] = it.node;
+    parents[right] = it.node;
+    ranges[2 * (size_t)it.node] = (int32_t)a;
+    ranges[2 * (size_t)it.node + 1] = (int32_t)b;
+  }
+}
+
+// ---- O7: leaf box = centre -/+ r; internal box = exact union of its children.
+// sphere_sorted[i] = sphere of the leaf at sorted position i.  aabbs[id] = lo3, hi3.
+void oracle_refit(const float* sphere_sorted, const int32_t* children, int64_t N, float* aabbs /*[2N-1][6]*/) {
+  if (N <= 0) return;
+  for (int64_t i = 0; i < N; ++i) {
+    const float* s = sphere_sorted + 4 * i;
+    float* bx = aabbs + 6 * (size_t)(N - 1 + i);
+    for (int k = 0; k < 3; ++k) { bx[k] = s[k] - s[3]; bx[3 + k] = s[k] + s[3]; }
+  }
+  if (N == 1) return;
+  // post-order over the tree (children before parents)
+  std::vector<int32_t> order;
+  std::vector<int32_t> stack{0};
+  while (!stack.empty()) {
+    int32_t j = stack.back();
+    stack.pop_back();
+    order.push_back(j);
+    for (int s = 0; s < 2; ++s) {
+      int32_t ch = children[2 * (size_t)j + s];
+      if (ch < N - 1) stack.push_back(ch);
+    }
+  }
+  for (size_t q = order.size(); q-- > 0;) {
+    int32_t j = order[q];
+    const float* l = aabbs + 6 * (size_t)children[2 * (size_t)j];
+    const float* r = aabbs + 6 * (size_t)children[2 * (size_t)j + 1];
+    float* bx = aabbs + 6 * (size_t)j;
+    for (int k = 0; k < 3; ++k) { bx[k] = fminf(l[k], r[k]); bx[3 + k] = fmaxf(l[3 + k], r[3 + k]); }
+  }
+}
+
+// ---- O8 for one ray and one sphere (pins: closed-form t).
+int oracle_ray_sphere(const float* o3, const float* d3, const float* sphere4, float* t_out) {
+  return ray_sphere(o3, d3, sphere4, t_out) ? 1 : 0;
+}
+
+// ---- O9 for a given hit list (pins: alpha-stack closed form).  rgba[i] belongs to hit i.
+int oracle_composite(int n, const float* t, const uint32_t* id, const float* rgba, float* out4) {
+  std::vector<Hit> hits((size_t)n);
+  for (int i = 0; i < n; ++i) hits[i] = {t[i], id[i], (uint32_t)i};
+  return composite(hits, rgba, out4);
+}
+
+// ---- L0: brute-force renderer -- every ray against every splat (the definition).
+// Arrays are in sorted order (any order gives the same image: hits are ordered by
+// (t, id)).  pixels == nullptr: whole frame into out[H2*W2*4]; otherwise only the
+// n_pixels listed pixel indices, out[n_pixels*4].  hits_used (optional) receives the
+// number of composited hits per output pixel.
+void oracle_render_brute(const float* sphere, const float* rgba, const uint32_t* ids, int64_t N,
+                         const float* cam13, int W2, int H2, const int64_t* pixels, int64_t n_pixels,
+                         float* out, int32_t* hits_used) {
+  Camera c = load_camera(cam13);
+  int64_t total = pixels ? n_pixels : (int64_t)W2 * H2;
+  std::vector<Hit> hits;
+  for (int64_t q = 0; q < total; ++q) {
+    int64_t p = pixels ? pixels[q] : q;
+    int x = (int)(p % W2), y = (int)(p / W2);
+    float dh[3], len;
+    pixel_ray(c, W2, H2, x, y, dh, &len);
+    hits.clear();
+    for (int64_t i = 0; i < N; ++i) {
+      float t;
+      if (ray_sphere(c.e, dh, sphere + 4 * i, &t)) hits.push_back({t, ids[i], (uint32_t)i});
+    }
+    int used = composite(hits, rgba, out + 4 * q);
+    if (hits_used) hits_used[q] = used;
+  }
+}
+
+// ---- L1: the same image through a recursive walk of the oracle's own tree.
+namespace {
+void walk(int32_t id, int64_t N, const int32_t* children, const float* aabbs, const float* sphere,
+          const uint32_t* ids, const float o[3], const float d[3], std::vector<Hit>& hits) {
+  if (!ray_box_conservative(o, d, aabbs + 6 * (size_t)id)) return;
+  if (id >= N - 1) {
+    int64_t i = id - (N - 1);
+    float t;
+    if (ray_sphere(o, d, sphere + 4 * i, &t)) hits.push_back({t, ids[i], (uint32_t)i});
+    return;
+  }
+  walk(children[2 * (size_t)id], N, children, aabbs, sphere, ids, o, d, hits);
+  walk(children[2 * (size_t)id + 1], N, children, aabbs, sphere, ids, o, d, hits);
+}
+}  // namespace
+
+void oracle_render_bvh(const float* sphere, const float* rgba, const uint32_t* ids, int64_t N,
+                       const int32_t* children, const float* aabbs, const float* cam13, int W2, int H2,
+                       const int64_t* pixels, int64_t n_pixels, float* out, int32_t* hits_used) {
+  Camera c = load_camera(cam13);
+  int64_t total = pixels ? n_pixels : (int64_t)W2 * H2;
+  std::vector<Hit> hits;
+  for (int64_t q = 0; q < total; ++q) {
+    int64_t p = pixels ? pixels[q] : q;
+    int x = (int)(p % W2), y = (int)(p / W2);
+    float dh[3], len;
+    pixel_ray(c, W2, H2, x, y, dh, &len);
+    hits.clear();
+    if (N > 0) walk(0, N, children, aabbs, sphere, ids, c.e, dh, hits);
+    int used = composite(hits, rgba, out + 4 * q);
+    if (hits_used) hits_used[q] = used;
+  }
+}
+
+}  // extern "C"
