@@ -1,0 +1,131 @@
+/* splats.h -- C ABI of the B200-native client hot path of arxiv 2006.14726
+ * (Zellmann, "Augmenting Image Warping-Based Remote Volume Rendering with Ray Tracing").
+ *
+ * The path (PAPER.md = the paper's text; SURVEY.md sec. 8 = the scope table):
+ *   2.5D frame (RGBA + one depth per pixel, sec. 2; sec. 4.2)
+ *   -> object-space sphere splats, Eq. 1 p = o + d t_i with a footprint
+ *      radius
+ *   -> LBVH over the spheres, rebuilt whenever a frame arrives
+ *   -> software ray tracing of the spheres from the current camera (sec. 4),
+ *      here with front-to-back compositing of every hit (BASELINE.json north_star).
+ *
+ * Conventions common to all calls
+ *   - One library-wide context (created by splats_create, destroyed by splats_destroy); the
+ *     calls are not thread-safe against each other.
+ *   - "dev" pointers are CUDA device pointers on the device that was current at
+ *     splats_create; "host" pointers are ordinary host memory (pinned memory makes the
+ *     *_host copies asynchronous).  The caller owns every buffer it passes in; the library
+ *     owns splats, keys, BVH and scratch, all allocated once in splats_create.
+ *   - splats_update / splats_render only ENQUEUE work on the stream given to splats_create and
+ *     return; input/output buffers must stay valid until that work has run.  No allocation
+ *     and no host<->device synchronisation happens on those two calls.
+ *   - Return value: 0 = ok, SPLATS_EINVAL (-1) invalid argument, SPLATS_ENOBVH (-2) render
+ *     before any update, SPLATS_ECUDA (-3) CUDA error, SPLATS_ESTATE (-4) no context /
+ *     context already exists.  splats_last_error() gives the text.  Nothing aborts or throws.
+ *   - There is no CPU fallback: without a CUDA device splats_create fails with SPLATS_ECUDA.
+ */
+#ifndef SPLATS_H_
+#define SPLATS_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPLATS_OK       0
+#define SPLATS_EINVAL  (-1)
+#define SPLATS_ENOBVH  (-2)
+#define SPLATS_ECUDA   (-3)
+#define SPLATS_ESTATE  (-4)
+
+/* "the camera the buffers are associated with".  POD, host memory, 13 floats.
+ * right/up/fwd must be an orthonormal basis of unit vectors; tan_half_fovy = tan(fovy/2) is
+ * computed by the caller (device code uses no transcendentals).  The aspect ratio is W/H of
+ * the call the camera is passed to.  Pixel (x, y), row 0 = top, has its centre at
+ * ndc ((2x+1-W)/W, (H-2y-1)/H); its ray is fwd + ndc_x*tan*W/H*right + ndc_y*tan*up. */
+typedef struct {
+  float eye[3];
+  float right[3];
+  float up[3];
+  float fwd[3];
+  float tan_half_fovy;
+} wr_camera;
+
+/* Allocate all device memory for source frames of up to max_W*max_H pixels (<= 2^28) and
+ * destination images of up to the same pixel count.  cuda_stream: a cudaStream_t (NULL = the
+ * legacy default stream) on which every later call enqueues its work. */
+int splats_create(void* cuda_stream, int max_W, int max_H);
+
+/* Frame received ("The client upon receiving the data will build an LBVH"):
+ * unproject every valid pixel into a sphere splat and build the LBVH over all splats.
+ *   color  dev, H*W*4 float32, premultiplied RGBA, row-major, row 0 = top; 16-byte aligned
+ *   depth  dev, H*W float32: ray parameter t_i of Eq. 1 for a unit-length ray direction
+ *          (distance from the eye); t <= 0, NaN or Inf marks a dropped pixel (PAPER.md:69:
+ *          zero-radius samples are never sent); 16-byte aligned
+ *   src_camera  host; the camera the frame was rendered from
+ *   r_scale     > 0; splat radius = r_scale * half-diagonal of the pixel's footprint at the
+ *               splat's view-axis depth (north_star)
+ * Steps: bounds, unproject+Morton+compaction, onesweep radix
+ * sort by (code, id), Karras hierarchy, bottom-up refit.  W*H = 0 valid pixels is not an
+ * error (the next render writes zeros).
+ * Errors: EINVAL for NULL pointers, W*H outside [1, capacity], non-finite or <= 0 r_scale,
+ * non-finite camera. */
+int splats_update(const float* color, const float* depth, const wr_camera* src_camera,
+                  int W, int H, float r_scale);
+
+/* Display frame ("the current pixel buffer is warped according to the new
+ * transformation"; ray trace the spheres): one primary ray per destination
+ * pixel through the BVH of the latest splats_update, every sphere entry hit ordered by
+ * (t, splat id) and composited front to back (premultiplied "over") until alpha >= 0.99.
+ *   out_rgba  dev, H2*W2*4 float32, premultiplied, background (0,0,0,0); 16-byte aligned
+ * W2 x H2 may differ from the source frame's size (W2*H2 <= capacity).
+ * Errors: EINVAL as above, ENOBVH if no update was enqueued yet. */
+int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
+
+/* The same two calls with HOST buffers (end-to-end path): the library copies the frame to
+ * device staging memory (cudaMemcpyAsync on the stream), runs the same kernels, and for the
+ * render copies the image back; splats_render_host returns after the image is in out_rgba. */
+int splats_update_host(const float* color_host, const float* depth_host,
+                       const wr_camera* src_camera, int W, int H, float r_scale);
+int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_rgba_host);
+
+/* Number of splats N of the latest update.  Synchronises the stream.  Parity/debug only. */
+int splats_count(unsigned* n_host);
+
+/* Export the BVH of the latest update in canonical form for the bit-exact acceptance
+ * checks.  All pointers are dev pointers (any may be NULL to skip it); synchronises.
+ *   keys        N  uint64   sorted 63-bit Morton codes
+ *   perm        N  uint32   splat ids (= source pixel indices) in sorted order
+ *   children    (N-1)*2 int32; node ids: internal j -> j, leaf at sorted position i -> N-1+i
+ *   parents     (2N-1) int32, indexed by node id; -1 for the root
+ *   node_aabbs  (2N-1)*6 float32: lo xyz, hi xyz per node id
+ * Internal nodes use Karras' numbering (root 0; an internal child covering sorted range
+ * [a,g] is node g when it is a left child, node a when it is a right child). */
+int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* parents,
+                  float* node_aabbs);
+
+/* Export the splats themselves in sorted order (dev pointers, may be NULL): sphere N*4
+ * float32 (cx, cy, cz, r), rgba N*4 float32; and the scene bounds (min/max of the centres)
+ * lo_hi: 6 float32.  Synchronises.  Parity/debug only. */
+int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
+
+/* Per-stage device times of the latest update/render, measured with CUDA events on the
+ * library's stream.  Off by default (the events cost a few microseconds).
+ * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all passes), 3 hierarchy+gather,
+ * 4 refit, 5 render.  Synchronises the stream. */
+#define SPLATS_NUM_STAGES 6
+int splats_set_profiling(int on);
+int splats_stage_ms(float* ms /* host, SPLATS_NUM_STAGES floats */);
+
+/* How many kernels this library has launched since splats_create. */
+unsigned long long splats_launch_count(void);
+
+/* Block until everything enqueued so far has run. */
+int splats_synchronize(void);
+
+const char* splats_last_error(void);
+void splats_destroy(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPLATS_H_ */

@@ -1,0 +1,180 @@
+"""Thin Python binding of the C ABI in include/splats.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libsplats.so; this file converts
+torch tensors / numpy cameras into raw pointers and turns error codes into exceptions.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback:
+if the shared library is missing and cannot be built, importing the symbols raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+NUM_STAGES = 6
+STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "hierarchy_gather", "refit", "render")
+
+
+class SplatsError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"splats error {code}: {msg}")
+        self.code = code
+
+
+class wr_camera(ctypes.Structure):
+    _fields_ = [("eye", ctypes.c_float * 3), ("right", ctypes.c_float * 3), ("up", ctypes.c_float * 3),
+                ("fwd", ctypes.c_float * 3), ("tan_half_fovy", ctypes.c_float)]
+
+
+_lib = None
+_vp = ctypes.c_void_p
+_ci = ctypes.c_int
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsplats.so (building it with nvcc if it is stale or missing)."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        if not Path(path).exists():
+            raise RuntimeError(f"{path} is missing: the CUDA extension is required (no CPU fallback)")
+        L = ctypes.CDLL(str(path))
+        cam_p = ctypes.POINTER(wr_camera)
+        L.splats_create.argtypes = [_vp, _ci, _ci]
+        L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
+        L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
+        L.splats_render_host.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_count.argtypes = [ctypes.POINTER(ctypes.c_uint)]
+        L.splats_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
+        L.splats_export_splats.argtypes = [_vp, _vp, _vp]
+        L.splats_set_profiling.argtypes = [_ci]
+        L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float)]
+        L.splats_launch_count.restype = ctypes.c_ulonglong
+        L.splats_last_error.restype = ctypes.c_char_p
+        L.splats_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise SplatsError(rc, lib().splats_last_error().decode())
+
+
+def _cam(cam) -> wr_camera:
+    a = np.ascontiguousarray(np.asarray(cam, dtype=np.float32).reshape(13))
+    c = wr_camera()
+    ctypes.memmove(ctypes.byref(c), a.ctypes.data, 13 * 4)
+    return c
+
+
+def _dev_ptr(t: torch.Tensor, dtype, numel: int | None = None) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TypeError(f"expected a contiguous CUDA tensor of dtype {dtype}")
+    if numel is not None and t.numel() < numel:
+        raise ValueError(f"tensor too small: {t.numel()} < {numel}")
+    return t.data_ptr()
+
+
+def _host_ptr(t, numel: int) -> int:
+    if isinstance(t, torch.Tensor):
+        if t.is_cuda or not t.is_contiguous() or t.dtype != torch.float32 or t.numel() < numel:
+            raise TypeError("expected a contiguous float32 host tensor of sufficient size")
+        return t.data_ptr()
+    a = t
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags["C_CONTIGUOUS"] and a.size >= numel):
+        raise TypeError("expected a contiguous float32 numpy array of sufficient size")
+    return a.ctypes.data
+
+
+# ----------------------------------------------------------------------------- the C calls
+def splats_create(max_W: int, max_H: int, stream: torch.cuda.Stream | None = None) -> None:
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: this library has no CPU fallback")
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().splats_create(_vp(s.cuda_stream), int(max_W), int(max_H)))
+
+
+def splats_update(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, H: int, r_scale: float) -> None:
+    c = _cam(src_camera)
+    _check(lib().splats_update(_dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H),
+                               ctypes.byref(c), int(W), int(H), float(r_scale)))
+
+
+def splats_render(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
+    c = _cam(dst_camera)
+    _check(lib().splats_render(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
+
+
+def splats_update_host(color, depth, src_camera, W: int, H: int, r_scale: float) -> None:
+    c = _cam(src_camera)
+    _check(lib().splats_update_host(_host_ptr(color, W * H * 4), _host_ptr(depth, W * H), ctypes.byref(c),
+                                    int(W), int(H), float(r_scale)))
+
+
+def splats_render_host(dst_camera, W2: int, H2: int, out_rgba) -> None:
+    c = _cam(dst_camera)
+    _check(lib().splats_render_host(ctypes.byref(c), int(W2), int(H2), _host_ptr(out_rgba, W2 * H2 * 4)))
+
+
+def splats_count() -> int:
+    n = ctypes.c_uint(0)
+    _check(lib().splats_count(ctypes.byref(n)))
+    return int(n.value)
+
+
+def splats_export():
+    """dict of CUDA tensors: keys (int64 view of uint64), perm, children, parents, node_aabbs."""
+    n = splats_count()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    keys = torch.empty(n, dtype=torch.int64, device=dev)
+    perm = torch.empty(n, dtype=torch.int32, device=dev)
+    children = torch.empty((max(n - 1, 0), 2), dtype=torch.int32, device=dev)
+    parents = torch.empty(max(2 * n - 1, 0), dtype=torch.int32, device=dev)
+    aabbs = torch.empty((max(2 * n - 1, 0), 6), dtype=torch.float32, device=dev)
+    if n:
+        _check(lib().splats_export(keys.data_ptr(), perm.data_ptr(), children.data_ptr() if n > 1 else None,
+                                   parents.data_ptr(), aabbs.data_ptr()))
+    return dict(N=n, keys=keys, perm=perm, children=children, parents=parents, node_aabbs=aabbs)
+
+
+def splats_export_splats():
+    n = splats_count()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    sphere = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    rgba = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    lo_hi = torch.empty(6, dtype=torch.float32, device=dev)
+    _check(lib().splats_export_splats(sphere.data_ptr() if n else None, rgba.data_ptr() if n else None,
+                                      lo_hi.data_ptr()))
+    return dict(N=n, sphere=sphere, rgba=rgba, lo_hi=lo_hi)
+
+
+def splats_set_profiling(on: bool) -> None:
+    _check(lib().splats_set_profiling(1 if on else 0))
+
+
+def splats_stage_ms() -> dict:
+    ms = (ctypes.c_float * NUM_STAGES)()
+    _check(lib().splats_stage_ms(ms))
+    return {name: float(ms[i]) for i, name in enumerate(STAGE_NAMES)}
+
+
+def splats_launch_count() -> int:
+    return int(lib().splats_launch_count())
+
+
+def splats_synchronize() -> None:
+    _check(lib().splats_synchronize())
+
+
+def splats_last_error() -> str:
+    return lib().splats_last_error().decode()
+
+
+def splats_destroy() -> None:
+    lib().splats_destroy()

@@ -1,0 +1,108 @@
+// common.cuh -- shared device types and helpers of the splat-warp kernels (sm_100a).
+//
+// Arithmetic contract: every float32 operation that decides an integer
+// (Morton code), a hit or a composited value is written with the explicit round-to-nearest
+// intrinsics below, so nvcc can neither contract a*b+c into an FMA nor split an FMA that the
+// spec asks for.  Slab tests are free (only conservative) and use ordinary operators.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sw {
+
+// ---- explicit IEEE float32 ops
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float div_(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float sqrt_(float a) { return __fsqrt_rn(a); }
+
+// ---- camera as kernel parameter (host fills the derived constants in float32)
+struct DevCamera {
+  float e[3], R[3], U[3], F[3];
+  float tau;    // tan(fovy/2)
+  float ta;     // fl(fl(tau*W)/H): horizontal half extent
+  float fW, fH; // (float)W, (float)H
+  int W, H;
+};
+
+// Ray through the centre of pixel (x, y), row 0 = top (Eq. 1's d):
+// d = F + u R + v U, returned normalised together with the un-normalised length.
+__device__ __forceinline__ void pixel_ray(const DevCamera& c, int x, int y, float d[3], float& len) {
+  float nx = div_(__int2float_rn(2 * x + 1 - c.W), c.fW);
+  float ny = div_(__int2float_rn(c.H - 2 * y - 1), c.fH);
+  float u = mul_(nx, c.ta);
+  float v = mul_(ny, c.tau);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) d[k] = fma_(v, c.U[k], fma_(u, c.R[k], c.F[k]));
+  len = sqrt_(fma_(d[2], d[2], fma_(d[1], d[1], mul_(d[0], d[0]))));
+#pragma unroll
+  for (int k = 0; k < 3; ++k) d[k] = div_(d[k], len);
+}
+
+__device__ __forceinline__ bool depth_valid(float t) {  // zero-radius samples are dropped
+  return (t > 0.0f) && (t < __int_as_float(0x7f800000));
+}
+
+// Eq. 1: p = o + d t.
+__device__ __forceinline__ void splat_centre(const DevCamera& c, int x, int y, float t, float p[3], float& len) {
+  float d[3];
+  pixel_ray(c, x, y, d, len);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) p[k] = fma_(t, d[k], c.e[k]);
+}
+
+// ---- order-preserving float <-> uint32 map for atomicMin / atomicMax
+__device__ __forceinline__ uint32_t f2ord(float f) {
+  uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(uint32_t u) {
+  return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+}
+
+// ---- per-frame device state, double buffered by frame parity so that frame f can reset
+// the accumulators of frame f+1 without a race or an extra launch.
+struct FrameState {
+  uint32_t lo[3];      // ordered-uint min of valid centres   (init 0xffffffff)
+  uint32_t hi[3];      // ordered-uint max                     (init 0)
+  uint32_t n;          // number of valid splats               (init 0)
+  uint32_t pad0;
+  float root_lo[3];    // AABB of the whole scene (root node box), written by refit
+  float root_hi[3];
+  uint32_t pad1[2];
+  uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
+};
+
+// 64-byte BVH node: both child boxes live in the parent, so one node fetch (four 16-byte
+// vector loads from one 64-byte-aligned record) tests both children.
+//   b[0..5]  left child box  lo xyz, hi xyz      b[6..11] right child box
+//   left/right: >= 0 internal node index, < 0: ~leaf (leaf = sorted position)
+//   parent: (parent index << 1) | is_right_child, -1 for the root
+//   flag: arrival counter of the bottom-up refit
+struct __align__(64) Node {
+  float b[12];
+  int left, right;
+  int parent;
+  unsigned flag;
+};
+static_assert(sizeof(Node) == 64, "node record must be 64 bytes");
+
+__device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) {
+  uint64_t v;
+  asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void st_volatile_u64(uint64_t* p, uint64_t v) {
+  asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+__device__ __forceinline__ float4 ldg_stream_f4(const float4* p) {  // read-once data: do not keep in L1
+  float4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+  return r;
+}
+
+}  // namespace sw

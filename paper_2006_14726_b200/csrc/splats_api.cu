@@ -1,0 +1,392 @@
+// splats_api.cu -- host side of the C ABI declared in include/splats.h: one context that owns
+// all device memory, argument checks, and the kernel launch sequence of the two hot calls.
+// Nothing here computes on the CPU except the per-call camera constants; there is no CPU
+// fallback (every entry point fails with SPLATS_ECUDA / SPLATS_ESTATE without a device).
+#include "../../include/splats.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "build_kernels.cuh"
+#include "common.cuh"
+#include "lbvh.cuh"
+#include "onesweep.cuh"
+#include "render.cuh"
+
+namespace {
+
+using namespace sw;
+
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
+
+struct Context {
+  cudaStream_t stream = nullptr;
+  int max_w = 0, max_h = 0;
+  int64_t cap = 0;
+  int num_sms = 0;
+  // device memory
+  FrameState* state = nullptr;      // [2], by frame parity
+  uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
+  uint64_t* key[2] = {nullptr, nullptr};
+  uint32_t* val[2] = {nullptr, nullptr};
+  uint64_t* status = nullptr;       // [max sort tiles][256]
+  float4* sphere = nullptr;
+  float4* rgba = nullptr;
+  Node* nodes = nullptr;
+  int* leaf_parent = nullptr;
+  float* stage_color = nullptr;     // staging for the *_host calls
+  float* stage_depth = nullptr;
+  float* stage_out = nullptr;
+  // frame bookkeeping
+  unsigned frame = 0;               // number of updates enqueued
+  int parity = 0;                   // FrameState of the latest update
+  uint32_t epoch = 0;
+  bool has_bvh = false;
+  int sort_grid = 0;
+  size_t sort_smem = 0;
+  // profiling
+  bool profiling = false;
+  cudaEvent_t ev[8] = {};
+  bool ev_update_valid = false, ev_render_valid = false;
+  unsigned long long launches = 0;
+};
+
+Context* g_ctx = nullptr;
+std::string g_err = "";
+
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+  return fail(SPLATS_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call)                                   \
+  do {                                             \
+    cudaError_t e_ = (call);                       \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+bool finite_camera(const wr_camera* c) {
+  const float* f = reinterpret_cast<const float*>(c);
+  for (int i = 0; i < 13; ++i)
+    if (!std::isfinite(f[i])) return false;
+  return c->tan_half_fovy > 0.0f;
+}
+
+DevCamera make_camera(const wr_camera* c, int W, int H) {
+  DevCamera d;
+  for (int k = 0; k < 3; ++k) { d.e[k] = c->eye[k]; d.R[k] = c->right[k]; d.U[k] = c->up[k]; d.F[k] = c->fwd[k]; }
+  d.tau = c->tan_half_fovy;
+  d.fW = (float)W;
+  d.fH = (float)H;
+  volatile float tw = d.tau * d.fW;  // two separately rounded float32 operations
+  d.ta = tw / d.fH;
+  d.W = W;
+  d.H = H;
+  return d;
+}
+
+// k_r = r_scale * sqrt(1/2) * (2 tau / H), each product / quotient rounded to float32.
+float radius_factor(const wr_camera* c, int H, float r_scale) {
+  const float SQRT_HALF = 0.70710678118654752440f;
+  volatile float a = r_scale * SQRT_HALF;
+  volatile float b = 2.0f * c->tan_half_fovy;
+  volatile float q = b / (float)H;
+  return a * q;
+}
+
+template <typename T>
+cudaError_t dmalloc(T** p, size_t count) {
+  return cudaMalloc(reinterpret_cast<void**>(p), count * sizeof(T));
+}
+
+void free_all(Context* c) {
+  cudaFree(c->state); cudaFree(c->tile_count);
+  cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
+  cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
+  cudaFree(c->leaf_parent); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
+  for (auto& e : c->ev)
+    if (e) cudaEventDestroy(e);
+}
+
+int ensure_staging(Context* c) {
+  if (!c->stage_color) {
+    CU(dmalloc(&c->stage_color, (size_t)c->cap * 4));
+    CU(dmalloc(&c->stage_depth, (size_t)c->cap));
+    CU(dmalloc(&c->stage_out, (size_t)c->cap * 4));
+  }
+  return SPLATS_OK;
+}
+
+int do_update(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale) {
+  const int64_t P = (int64_t)W * H;
+  const DevCamera dc = make_camera(cam, W, H);
+  const float k_r = radius_factor(cam, H, r_scale);
+  const int parity = (int)(c->frame & 1u);
+  FrameState* st = c->state + parity;
+  FrameState* st_next = c->state + (parity ^ 1);
+  const int tiles = (int)((P + TILE_PX - 1) / TILE_PX);
+  cudaStream_t s = c->stream;
+  const bool prof = c->profiling;
+
+  if (prof) cudaEventRecord(c->ev[0], s);
+  bounds_kernel<<<tiles, BUILD_THREADS, 0, s>>>(depth, P, dc, st, c->tile_count);
+  if (prof) cudaEventRecord(c->ev[1], s);
+  const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
+  unproject_kernel<<<grid2, BUILD_THREADS, 0, s>>>(depth, P, tiles, dc, st, st_next, c->tile_count, c->key[0], c->val[0]);
+  if (prof) cudaEventRecord(c->ev[2], s);
+  const int max_sort_tiles = (int)((P + SORT_TILE - 1) / SORT_TILE);
+  const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
+  for (int pass = 0; pass < 8; ++pass) {
+    const int in = pass & 1;
+    onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(
+        c->key[in], c->val[in], c->key[in ^ 1], c->val[in ^ 1], st, pass, c->status, ++c->epoch);
+  }
+  if (prof) cudaEventRecord(c->ev[3], s);
+  const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
+  const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
+  emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
+                                             k_r, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
+  if (prof) cudaEventRecord(c->ev[4], s);
+  refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
+  if (prof) cudaEventRecord(c->ev[5], s);
+  c->launches += 12;
+  c->ev_update_valid = prof;
+  CU(cudaGetLastError());
+  c->parity = parity;
+  c->frame += 1;
+  c->has_bvh = true;
+  return SPLATS_OK;
+}
+
+int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out) {
+  RenderParams prm;
+  prm.cam = make_camera(cam, W2, H2);
+  prm.nodes = c->nodes;
+  prm.sphere = c->sphere;
+  prm.rgba = c->rgba;
+  prm.ids = c->val[0];
+  prm.st = c->state + c->parity;
+  prm.out = reinterpret_cast<float4*>(out);
+  dim3 grid((W2 + 15) / 16, (H2 + 7) / 8);
+  if (c->profiling) cudaEventRecord(c->ev[6], c->stream);
+  render_kernel<<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  if (c->profiling) cudaEventRecord(c->ev[7], c->stream);
+  c->ev_render_valid = c->profiling;
+  c->launches += 1;
+  CU(cudaGetLastError());
+  return SPLATS_OK;
+}
+
+int check_frame_args(Context* c, const void* a, const void* b, const wr_camera* cam, int W, int H) {
+  if (!c) return fail(SPLATS_ESTATE, "no context: call splats_create first");
+  if (!a || !b || !cam) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (W <= 0 || H <= 0 || (int64_t)W * H > c->cap) return fail(SPLATS_EINVAL, "W*H outside [1, capacity]");
+  if (!finite_camera(cam)) return fail(SPLATS_EINVAL, "camera is not finite or tan_half_fovy <= 0");
+  return SPLATS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int splats_create(void* cuda_stream, int max_W, int max_H) {
+  if (g_ctx) return fail(SPLATS_ESTATE, "context already exists: call splats_destroy first");
+  if (max_W <= 0 || max_H <= 0 || (int64_t)max_W * max_H > (1ll << 28))
+    return fail(SPLATS_EINVAL, "max_W*max_H outside [1, 2^28]");
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  Context* c = new Context();
+  c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  c->max_w = max_W;
+  c->max_h = max_H;
+  c->cap = (int64_t)max_W * max_H;
+  cudaError_t e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const size_t cap = (size_t)c->cap;
+  const size_t max_sort_tiles = (cap + SORT_TILE - 1) / SORT_TILE;
+  if (e == cudaSuccess) e = dmalloc(&c->state, 2);
+  if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
+  for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+    e = dmalloc(&c->key[i], cap);
+    if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
+  }
+  if (e == cudaSuccess) e = dmalloc(&c->status, max_sort_tiles * RADIX);
+  if (e == cudaSuccess) e = dmalloc(&c->sphere, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->rgba, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->nodes, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
+  if (e == cudaSuccess) e = cudaMemset(c->status, 0, max_sort_tiles * RADIX * sizeof(uint64_t));
+  if (e == cudaSuccess) {
+    FrameState init;
+    memset(&init, 0, sizeof(init));
+    for (int a = 0; a < 3; ++a) init.lo[a] = 0xffffffffu;
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i)
+      e = cudaMemcpy(c->state + i, &init, sizeof(init), cudaMemcpyHostToDevice);
+  }
+  if (e == cudaSuccess) {
+    c->sort_smem = sizeof(SortSmem<SORT_ITEMS>);
+    e = cudaFuncSetAttribute(onesweep_kernel<SORT_ITEMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem);
+  }
+  int occ = 0;
+  if (e == cudaSuccess)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onesweep_kernel<SORT_ITEMS>, SORT_THREADS, c->sort_smem);
+  if (e == cudaSuccess && occ < 1) { free_all(c); delete c; return fail(SPLATS_ECUDA, "onesweep kernel does not fit on an SM"); }
+  for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
+  if (e != cudaSuccess) {
+    free_all(c);
+    delete c;
+    return cuda_fail(e, "splats_create");
+  }
+  c->sort_grid = c->num_sms * occ;  // co-resident persistent grid (see onesweep.cuh)
+  g_ctx = c;
+  return SPLATS_OK;
+}
+
+int splats_update(const float* color, const float* depth, const wr_camera* src_camera, int W, int H, float r_scale) {
+  int rc = check_frame_args(g_ctx, color, depth, src_camera, W, H);
+  if (rc) return rc;
+  if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
+  if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
+    return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
+  return do_update(g_ctx, color, depth, src_camera, W, H, r_scale);
+}
+
+int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba) {
+  int rc = check_frame_args(g_ctx, out_rgba, out_rgba, dst_camera, W2, H2);
+  if (rc) return rc;
+  if (reinterpret_cast<uintptr_t>(out_rgba) & 15u) return fail(SPLATS_EINVAL, "out_rgba must be 16-byte aligned");
+  if (!g_ctx->has_bvh) return fail(SPLATS_ENOBVH, "splats_render before any splats_update");
+  return do_render(g_ctx, dst_camera, W2, H2, out_rgba);
+}
+
+int splats_update_host(const float* color_host, const float* depth_host, const wr_camera* src_camera, int W, int H,
+                       float r_scale) {
+  int rc = check_frame_args(g_ctx, color_host, depth_host, src_camera, W, H);
+  if (rc) return rc;
+  if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
+  Context* c = g_ctx;
+  rc = ensure_staging(c);
+  if (rc) return rc;
+  const size_t P = (size_t)W * H;
+  CU(cudaMemcpyAsync(c->stage_color, color_host, P * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(c->stage_depth, depth_host, P * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+  return do_update(c, c->stage_color, c->stage_depth, src_camera, W, H, r_scale);
+}
+
+int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_rgba_host) {
+  int rc = check_frame_args(g_ctx, out_rgba_host, out_rgba_host, dst_camera, W2, H2);
+  if (rc) return rc;
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_host before any update");
+  rc = ensure_staging(c);
+  if (rc) return rc;
+  rc = do_render(c, dst_camera, W2, H2, c->stage_out);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(out_rgba_host, c->stage_out, (size_t)W2 * H2 * 4 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
+int splats_count(unsigned* n_host) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  if (!n_host) return fail(SPLATS_EINVAL, "null pointer argument");
+  Context* c = g_ctx;
+  if (!c->has_bvh) { *n_host = 0; return SPLATS_OK; }
+  CU(cudaMemcpyAsync(n_host, &c->state[c->parity].n, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
+int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* parents, float* node_aabbs) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export before any update");
+  unsigned n = 0;
+  int rc = splats_count(&n);
+  if (rc) return rc;
+  if (n == 0) return SPLATS_OK;
+  if (keys) CU(cudaMemcpyAsync(keys, c->key[0], (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream));
+  if (perm) CU(cudaMemcpyAsync(perm, c->val[0], (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
+  if (children || parents || node_aabbs) {
+    const int grid = (int)((n + LBVH_THREADS - 1) / LBVH_THREADS);
+    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->nodes, c->leaf_parent, c->sphere, c->state + c->parity,
+                                                        children, parents, node_aabbs);
+    c->launches += 1;
+    CU(cudaGetLastError());
+  }
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
+int splats_export_splats(float* sphere, float* rgba, float* lo_hi) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export_splats before any update");
+  unsigned n = 0;
+  int rc = splats_count(&n);
+  if (rc) return rc;
+  if (sphere && n) CU(cudaMemcpyAsync(sphere, c->sphere, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  if (rgba && n) CU(cudaMemcpyAsync(rgba, c->rgba, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  if (lo_hi) {
+    FrameState hs;
+    CU(cudaMemcpyAsync(&hs, c->state + c->parity, sizeof(uint32_t) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    float h[6];
+    for (int a = 0; a < 3; ++a) {
+      uint32_t ulo = hs.lo[a], uhi = hs.hi[a];
+      uint32_t blo = (ulo & 0x80000000u) ? (ulo & 0x7fffffffu) : ~ulo;
+      uint32_t bhi = (uhi & 0x80000000u) ? (uhi & 0x7fffffffu) : ~uhi;
+      memcpy(&h[a], &blo, 4);
+      memcpy(&h[3 + a], &bhi, 4);
+      if (n == 0) h[a] = h[3 + a] = 0.0f;
+    }
+    CU(cudaMemcpyAsync(lo_hi, h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+  }
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
+int splats_set_profiling(int on) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  g_ctx->profiling = on != 0;
+  g_ctx->ev_update_valid = g_ctx->ev_render_valid = false;
+  return SPLATS_OK;
+}
+
+int splats_stage_ms(float* ms) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  if (!ms) return fail(SPLATS_EINVAL, "null pointer argument");
+  Context* c = g_ctx;
+  CU(cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < SPLATS_NUM_STAGES; ++i) ms[i] = 0.0f;
+  if (c->ev_update_valid)
+    for (int i = 0; i < 5; ++i) CU(cudaEventElapsedTime(&ms[i], c->ev[i], c->ev[i + 1]));
+  if (c->ev_render_valid) CU(cudaEventElapsedTime(&ms[5], c->ev[6], c->ev[7]));
+  return SPLATS_OK;
+}
+
+unsigned long long splats_launch_count(void) { return g_ctx ? g_ctx->launches : 0ull; }
+
+int splats_synchronize(void) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  CU(cudaStreamSynchronize(g_ctx->stream));
+  return SPLATS_OK;
+}
+
+const char* splats_last_error(void) { return g_err.c_str(); }
+
+void splats_destroy(void) {
+  if (!g_ctx) return;
+  cudaStreamSynchronize(g_ctx->stream);
+  free_all(g_ctx);
+  delete g_ctx;
+  g_ctx = nullptr;
+}
+
+}  // extern "C"

@@ -1,0 +1,187 @@
+"""-m gpu: the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bar (BASELINE.json north_star): Morton codes, sorted permutation, tree topology and AABBs
+bit-exact; composited RGBA within 1e-3 per channel with at most 0.01 % of pixels beyond."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from gpu_common import Session, assert_bvh_bit_exact, assert_rgba_close, check_scene
+from paper_2006_14726_b200 import binding as sp
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config0_full_brute_force():
+    cfg = synth.make_config(0)
+    color, depth = synth.source_frame(cfg, 0)
+    with Session(cfg.W, cfg.H) as s:
+        sc, stats = check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale,
+                                cfg.dst_cams + cfg.src_cams, mode="brute")
+        # identity camera: bit-exact reproduction of the source image (closed form (iii))
+        got = s.render(cfg.src_cams[0], cfg.W, cfg.H)
+        v = depth > 0
+        assert np.array_equal(got[v], color[v]) and np.all(got[~v] == 0)
+
+
+@pytest.mark.parametrize("W,H,fill,r_scale", [
+    (33, 31, 0.9, 1.0), (48, 27, 0.6, 2.0), (127, 65, 0.3, 3.0), (256, 100, 0.6, 1.0), (7, 5, 1.0, 0.5),
+])
+def test_random_frames_ragged_sizes(W, H, fill, r_scale):
+    color, depth, cam = synth.random_frame(W, H, seed=W * 1000 + H, fill=fill)
+    dst = [synth.orbit_camera(5.0), synth.orbit_camera(-20.0, 10.0, 2.5), synth.orbit_camera(15.0, shift_right=0.4), cam]
+    sizes = [(W, H), (40, 30), (W + 3, H + 1), (W, H)]
+    with Session(max(W + 3, 40), max(H + 1, 30)) as s:
+        check_scene(s, color, depth, cam, W, H, r_scale, dst, sizes, mode="brute" if W * H < 6000 else "bvh")
+
+
+def test_low_alpha_stack_forces_relaunch():
+    # alpha 0.05 everywhere, r_scale 4: every ray needs far more than K = 8 hits
+    W, H = 40, 30
+    color, depth, cam = synth.random_frame(W, H, seed=5, fill=1.0)
+    color[..., 3] = 0.05
+    color[..., :3] *= 0.05
+    depth[...] = np.linspace(3.0, 3.4, W * H, dtype=np.float32).reshape(H, W)
+    with Session(W, H) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 4.0, [cam, synth.orbit_camera(3.0)], mode="brute")
+        _, used = oracle.render(sc, cam, W, H, "brute", return_hits=True)
+        assert used.max() > 16  # the oracle itself needed more than two k-buffers' worth
+
+
+def test_coaxial_stack_closed_form_90_hits():
+    # closed form (ii): alpha 0.05 -> 90 hits, A = 1 - 0.95^90.  A 1x1 source cannot produce
+    # coaxial splats, so use a frame whose splats all project onto the destination pixel.
+    W, H = 12, 12
+    color, depth, cam = synth.random_frame(W, H, seed=9, fill=1.0)
+    color[...] = np.array([0.01, 0.02, 0.03, 0.05], np.float32)
+    depth[...] = 3.0
+    with Session(W, H) as s:
+        s.update(color, depth, cam, W, H, 1.0)
+        far = synth.orbit_camera(0.0, 0.0, 400.0)   # all 144 splats fall inside one far pixel's ray
+        got = s.render(far, 1, 1)
+        sc = oracle.build_scene(color, depth, cam, W, H, 1.0)
+        ref, used = oracle.render(sc, far, 1, 1, "brute", return_hits=True)
+        assert_rgba_close(got, ref)
+        if used[0, 0] >= 90:
+            assert got[0, 0, 3] == pytest.approx(1 - 0.95 ** 90, abs=1e-5)
+
+
+def test_all_invalid_frame_renders_zeros():
+    W, H = 64, 48
+    color = np.ones((H, W, 4), np.float32)
+    depth = np.zeros((H, W), np.float32)
+    depth[3, 4] = np.nan
+    depth[5, 6] = -1.0
+    depth[7, 8] = np.inf
+    cam = synth.orbit_camera(0.0)
+    with Session(W, H) as s:
+        s.update(color, depth, cam, W, H, 1.0)
+        assert sp.splats_count() == 0
+        assert np.all(s.render(cam, W, H) == 0)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3])
+def test_tiny_splat_counts(n):
+    W, H = 9, 7
+    color, depth, cam = synth.random_frame(W, H, seed=n, fill=1.0)
+    keep = np.zeros(W * H, bool)
+    keep[[31, 32, 40][:n]] = True
+    depth.reshape(-1)[~keep] = 0
+    with Session(W, H) as s:
+        check_scene(s, color, depth, cam, W, H, 1.0, [cam, synth.orbit_camera(2.0)], mode="brute")
+
+
+def test_duplicate_morton_codes_from_outlier():
+    # one far outlier stretches the bounds so most centres collapse into a few cells
+    W, H = 64, 64
+    color, depth, cam = synth.random_frame(W, H, seed=21, fill=0.8)
+    depth[depth > 0] = 3.0
+    depth[0, 0] = 3.0e7
+    with Session(W, H) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(4.0)], mode="bvh")
+        codes = sc["sorted_codes"]
+        assert (codes[1:] == codes[:-1]).sum() > 100   # the case really has duplicates
+
+
+def test_zero_extent_axis():
+    # one-row image from an axis-aligned camera: every centre has exactly the eye's y
+    W, H = 200, 1
+    color, depth, cam = synth.random_frame(W, H, seed=4, fill=0.9)
+    with Session(W, 8) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [cam, synth.orbit_camera(1.0)], [(W, 1), (W, 8)], mode="brute")
+        assert sc["lo"][1] == sc["hi"][1]
+
+
+def test_config1_full():
+    cfg = synth.make_config(1)
+    color, depth = synth.source_frame(cfg, 0)
+    with Session(cfg.W, cfg.H) as s:
+        check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams, mode="bvh")
+
+
+def test_repeated_updates_and_size_changes():
+    # frame-parity double buffering: A, B (other size), A again must reproduce A
+    cfg = synth.make_config(0)
+    colorA, depthA = synth.source_frame(cfg, 0)
+    colorB, depthB, camB = synth.random_frame(100, 37, seed=77, fill=0.5)
+    dst = synth.orbit_camera(7.0)
+    with Session(128, 64) as s:
+        s.update(colorA, depthA, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
+        a1 = s.render(dst, 64, 64)
+        scB, _ = check_scene(s, colorB, depthB, camB, 100, 37, 2.0, [dst], [(80, 40)], mode="brute")
+        scA, _ = check_scene(s, colorA, depthA, cfg.src_cams[0], cfg.W, cfg.H, 1.0, [dst], mode="brute")
+        a2 = s.render(dst, 64, 64)
+        assert np.array_equal(a1, a2)
+
+
+def test_host_buffer_entry_points_match_device_ones():
+    cfg = synth.make_config(0)
+    color, depth = synth.source_frame(cfg, 0)
+    with Session(cfg.W, cfg.H) as s:
+        s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
+        a = s.render(cfg.dst_cams[0], 64, 64)
+        hc = torch.from_numpy(color).pin_memory()
+        hd = torch.from_numpy(depth).pin_memory()
+        ho = torch.empty((64, 64, 4), dtype=torch.float32).pin_memory()
+        sp.splats_update_host(hc, hd, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
+        sp.splats_render_host(cfg.dst_cams[0], 64, 64, ho)
+        assert np.array_equal(ho.numpy(), a)
+
+
+def test_error_codes():
+    cfg = synth.make_config(0)
+    color, depth = synth.source_frame(cfg, 0)
+    cam = cfg.src_cams[0]
+    with pytest.raises(sp.SplatsError) as e:
+        sp.splats_update(torch.zeros(16, device="cuda"), torch.zeros(4, device="cuda"), cam, 2, 2, 1.0)
+    assert e.value.code == -4   # no context
+    with Session(64, 64) as s:
+        out = torch.empty((64, 64, 4), device="cuda")
+        with pytest.raises(sp.SplatsError) as e:
+            sp.splats_render(cam, 64, 64, out)
+        assert e.value.code == -2   # no BVH yet
+        dc, dd = torch.from_numpy(color).cuda(), torch.from_numpy(depth).cuda()
+        for bad in (0.0, -1.0, float("nan"), float("inf")):
+            with pytest.raises(sp.SplatsError) as e:
+                sp.splats_update(dc, dd, cam, 64, 64, bad)
+            assert e.value.code == -1
+        badcam = cam.copy(); badcam[4] = np.nan
+        with pytest.raises(sp.SplatsError) as e:
+            sp.splats_update(dc, dd, badcam, 64, 64, 1.0)
+        assert e.value.code == -1
+        with pytest.raises(sp.SplatsError) as e:
+            sp._check(sp.lib().splats_update(dc.data_ptr(), dd.data_ptr(), None, 64, 64, 1.0))
+        assert e.value.code == -1
+        big = torch.zeros(65 * 64 * 4, device="cuda")
+        with pytest.raises(sp.SplatsError) as e:
+            sp.splats_update(big, big, cam, 65, 64, 1.0)   # beyond capacity
+        assert e.value.code == -1
+        with pytest.raises(sp.SplatsError) as e:
+            sp.splats_create(8, 8)                          # context already exists
+        assert e.value.code == -4
+        sp.splats_update(dc, dd, cam, 64, 64, 1.0)          # still usable after the errors
+        sp.splats_render(cam, 64, 64, out)
+        torch.cuda.synchronize()
+        assert "context" in sp.splats_last_error() or sp.splats_last_error() != ""
