@@ -6,7 +6,7 @@
 // One thread per destination pixel, one warp per 8x4 pixel tile, four warps (16x8 pixels)
 // per block.  Traversal keeps the K nearest hits beyond a cursor (t, id) in a register
 // k-buffer sorted by (t, id); after the walk they are composited in order, and if the ray is
-// not yet opaque (alpha < 0.99) while hits were dropped from the full k-buffer, the ray is
+// not yet opaque (alpha < 0.99) and the k-buffer was full (hits may have been dropped), the ray is
 // re-launched from the last composited (t, id).  The result is exactly "sort all hits by
 // (t, id), composite until alpha >= 0.99" (oracle step O9), whatever K is.
 //
@@ -36,12 +36,12 @@ struct RenderParams {
 struct KBuffer {
   float t[KBUF];
   uint32_t leaf[KBUF];
-  bool overflow;
   __device__ __forceinline__ void clear() {
 #pragma unroll
     for (int i = 0; i < KBUF; ++i) { t[i] = __int_as_float(0x7f800000); leaf[i] = EMPTY_LEAF; }
-    overflow = false;
   }
+  // A full buffer may have dropped hits (evicted here, or culled by the t <= t[K-1] bound).
+  __device__ __forceinline__ bool full() const { return leaf[KBUF - 1] != EMPTY_LEAF; }
   // sorted insertion by (t, id); the largest entry falls out when the buffer is full
   __device__ __forceinline__ void insert(float ct, uint32_t cl, const uint32_t* __restrict__ ids) {
 #pragma unroll
@@ -53,7 +53,6 @@ struct KBuffer {
         const uint32_t tl = leaf[i]; leaf[i] = cl; cl = tl;
       }
     }
-    if (cl != EMPTY_LEAF) overflow = true;
   }
 };
 
@@ -169,7 +168,7 @@ render_kernel(RenderParams prm) {
           if (A >= 0.99f) opaque = true;
         }
       }
-      if (opaque || !kb.overflow) {
+      if (opaque || !kb.full()) {
         finished = true;
       } else {  // re-launch from the last composited hit
         cur_t = kb.t[KBUF - 1];
