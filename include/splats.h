@@ -108,13 +108,16 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
  * lo_hi: 6 float32.  Synchronises.  Parity/debug only. */
 int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 
-/* Per-stage device times of the latest update/render, measured with CUDA events on the
- * library's stream.  Off by default (the events cost a few microseconds).
- * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all passes), 3 hierarchy+gather,
- * 4 refit, 5 render.  Synchronises the stream. */
+/* Per-stage device times, measured with CUDA events recorded on the library's stream around
+ * each stage of every update / render issued while profiling is on.  Off by default (the
+ * event records cost about a microsecond each).  splats_stage_ms synchronises the stream,
+ * returns for each stage the SUM of its durations in milliseconds and how many times it ran
+ * since profiling was switched on or since the previous query, and clears the record.
+ * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 hierarchy+gather,
+ * 4 refit, 5 render.  calls may be NULL. */
 #define SPLATS_NUM_STAGES 6
 int splats_set_profiling(int on);
-int splats_stage_ms(float* ms /* host, SPLATS_NUM_STAGES floats */);
+int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);
 
 /* How many kernels this library has launched since splats_create. */
 unsigned long long splats_launch_count(void);

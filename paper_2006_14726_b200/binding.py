@@ -53,7 +53,7 @@ def lib() -> ctypes.CDLL:
         L.splats_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
         L.splats_export_splats.argtypes = [_vp, _vp, _vp]
         L.splats_set_profiling.argtypes = [_ci]
-        L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float)]
+        L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_uint)]
         L.splats_launch_count.restype = ctypes.c_ulonglong
         L.splats_last_error.restype = ctypes.c_char_p
         L.splats_destroy.restype = None
@@ -159,9 +159,11 @@ def splats_set_profiling(on: bool) -> None:
 
 
 def splats_stage_ms() -> dict:
+    """{stage name: (sum of durations in ms, number of runs)} since the last query."""
     ms = (ctypes.c_float * NUM_STAGES)()
-    _check(lib().splats_stage_ms(ms))
-    return {name: float(ms[i]) for i, name in enumerate(STAGE_NAMES)}
+    calls = (ctypes.c_uint * NUM_STAGES)()
+    _check(lib().splats_stage_ms(ms, calls))
+    return {name: (float(ms[i]), int(calls[i])) for i, name in enumerate(STAGE_NAMES)}
 
 
 def splats_launch_count() -> int:

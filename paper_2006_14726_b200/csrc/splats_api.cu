@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "build_kernels.cuh"
 #include "common.cuh"
@@ -49,9 +50,21 @@ struct Context {
   size_t sort_smem = 0;
   // profiling
   bool profiling = false;
-  cudaEvent_t ev[8] = {};
-  bool ev_update_valid = false, ev_render_valid = false;
+  std::vector<cudaEvent_t> pool;    // events, grown on demand while profiling is on
+  size_t pool_used = 0;
+  struct Span { int stage; size_t e0, e1; };
+  std::vector<Span> spans;          // one per (call, stage) since the last splats_stage_ms
   unsigned long long launches = 0;
+
+  size_t mark() {                   // record the next pooled event on the stream
+    if (pool_used == pool.size()) {
+      cudaEvent_t e = nullptr;
+      cudaEventCreate(&e);
+      pool.push_back(e);
+    }
+    cudaEventRecord(pool[pool_used], stream);
+    return pool_used++;
+  }
 };
 
 Context* g_ctx = nullptr;
@@ -111,7 +124,7 @@ void free_all(Context* c) {
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
   cudaFree(c->leaf_parent); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
-  for (auto& e : c->ev)
+  for (auto& e : c->pool)
     if (e) cudaEventDestroy(e);
 }
 
@@ -135,12 +148,13 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   cudaStream_t s = c->stream;
   const bool prof = c->profiling;
 
-  if (prof) cudaEventRecord(c->ev[0], s);
+  size_t m[6] = {0, 0, 0, 0, 0, 0};
+  if (prof) m[0] = c->mark();
   bounds_kernel<<<tiles, BUILD_THREADS, 0, s>>>(depth, P, dc, st, c->tile_count);
-  if (prof) cudaEventRecord(c->ev[1], s);
+  if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
   unproject_kernel<<<grid2, BUILD_THREADS, 0, s>>>(depth, P, tiles, dc, st, st_next, c->tile_count, c->key[0], c->val[0]);
-  if (prof) cudaEventRecord(c->ev[2], s);
+  if (prof) m[2] = c->mark();
   const int max_sort_tiles = (int)((P + SORT_TILE - 1) / SORT_TILE);
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
   for (int pass = 0; pass < 8; ++pass) {
@@ -148,16 +162,17 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
     onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(
         c->key[in], c->val[in], c->key[in ^ 1], c->val[in ^ 1], st, pass, c->status, ++c->epoch);
   }
-  if (prof) cudaEventRecord(c->ev[3], s);
+  if (prof) m[3] = c->mark();
   const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
   const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
   emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
                                              k_r, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
-  if (prof) cudaEventRecord(c->ev[4], s);
+  if (prof) m[4] = c->mark();
   refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
-  if (prof) cudaEventRecord(c->ev[5], s);
+  if (prof) m[5] = c->mark();
   c->launches += 12;
-  c->ev_update_valid = prof;
+  if (prof)
+    for (int i = 0; i < 5; ++i) c->spans.push_back({i, m[i], m[i + 1]});
   CU(cudaGetLastError());
   c->parity = parity;
   c->frame += 1;
@@ -175,10 +190,10 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out) {
   prm.st = c->state + c->parity;
   prm.out = reinterpret_cast<float4*>(out);
   dim3 grid((W2 + 15) / 16, (H2 + 7) / 8);
-  if (c->profiling) cudaEventRecord(c->ev[6], c->stream);
+  size_t m0 = 0;
+  if (c->profiling) m0 = c->mark();
   render_kernel<<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
-  if (c->profiling) cudaEventRecord(c->ev[7], c->stream);
-  c->ev_render_valid = c->profiling;
+  if (c->profiling) c->spans.push_back({5, m0, c->mark()});
   c->launches += 1;
   CU(cudaGetLastError());
   return SPLATS_OK;
@@ -237,7 +252,6 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (e == cudaSuccess)
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onesweep_kernel<SORT_ITEMS>, SORT_THREADS, c->sort_smem);
   if (e == cudaSuccess && occ < 1) { free_all(c); delete c; return fail(SPLATS_ECUDA, "onesweep kernel does not fit on an SM"); }
-  for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
   if (e != cudaSuccess) {
     free_all(c);
     delete c;
@@ -355,19 +369,25 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi) {
 int splats_set_profiling(int on) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   g_ctx->profiling = on != 0;
-  g_ctx->ev_update_valid = g_ctx->ev_render_valid = false;
+  g_ctx->spans.clear();
+  g_ctx->pool_used = 0;
   return SPLATS_OK;
 }
 
-int splats_stage_ms(float* ms) {
+int splats_stage_ms(float* ms_sum, unsigned* calls) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
-  if (!ms) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (!ms_sum) return fail(SPLATS_EINVAL, "null pointer argument");
   Context* c = g_ctx;
   CU(cudaStreamSynchronize(c->stream));
-  for (int i = 0; i < SPLATS_NUM_STAGES; ++i) ms[i] = 0.0f;
-  if (c->ev_update_valid)
-    for (int i = 0; i < 5; ++i) CU(cudaEventElapsedTime(&ms[i], c->ev[i], c->ev[i + 1]));
-  if (c->ev_render_valid) CU(cudaEventElapsedTime(&ms[5], c->ev[6], c->ev[7]));
+  for (int i = 0; i < SPLATS_NUM_STAGES; ++i) { ms_sum[i] = 0.0f; if (calls) calls[i] = 0; }
+  for (const auto& sp : c->spans) {
+    float ms = 0.0f;
+    CU(cudaEventElapsedTime(&ms, c->pool[sp.e0], c->pool[sp.e1]));
+    ms_sum[sp.stage] += ms;
+    if (calls) calls[sp.stage] += 1;
+  }
+  c->spans.clear();
+  c->pool_used = 0;
   return SPLATS_OK;
 }
 

@@ -1,0 +1,66 @@
+"""-m gpu: parity at BASELINE.json's full sizes (configs 2, 3, 4), in the launch configuration
+bench.py times.  The BVH is compared in full (bit-exact); images are compared in full where the
+oracle's BVH walk finishes in seconds, else on seeded random pixel samples, and always
+spot-checked against the brute-force definition on a smaller sample."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from gpu_common import Session, assert_bvh_bit_exact, assert_rgba_close
+
+pytestmark = pytest.mark.gpu
+
+
+def _check_renders(s, sc, cams, W, H, full, n_bvh, n_brute, seed):
+    for i, cam in enumerate(cams):
+        got = s.render(cam, W, H)
+        rng = np.random.default_rng(seed + i)
+        if full:
+            ref = oracle.render(sc, cam, W, H, "bvh")
+            assert_rgba_close(got, ref, f"camera {i} full frame")
+            assert (ref[..., 3] > 0).mean() > 0.01
+        else:
+            px = rng.choice(W * H, size=n_bvh, replace=False).astype(np.int64)
+            assert_rgba_close(got.reshape(-1, 4)[px], oracle.render(sc, cam, W, H, "bvh", pixels=px), f"camera {i} sampled")
+        # brute-force spot check, biased towards covered pixels
+        covered = np.nonzero(got.reshape(-1, 4)[:, 3] > 0)[0]
+        px = np.concatenate([rng.choice(covered, size=min(n_brute, covered.size), replace=False),
+                             rng.choice(W * H, size=n_brute // 4, replace=False)]).astype(np.int64)
+        assert_rgba_close(got.reshape(-1, 4)[px], oracle.render(sc, cam, W, H, "brute", pixels=px), f"camera {i} brute")
+
+
+def test_config2_full_size():
+    cfg = synth.make_config(2)
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+    with Session(cfg.W, cfg.H) as s:
+        s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+        assert_bvh_bit_exact(sc)
+        _check_renders(s, sc, [cfg.dst_cams[i] for i in (0, 29, 59)], cfg.W, cfg.H, True, 0, 256, 20)
+
+
+@pytest.mark.parametrize("build", [0, 7, 14])
+def test_config3_full_size(build):
+    cfg = synth.make_config(3)
+    color, depth = synth.source_frame(cfg, build)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[build], cfg.W, cfg.H, cfg.r_scale)
+    cams = [cfg.dst_cams[4 * build + j] for j in (0, 3)]
+    with Session(cfg.W, cfg.H) as s:
+        s.update(color, depth, cfg.src_cams[build], cfg.W, cfg.H, cfg.r_scale)
+        assert_bvh_bit_exact(sc)
+        _check_renders(s, sc, cams, cfg.W, cfg.H, True, 0, 256, 30 + build)
+        # frame 4*build is rendered from its own source camera: identity reprojection
+        got = s.render(cfg.dst_cams[4 * build], cfg.W, cfg.H)
+        v = depth > 0
+        assert np.array_equal(got[v], color[v]) and np.all(got[~v] == 0)
+
+
+def test_config4_full_size():
+    cfg = synth.make_config(4)
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+    with Session(cfg.W, cfg.H) as s:
+        s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+        assert_bvh_bit_exact(sc)
+        _check_renders(s, sc, cfg.dst_cams, cfg.W, cfg.H, False, 200_000, 192, 40)
