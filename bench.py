@@ -144,17 +144,14 @@ class ClockSampler:
 # --------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     from paper_2006_14726_b200 import binding as sp
+    from paper_2006_14726_b200 import replicas
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local_rank = replicas.world_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    replicas.init("nccl")
     assert world == args.gpus or world == 1, f"--gpus {args.gpus} but WORLD_SIZE={world}"
 
     cfg, frames = make_workload(args.config, args.groups)
@@ -173,11 +170,7 @@ def run_ours(args):
         for j, cam in enumerate(f["dst_cams"]):
             sp.splats_render(cam, W, H, d_out[j])
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
+    barrier = replicas.barrier
 
     def timed(fn, K: int) -> float:
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -187,12 +180,7 @@ def run_ours(args):
             fn(k)
         e1.record()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return replicas.max_over_ranks(e0.elapsed_time(e1))
 
     K, Wm = args.steps, args.warmup
     for k in range(Wm):
@@ -289,9 +277,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg, frames)
     sp.splats_destroy()
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
+    replicas.shutdown()
     if rank == 0:
         print(json.dumps(out), flush=True)
 
