@@ -33,6 +33,16 @@ struct RenderParams {
   float4* out;
 };
 
+#ifdef SPLATS_STATS
+// Debug build only (-DSPLATS_STATS): traversal counters, read back with splats_debug_stats().
+__device__ unsigned long long g_stats[8];  // 0 node visits, 1 leaf tests, 2 hits kept, 3 passes, 4 rays past root, 5 max stack
+#define STAT_ADD(i, v) atomicAdd(&g_stats[i], (unsigned long long)(v))
+#define STAT_MAX(i, v) atomicMax(&g_stats[i], (unsigned long long)(v))
+#else
+#define STAT_ADD(i, v)
+#define STAT_MAX(i, v)
+#endif
+
 struct KBuffer {
   float t[KBUF];
   uint32_t leaf[KBUF];
@@ -104,10 +114,12 @@ render_kernel(RenderParams prm) {
     if (!finished) {
       kb.clear();
       const float t_lo = fmaxf(cur_t, 0.0f);
+      STAT_ADD(3, 1);
 
       auto test_leaf = [&](uint32_t leaf) {
         const float4 s = __ldg(prm.sphere + leaf);
         float t;
+        STAT_ADD(1, 1);
         if (ray_sphere(o, d, s, t)) {
           if (t > cur_t || (t == cur_t && __ldg(prm.ids + leaf) > cur_id)) kb.insert(t, leaf, prm.ids);
         }
@@ -120,6 +132,8 @@ render_kernel(RenderParams prm) {
         while (true) {
           const float4* np = reinterpret_cast<const float4*>(prm.nodes + node);
           const float4 n0 = __ldg(np), n1 = __ldg(np + 1), n2 = __ldg(np + 2), n3 = __ldg(np + 3);
+          STAT_ADD(0, 1);
+          STAT_MAX(5, sp);
           const float t_hi = kb.t[KBUF - 1];
           // left box: lo (n0.x n0.y n0.z) hi (n0.w n1.x n1.y); right box: lo (n1.z n1.w n2.x) hi (n2.y n2.z n2.w)
           float a0 = (n0.x - op[0]) * idir[0], a1 = (n0.w - om[0]) * idir[0];

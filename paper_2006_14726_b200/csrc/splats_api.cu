@@ -399,6 +399,19 @@ int splats_synchronize(void) {
   return SPLATS_OK;
 }
 
+#ifdef SPLATS_STATS
+int splats_debug_stats(unsigned long long* out8, int reset) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  CU(cudaStreamSynchronize(g_ctx->stream));
+  CU(cudaMemcpyFromSymbol(out8, sw::g_stats, sizeof(unsigned long long) * 8));
+  if (reset) {
+    unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    CU(cudaMemcpyToSymbol(sw::g_stats, z, sizeof(z)));
+  }
+  return SPLATS_OK;
+}
+#endif
+
 const char* splats_last_error(void) { return g_err.c_str(); }
 
 void splats_destroy(void) {
