@@ -50,7 +50,7 @@ typedef struct {
   float tan_half_fovy;
 } wr_camera;
 
-/* Allocate all device memory for source frames of up to max_W*max_H pixels (<= 2^28) and
+/* Allocate all device memory for source frames of up to max_W*max_H pixels (< 2^26) and
  * destination images of up to the same pixel count.  cuda_stream: a cudaStream_t (NULL = the
  * legacy default stream) on which every later call enqueues its work. */
 int splats_create(void* cuda_stream, int max_W, int max_H);

@@ -78,9 +78,22 @@ struct FrameState {
 // 64-byte BVH node: both child boxes live in the parent, so one node fetch (four 16-byte
 // vector loads from one 64-byte-aligned record) tests both children.
 //   b[0..5]  left child box  lo xyz, hi xyz      b[6..11] right child box
-//   left/right: >= 0 internal node index, < 0: ~leaf (leaf = sorted position)
+//   left/right: traversal links.  >= 0: internal node index (Karras numbering).  < 0: a
+//     *leaf range*: the child subtree covers <= LEAF_MAX consecutive splats of the sorted
+//     order, first | (count - 1) << 26 | 1 << 31; the traversal tests those spheres directly
+//     instead of walking the subtree (a sphere test is far cheaper than a node visit).  The
+//     canonical Karras links are recovered from the code: a range of 1 is the leaf `first`,
+//     a longer left (right) range is internal node first + count - 1 (first).
 //   parent: (parent index << 1) | is_right_child, -1 for the root
 //   flag: arrival counter of the bottom-up refit
+constexpr int LEAF_MAX = 8;                  // <= 32 (5-bit count field)
+constexpr uint32_t LEAF_FIRST_MASK = (1u << 26) - 1;  // capacity: 2^26 - 1 splats
+__host__ __device__ __forceinline__ uint32_t leaf_range_code(uint32_t first, uint32_t count) {
+  return 0x80000000u | ((count - 1u) << 26) | first;
+}
+__host__ __device__ __forceinline__ uint32_t leaf_range_first(uint32_t code) { return code & LEAF_FIRST_MASK; }
+__host__ __device__ __forceinline__ uint32_t leaf_range_count(uint32_t code) { return ((code >> 26) & 31u) + 1u; }
+
 struct __align__(64) Node {
   float b[12];
   int left, right;

@@ -59,14 +59,14 @@ emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm
     }
     const int gamma = i + s * d + min(d, 0);
     const int first = min(i, j), last = max(i, j);
-    const int left = (first == gamma) ? ~gamma : gamma;
-    const int right = (last == gamma + 1) ? ~(gamma + 1) : gamma + 1;
-    nodes[i].left = left;
-    nodes[i].right = right;
+    const bool leaf_l = first == gamma, leaf_r = last == gamma + 1;
+    const int cnt_l = gamma - first + 1, cnt_r = last - gamma;
+    nodes[i].left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : gamma;
+    nodes[i].right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)gamma + 1u, (uint32_t)cnt_r) : gamma + 1;
     nodes[i].flag = 0u;
     if (i == 0) nodes[0].parent = -1;
-    if (left < 0) leaf_parent[gamma] = (i << 1); else nodes[left].parent = (i << 1);
-    if (right < 0) leaf_parent[gamma + 1] = (i << 1) | 1; else nodes[right].parent = (i << 1) | 1;
+    if (leaf_l) leaf_parent[gamma] = (i << 1); else nodes[gamma].parent = (i << 1);
+    if (leaf_r) leaf_parent[gamma + 1] = (i << 1) | 1; else nodes[gamma + 1].parent = (i << 1) | 1;
   }
 }
 
@@ -123,8 +123,19 @@ export_kernel(const Node* __restrict__ nodes, const int* __restrict__ leaf_paren
     if (i < n - 1) {
       const Node nd = nodes[i];
       if (children) {
-        children[2 * i] = nd.left < 0 ? n - 1 + ~nd.left : nd.left;
-        children[2 * i + 1] = nd.right < 0 ? n - 1 + ~nd.right : nd.right;
+        // canonical Karras links from the traversal links (common.cuh, Node)
+        const uint32_t l = (uint32_t)nd.left, r = (uint32_t)nd.right;
+        int cl = nd.left, cr = nd.right;
+        if (nd.left < 0) {
+          const int f = (int)leaf_range_first(l), c = (int)leaf_range_count(l);
+          cl = c == 1 ? n - 1 + f : f + c - 1;
+        }
+        if (nd.right < 0) {
+          const int f = (int)leaf_range_first(r), c = (int)leaf_range_count(r);
+          cr = c == 1 ? n - 1 + f : f;
+        }
+        children[2 * i] = cl;
+        children[2 * i + 1] = cr;
       }
       if (parents) parents[i] = nd.parent < 0 ? -1 : (nd.parent >> 1);
       if (aabbs) {

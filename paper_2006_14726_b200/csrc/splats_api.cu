@@ -213,8 +213,8 @@ extern "C" {
 
 int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (g_ctx) return fail(SPLATS_ESTATE, "context already exists: call splats_destroy first");
-  if (max_W <= 0 || max_H <= 0 || (int64_t)max_W * max_H > (1ll << 28))
-    return fail(SPLATS_EINVAL, "max_W*max_H outside [1, 2^28]");
+  if (max_W <= 0 || max_H <= 0 || (int64_t)max_W * max_H >= (1ll << 26))
+    return fail(SPLATS_EINVAL, "max_W*max_H outside [1, 2^26)");
   int dev = 0;
   CU(cudaGetDevice(&dev));
   Context* c = new Context();
