@@ -86,7 +86,10 @@ struct FrameState {
 //     a longer left (right) range is internal node first + count - 1 (first).
 //   parent: (parent index << 1) | is_right_child, -1 for the root
 //   flag: arrival counter of the bottom-up refit
-constexpr int LEAF_MAX = 8;                  // <= 32 (5-bit count field)
+#ifndef SPLATS_LEAF_MAX
+#define SPLATS_LEAF_MAX 1
+#endif
+constexpr int LEAF_MAX = SPLATS_LEAF_MAX;    // <= 32 (5-bit count field)
 constexpr uint32_t LEAF_FIRST_MASK = (1u << 26) - 1;  // capacity: 2^26 - 1 splats
 __host__ __device__ __forceinline__ uint32_t leaf_range_code(uint32_t first, uint32_t count) {
   return 0x80000000u | ((count - 1u) << 26) | first;

@@ -18,7 +18,10 @@
 namespace sw {
 
 constexpr int RENDER_THREADS = 128;
-constexpr int KBUF = 4;
+#ifndef SPLATS_KBUF
+#define SPLATS_KBUF 4
+#endif
+constexpr int KBUF = SPLATS_KBUF;
 constexpr int SSTACK = 16;
 constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
 constexpr uint32_t EMPTY_LEAF = 0xffffffffu;
@@ -32,6 +35,7 @@ struct RenderParams {
   const uint32_t* ids;
   const FrameState* st;
   float4* out;
+  unsigned* sched;  // [0] tile ticket, [1] blocks done (both zero between launches)
 };
 
 #ifdef SPLATS_STATS
@@ -84,32 +88,113 @@ __device__ __forceinline__ bool ray_sphere(const float o[3], const float d[3], c
   return t >= 0.0f;
 }
 
-__global__ void __launch_bounds__(RENDER_THREADS)
+// Screen rectangle (in 8x4-pixel warp tiles) that contains every pixel whose ray can touch the
+// scene box: the projection of a convex box is the hull of its projected corners.  A corner at
+// or behind the eye plane makes the rectangle the whole screen.  Computed by 8 lanes of warp 0.
+__device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo[3], const float hi[3], int lane,
+                                            int rect[4]) {
+  const int c = lane & 7;
+  const float v[3] = {((c & 1) ? hi[0] : lo[0]) - cam.e[0], ((c & 2) ? hi[1] : lo[1]) - cam.e[1],
+                      ((c & 4) ? hi[2] : lo[2]) - cam.e[2]};
+  const float z = v[0] * cam.F[0] + v[1] * cam.F[1] + v[2] * cam.F[2];
+  const float xr = v[0] * cam.R[0] + v[1] * cam.R[1] + v[2] * cam.R[2];
+  const float yu = v[0] * cam.U[0] + v[1] * cam.U[1] + v[2] * cam.U[2];
+  const bool behind = !(z > 1e-6f * (fabsf(xr) + fabsf(yu) + fabsf(z)) && z > 0.0f);
+  // pixel centre x has ndc (2x+1-W)/W; row y has ndc (H-2y-1)/H
+  float px = ((xr / (z * cam.ta)) * cam.fW + cam.fW - 1.0f) * 0.5f;
+  float py = (cam.fH - 1.0f - (yu / (z * cam.tau)) * cam.fH) * 0.5f;
+  float x0 = px, x1 = px, y0 = py, y1 = py;
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) {
+    x0 = fminf(x0, __shfl_xor_sync(0xffffffffu, x0, o));
+    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, o));
+    y0 = fminf(y0, __shfl_xor_sync(0xffffffffu, y0, o));
+    y1 = fmaxf(y1, __shfl_xor_sync(0xffffffffu, y1, o));
+  }
+  const bool any_behind = __any_sync(0xffffffffu, behind);
+  const int tiles_x = (cam.W + 7) >> 3, tiles_y = (cam.H + 3) >> 2;
+  if (any_behind || !(x0 == x0) || !(x1 == x1) || !(y0 == y0) || !(y1 == y1)) {
+    rect[0] = 0; rect[1] = 0; rect[2] = (tiles_x + 1) & ~1; rect[3] = (tiles_y + 1) & ~1;
+    return;
+  }
+  // two pixels of slack: far more than the float32 error of the projection above
+  const float fx0 = fmaxf(floorf(x0) - 2.0f, 0.0f), fx1 = fminf(ceilf(x1) + 2.0f, cam.fW - 1.0f);
+  const float fy0 = fmaxf(floorf(y0) - 2.0f, 0.0f), fy1 = fminf(ceilf(y1) + 2.0f, cam.fH - 1.0f);
+  if (fx0 > fx1 || fy0 > fy1) { rect[0] = rect[1] = rect[2] = rect[3] = 0; return; }  // off screen
+  rect[0] = ((int)fx0 >> 4) << 1; rect[1] = ((int)fy0 >> 3) << 1;   // aligned to 16x8-pixel supertiles
+  rect[2] = (((int)fx1 >> 4) + 1) << 1; rect[3] = (((int)fy1 >> 3) + 1) << 1;   // exclusive
+}
+
+// Persistent grid (SMs x resident blocks).  (A) every pixel outside the scene's screen rectangle
+// is background: written as zeros by a grid-stride loop, no ray is set up for it.  (B) the 8x4
+// warp tiles inside the rectangle are handed out dynamically: a warp's first tile is its index
+// in the grid, every further one comes from an atomic ticket; the last block to finish re-arms
+// the ticket for the next launch.
+__global__ void __launch_bounds__(RENDER_THREADS, 8)
 render_kernel(RenderParams prm) {
   __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
   __shared__ float s_tn[SSTACK][RENDER_THREADS];
+  __shared__ int s_rect[4];
   uint32_t l_node[LSTACK];
   float l_tn[LSTACK];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const DevCamera& cam = prm.cam;
-  const int x = blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7);
-  const int y = blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3);
-  const bool inside = x < cam.W && y < cam.H;
   const int n = (int)prm.st->n;
   const float INF = __int_as_float(0x7f800000);
+  const float o[3] = {cam.e[0], cam.e[1], cam.e[2]};
 
-  float o[3] = {cam.e[0], cam.e[1], cam.e[2]};
-  float d[3], len;
-  pixel_ray(cam, min(x, cam.W - 1), min(y, cam.H - 1), d, len);
-
-  // Conservative slab test (free arithmetic): boxes are padded by far more
-  // than the float32 error of ray_sphere(), and the test is one FMA per plane:
-  // (plane -+ pad - o) / d = plane * idir - (o +- pad) * idir.
+  // conservative padding of every box: far more than the float32 error of ray_sphere()
   float m = 1.0f;
 #pragma unroll
   for (int a = 0; a < 3; ++a)
     m = fmaxf(m, fmaxf(fabsf(o[a]), fmaxf(fabsf(prm.st->root_lo[a]), fabsf(prm.st->root_hi[a]))));
   const float pad = 4e-5f * m;
+
+  if (warp == 0) {
+    int rect[4] = {0, 0, 0, 0};
+    if (n > 0) {
+      const float lo[3] = {prm.st->root_lo[0] - pad, prm.st->root_lo[1] - pad, prm.st->root_lo[2] - pad};
+      const float hi[3] = {prm.st->root_hi[0] + pad, prm.st->root_hi[1] + pad, prm.st->root_hi[2] + pad};
+      screen_rect(cam, lo, hi, lane, rect);
+    }
+    if (lane < 4) s_rect[lane] = rect[lane];
+  }
+  __syncthreads();
+  const int rx0 = s_rect[0], ry0 = s_rect[1], rx1 = s_rect[2], ry1 = s_rect[3];
+
+  // ---- (B) warp tiles inside the rectangle
+  // tickets [0, ntiles): trace one 8x4 tile (2x2 tiles = one 16x8 supertile are consecutive);
+  // tickets [ntiles, ntiles + nfill): zero FILL_PX background pixels outside the rectangle
+  constexpr int FILL_PX = 1024;
+  const int rw = rx1 - rx0, ntiles = rw * (ry1 - ry0);
+  const int total_px = cam.W * cam.H;
+  const int nfill = (total_px + FILL_PX - 1) / FILL_PX;
+  const int nwarps = gridDim.x * (RENDER_THREADS / 32);
+  int tile = blockIdx.x * (RENDER_THREADS / 32) + warp;
+  for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, lane == 0 ? atomicAdd(prm.sched, 1u) : 0u, 0)) {
+  if (tile >= ntiles) {
+    const int px0 = rx0 * 8, px1 = rx1 * 8, py0 = ry0 * 4, py1 = ry1 * 4;
+    const int base = (tile - ntiles) * FILL_PX;
+#pragma unroll 4
+    for (int k = lane; k < FILL_PX; k += 32) {
+      const int idx = base + k;
+      const int yy = idx / cam.W, xx = idx - yy * cam.W;
+      if (idx < total_px && !(xx >= px0 && xx < px1 && yy >= py0 && yy < py1))
+        prm.out[idx] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    }
+    continue;
+  }
+  const int sw = rw >> 1, super = tile >> 2;        // the rectangle is aligned to supertiles
+  const int ty = (super / sw) * 2 + ((tile >> 1) & 1), tx = (super % sw) * 2 + (tile & 1);
+  const int x = (rx0 + tx) * 8 + (lane & 7);
+  const int y = (ry0 + ty) * 4 + (lane >> 3);
+  const bool inside = x < cam.W && y < cam.H;
+
+  float d[3], len;
+  pixel_ray(cam, min(x, cam.W - 1), min(y, cam.H - 1), d, len);
+
+  // Conservative slab test (free arithmetic): one FMA per plane,
+  // (plane -+ pad - o) / d = plane * idir - (o +- pad) * idir.
   float idir[3], oip[3], oim[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -122,7 +207,7 @@ render_kernel(RenderParams prm) {
   float C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f;
   float cur_t = -1.0f;
   uint32_t cur_id = 0;
-  bool finished = !inside || n == 0;
+  bool finished = !inside;
   KBuffer kb;
 
   while (__any_sync(0xffffffffu, !finished)) {
@@ -231,6 +316,12 @@ render_kernel(RenderParams prm) {
     }
   }
   if (inside) prm.out[(size_t)y * cam.W + x] = make_float4(C[0], C[1], C[2], A);
+  }  // tile loop
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    if (atomicInc(prm.sched + 1, gridDim.x - 1) == gridDim.x - 1) prm.sched[0] = 0u;
+  }
 }
 
 }  // namespace sw

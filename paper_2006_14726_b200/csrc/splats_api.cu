@@ -31,6 +31,7 @@ struct Context {
   // device memory
   FrameState* state = nullptr;      // [2], by frame parity
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
+  unsigned* sched = nullptr;        // render tile ticket + done counter
   uint64_t* key[2] = {nullptr, nullptr};
   uint32_t* val[2] = {nullptr, nullptr};
   uint64_t* status = nullptr;       // [max sort tiles][256]
@@ -47,6 +48,7 @@ struct Context {
   uint32_t epoch = 0;
   bool has_bvh = false;
   int sort_grid = 0;
+  int render_grid = 0;
   size_t sort_smem = 0;
   // profiling
   bool profiling = false;
@@ -120,7 +122,7 @@ cudaError_t dmalloc(T** p, size_t count) {
 }
 
 void free_all(Context* c) {
-  cudaFree(c->state); cudaFree(c->tile_count);
+  cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
   cudaFree(c->leaf_parent); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
@@ -189,7 +191,10 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out) {
   prm.ids = c->val[0];
   prm.st = c->state + c->parity;
   prm.out = reinterpret_cast<float4*>(out);
-  dim3 grid((W2 + 15) / 16, (H2 + 7) / 8);
+  prm.sched = c->sched;
+  const int tiles = ((W2 + 7) / 8) * ((H2 + 3) / 4);
+  const int blocks_needed = (tiles + RENDER_THREADS / 32 - 1) / (RENDER_THREADS / 32);
+  const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
   render_kernel<<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
@@ -227,6 +232,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   const size_t max_sort_tiles = (cap + SORT_TILE - 1) / SORT_TILE;
   if (e == cudaSuccess) e = dmalloc(&c->state, 2);
   if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
+  if (e == cudaSuccess) e = dmalloc(&c->sched, 2);
+  if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * sizeof(unsigned));
   for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
     e = dmalloc(&c->key[i], cap);
     if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
@@ -258,6 +265,14 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     return cuda_fail(e, "splats_create");
   }
   c->sort_grid = c->num_sms * occ;  // co-resident persistent grid (see onesweep.cuh)
+  int rocc = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rocc, render_kernel, RENDER_THREADS, 0);
+  if (e != cudaSuccess || rocc < 1) {
+    free_all(c);
+    delete c;
+    return e != cudaSuccess ? cuda_fail(e, "splats_create") : fail(SPLATS_ECUDA, "render kernel does not fit on an SM");
+  }
+  c->render_grid = c->num_sms * rocc;
   g_ctx = c;
   return SPLATS_OK;
 }
