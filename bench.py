@@ -82,8 +82,10 @@ def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
         "bounds": 4 * P + 4 * (P // 2048 + 1),
         "unproject_morton_compact": 4 * P + 12 * N,
         "sort": 8 * 24 * N,                       # 8 passes x (read 12 N + write 12 N)
-        "hierarchy_gather": (8 + 4 + 4 + 16) * N + (16 + 16 + 16 + 4) * N,
-        "refit": (16 + 4) * N + 48 * N + 24 * N + 8 * N,
+        # pyramid mode: gather (perm 4, depth 4, colour 16) -> sphere 16 + rgba 16 + pyramid 32 (N entries)
+        "tree_1": (4 + 4 + 16) * N + (16 + 16 + 32) * N,
+        # keys 8 + sphere 16 + pyramid 32 read once, 64-byte node records written once
+        "tree_2": (8 + 16 + 32) * N + 64 * N,
         "render": 16 * P2 + (64 + 16 + 16 + 4) * N,  # image written once + BVH/splats read once
     }
 

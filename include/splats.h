@@ -108,13 +108,27 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
  * lo_hi: 6 float32.  Synchronises.  Parity/debug only. */
 int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 
+/* Implementation variants (same results, bit for bit; for A/B measurement).  Takes effect at
+ * the next splats_update.
+ *   SPLATS_OPT_REFIT: how step a5 (node boxes) is computed.
+ *     SPLATS_REFIT_PYRAMID (default): a bottom-up min/max pyramid over the sorted leaf boxes,
+ *       then every node reads its two child boxes as range queries (no atomics, no fences).
+ *     SPLATS_REFIT_ATOMIC: one thread per leaf climbs the tree; the second arrival at a node's
+ *       atomic counter forms the union and continues (the classic LBVH refit).
+ * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
+#define SPLATS_OPT_REFIT       0
+#define SPLATS_REFIT_PYRAMID   0
+#define SPLATS_REFIT_ATOMIC    1
+int splats_set_option(int option, int value);
+
 /* Per-stage device times, measured with CUDA events recorded on the library's stream around
  * each stage of every update / render issued while profiling is on.  Off by default (the
  * event records cost about a microsecond each).  splats_stage_ms synchronises the stream,
  * returns for each stage the SUM of its durations in milliseconds and how many times it ran
  * since profiling was switched on or since the previous query, and clears the record.
- * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 hierarchy+gather,
- * 4 refit, 5 render.  calls may be NULL. */
+ * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 first tree kernel
+ * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 second tree
+ * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render.  calls may be NULL. */
 #define SPLATS_NUM_STAGES 6
 int splats_set_profiling(int on);
 int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);

@@ -16,7 +16,8 @@ import torch
 from . import build as _build
 
 NUM_STAGES = 6
-STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "hierarchy_gather", "refit", "render")
+STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render")
+OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 
 
 class SplatsError(RuntimeError):
@@ -53,6 +54,7 @@ def lib() -> ctypes.CDLL:
         L.splats_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
         L.splats_export_splats.argtypes = [_vp, _vp, _vp]
         L.splats_set_profiling.argtypes = [_ci]
+        L.splats_set_option.argtypes = [_ci, _ci]
         L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_uint)]
         L.splats_launch_count.restype = ctypes.c_ulonglong
         L.splats_last_error.restype = ctypes.c_char_p
@@ -152,6 +154,10 @@ def splats_export_splats():
     _check(lib().splats_export_splats(sphere.data_ptr() if n else None, rgba.data_ptr() if n else None,
                                       lo_hi.data_ptr()))
     return dict(N=n, sphere=sphere, rgba=rgba, lo_hi=lo_hi)
+
+
+def splats_set_option(option: int, value: int) -> None:
+    _check(lib().splats_set_option(int(option), int(value)))
 
 
 def splats_set_profiling(on: bool) -> None:

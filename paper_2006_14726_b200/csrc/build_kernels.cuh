@@ -149,6 +149,7 @@ unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevC
   if (blockIdx.x == 0) {  // re-arm the accumulators of the next frame (other parity)
     if (tid < 3) { st_next->lo[tid] = 0xffffffffu; st_next->hi[tid] = 0u; }
     if (tid == 3) st_next->n = 0u;
+    if (tid == 4) st_next->pyr_done = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
   }

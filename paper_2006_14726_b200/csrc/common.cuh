@@ -68,7 +68,7 @@ struct FrameState {
   uint32_t lo[3];      // ordered-uint min of valid centres   (init 0xffffffff)
   uint32_t hi[3];      // ordered-uint max                     (init 0)
   uint32_t n;          // number of valid splats               (init 0)
-  uint32_t pad0;
+  uint32_t pyr_done;   // blocks of leaf_pyramid_kernel that have finished (init 0)
   float root_lo[3];    // AABB of the whole scene (root node box), written by refit
   float root_hi[3];
   uint32_t pad1[2];

@@ -39,6 +39,9 @@ struct Context {
   float4* rgba = nullptr;
   Node* nodes = nullptr;
   int* leaf_parent = nullptr;
+  float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
+  PyramidLayout pyr_layout;
+  int refit_mode = SPLATS_REFIT_PYRAMID;
   float* stage_color = nullptr;     // staging for the *_host calls
   float* stage_depth = nullptr;
   float* stage_out = nullptr;
@@ -125,7 +128,7 @@ void free_all(Context* c) {
   cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
-  cudaFree(c->leaf_parent); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
   for (auto& e : c->pool)
     if (e) cudaEventDestroy(e);
 }
@@ -167,10 +170,18 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   if (prof) m[3] = c->mark();
   const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
   const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
-  emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
-                                             k_r, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
-  if (prof) m[4] = c->mark();
-  refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
+  if (c->refit_mode == SPLATS_REFIT_ATOMIC) {
+    emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
+                                               k_r, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
+    if (prof) m[4] = c->mark();
+    refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
+  } else {
+    const int pgrid = (int)((P + PYR_LEAVES - 1) / PYR_LEAVES);
+    leaf_pyramid_kernel<<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], depth, reinterpret_cast<const float4*>(color), dc, k_r,
+                                                      st, c->sphere, c->rgba, c->pyr);
+    if (prof) m[4] = c->mark();
+    emit_boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->sphere, c->pyr, st, c->nodes);
+  }
   if (prof) m[5] = c->mark();
   c->launches += 12;
   if (prof)
@@ -243,6 +254,16 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (e == cudaSuccess) e = dmalloc(&c->rgba, cap);
   if (e == cudaSuccess) e = dmalloc(&c->nodes, cap);
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
+  {  // pyramid levels 1.. : ceil(cap / 2^k) entries each
+    size_t off = 0;
+    c->pyr_layout.off[0] = 0;
+    for (int k = 1; k <= PYR_MAX_LEVELS; ++k) {
+      c->pyr_layout.off[k] = (uint32_t)off;
+      off += (cap + ((size_t)1 << k) - 1) >> k;
+    }
+    if (e == cudaSuccess) e = dmalloc(&c->pyr, 2 * off);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_pyr, &c->pyr_layout, sizeof(PyramidLayout));
+  }
   if (e == cudaSuccess) e = cudaMemset(c->status, 0, max_sort_tiles * RADIX * sizeof(uint64_t));
   if (e == cudaSuccess) {
     FrameState init;
@@ -343,9 +364,10 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   if (keys) CU(cudaMemcpyAsync(keys, c->key[0], (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream));
   if (perm) CU(cudaMemcpyAsync(perm, c->val[0], (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
   if (children || parents || node_aabbs) {
+    if (parents) CU(cudaMemsetAsync(parents, 0xff, (size_t)(2 * n - 1) * sizeof(int), c->stream));
     const int grid = (int)((n + LBVH_THREADS - 1) / LBVH_THREADS);
-    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->nodes, c->leaf_parent, c->sphere, c->state + c->parity,
-                                                        children, parents, node_aabbs);
+    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->nodes, c->sphere, c->state + c->parity, children, parents,
+                                                        node_aabbs);
     c->launches += 1;
     CU(cudaGetLastError());
   }
@@ -379,6 +401,18 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi) {
   }
   CU(cudaStreamSynchronize(c->stream));
   return SPLATS_OK;
+}
+
+int splats_set_option(int option, int value) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  switch (option) {
+    case SPLATS_OPT_REFIT:
+      if (value != SPLATS_REFIT_PYRAMID && value != SPLATS_REFIT_ATOMIC) return fail(SPLATS_EINVAL, "unknown refit mode");
+      g_ctx->refit_mode = value;
+      return SPLATS_OK;
+    default:
+      return fail(SPLATS_EINVAL, "unknown option");
+  }
 }
 
 int splats_set_profiling(int on) {

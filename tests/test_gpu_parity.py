@@ -121,6 +121,32 @@ def test_config1_full():
         check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams, mode="bvh")
 
 
+@pytest.mark.parametrize("W,H", [(32, 32), (41, 25), (683, 3), (64, 64)])
+def test_pyramid_block_boundaries(W, H):
+    # N = 1024, 1025, 2049, 4096: exactly one pyramid block, one leaf into the next, ...
+    color, depth, cam = synth.random_frame(W, H, seed=W + H, fill=1.0)
+    with Session(W, H) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(3.0)], mode="bvh")
+        assert sc["N"] == W * H
+
+
+def test_atomic_refit_mode_gives_the_same_tree():
+    # SPLATS_OPT_REFIT: the classic atomic-counter refit must give the bit-identical BVH
+    cfg = synth.make_config(1)
+    color, depth = synth.source_frame(cfg, 0)
+    with Session(cfg.W, cfg.H) as s:
+        sp.splats_set_option(sp.OPT_REFIT, sp.REFIT_ATOMIC)
+        check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams[:1], mode="bvh")
+        c2, d2, cam2 = synth.random_frame(127, 65, seed=3, fill=0.4)
+        check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
+        sp.splats_set_option(sp.OPT_REFIT, sp.REFIT_PYRAMID)
+        check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
+        with pytest.raises(sp.SplatsError):
+            sp.splats_set_option(sp.OPT_REFIT, 7)
+        with pytest.raises(sp.SplatsError):
+            sp.splats_set_option(99, 0)
+
+
 def test_repeated_updates_and_size_changes():
     # frame-parity double buffering: A, B (other size), A again must reproduce A
     cfg = synth.make_config(0)
