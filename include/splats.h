@@ -115,10 +115,21 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *       then every node reads its two child boxes as range queries (no atomics, no fences).
  *     SPLATS_REFIT_ATOMIC: one thread per leaf climbs the tree; the second arrival at a node's
  *       atomic counter forms the union and continues (the classic LBVH refit).
+ *   SPLATS_OPT_SORT: how step a3 (order by (code, id)) is computed.
+ *     SPLATS_SORT_HYBRID (default): one launch; 4 onesweep passes over the top 31 code bits,
+ *       then a check that no two neighbours share them (true for one-sample-per-pixel frames);
+ *       short runs are fixed up by a stable insertion sort, longer ones make the same launch
+ *       redo the sort with all 8 passes.
+ *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
+ *     SPLATS_SORT_LSD8_LAUNCHES: one launch per pass.
  * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
 #define SPLATS_OPT_REFIT       0
 #define SPLATS_REFIT_PYRAMID   0
 #define SPLATS_REFIT_ATOMIC    1
+#define SPLATS_OPT_SORT        1
+#define SPLATS_SORT_HYBRID         0
+#define SPLATS_SORT_LSD8           1
+#define SPLATS_SORT_LSD8_LAUNCHES  2
 int splats_set_option(int option, int value);
 
 /* Per-stage device times, measured with CUDA events recorded on the library's stream around

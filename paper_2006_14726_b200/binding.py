@@ -18,6 +18,7 @@ from . import build as _build
 NUM_STAGES = 6
 STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
+OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 
 
 class SplatsError(RuntimeError):

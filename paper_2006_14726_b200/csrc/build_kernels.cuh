@@ -150,6 +150,8 @@ unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevC
     if (tid < 3) { st_next->lo[tid] = 0xffffffffu; st_next->hi[tid] = 0u; }
     if (tid == 3) st_next->n = 0u;
     if (tid == 4) st_next->pyr_done = 0u;
+    if (tid == 5) st_next->sort_bar = 0u;
+    if (tid == 6) st_next->sort_fallback = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
   }

@@ -71,7 +71,8 @@ struct FrameState {
   uint32_t pyr_done;   // blocks of leaf_pyramid_kernel that have finished (init 0)
   float root_lo[3];    // AABB of the whole scene (root node box), written by refit
   float root_hi[3];
-  uint32_t pad1[2];
+  uint32_t sort_bar;       // grid barrier counter of the sort launch (init 0)
+  uint32_t sort_fallback;  // set when the hybrid sort has to redo all 8 passes (init 0)
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
 

@@ -2,16 +2,29 @@
 // of (63-bit Morton code, splat id) pairs, 8 bits per pass, stable (
 // LBVH).
 //
-// One launch per digit.  The grid is persistent and co-resident (<= SMs x occupancy), tiles
-// are dealt round-robin (block b owns tiles b, b+G, ...), and each tile obtains the global
-// offset of each of its 256 digit bins by a chained scan with decoupled look-back over the
-// tiles before it.  Because all blocks are resident and every block walks its tiles in
-// ascending order, the lowest unfinished tile can always make progress: no deadlock, no
-// atomic ticket.  The look-back status words carry an epoch (unique per pass and frame) so
-// the status array never needs clearing.
+// The grid is persistent and co-resident (<= SMs x occupancy), tiles are dealt round-robin
+// (block b owns tiles b, b+G, ...), and each tile obtains the global offset of each of its 256
+// digit bins by a chained scan with decoupled look-back over the tiles before it.  Because all
+// blocks are resident and every block walks its tiles in ascending order, the lowest
+// unfinished tile can always make progress: no deadlock, no atomic ticket.  The look-back
+// status words carry an epoch (unique per pass and frame) so the status array never needs
+// clearing.  The digit histograms (hence the bin bases) come from unproject_kernel, which had
+// the keys in registers anyway.
 //
-// The digit histograms (hence the bin bases) come from unproject_kernel, which had the keys
-// in registers anyway.
+// One launch runs several passes, separated by a grid barrier (the grid is co-resident
+// anyway), in one of three modes:
+//   SORT_HYBRID (default)  passes 4..7 only, i.e. a stable sort by the top 31 code bits (32..62); then
+//       every block checks its tiles for neighbours with equal top bits.  For the frames
+//       this library is made for (one sample per pixel of a surface: the 2048 x 1024 x 1024
+//       cells of those bits are finer than the sample pitch) there are none and the
+//       order is already the order by (code, id).  Short runs of equal top bits (<= RUN_MAX)
+//       are put in order by a stable insertion sort on the full code; a longer run raises a
+//       flag and the same launch then redoes the sort with all 8 passes (degenerate inputs:
+//       many equal codes).  The result is the same permutation in every case.
+//   SORT_LSD8     all 8 passes in one launch.
+//   SORT_SINGLE   one pass per launch (8 launches), the classic arrangement.
+// Within a launch a buffer is read in one pass and written in the next, so keys and values
+// are read with ld.global.cg (L2): a line cached in L1 by an earlier pass would be stale.
 #pragma once
 #include "common.cuh"
 
@@ -25,6 +38,19 @@ constexpr int RADIX = 256;
 constexpr uint64_t FLAG_AGG = 1ull << 30;  // tile aggregate available
 constexpr uint64_t FLAG_INC = 2ull << 30;  // inclusive prefix available
 constexpr uint32_t VALUE_MASK = (1u << 30) - 1;
+constexpr int LOOKBACK = 8;
+constexpr int RUN_MAX = 32;           // longest run of equal top bits fixed up in place
+constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
+
+struct SortArgs {
+  uint64_t* key[2];
+  uint32_t* val[2];
+  FrameState* st;
+  uint64_t* status;
+  uint32_t epoch0;   // this launch may use epochs epoch0 .. epoch0 + 11
+  int mode;
+  int pass;          // SORT_SINGLE: the digit; input buffer = pass & 1
+};
 
 template <int ITEMS>
 struct SortSmem {
@@ -59,23 +85,32 @@ __device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* tm
   return off + incl - v;
 }
 
+// Grid barrier over the nb participating blocks (all co-resident); `bar` only ever grows
+// within a frame and is re-armed by unproject_kernel of the next frame.
+__device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t nb, uint32_t& round) {
+  ++round;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(bar, 1u);
+    while (*reinterpret_cast<volatile uint32_t*>(bar) < round * nb) {}
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+// One 8-bit pass over all tiles of this block: in -> out.
 template <int ITEMS>
-__global__ void __launch_bounds__(SORT_THREADS)
-onesweep_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
-                uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
-                const FrameState* __restrict__ st, int pass, uint64_t* __restrict__ status, uint32_t epoch) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  SortSmem<ITEMS>& s = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
+__device__ __forceinline__ void onesweep_pass(SortSmem<ITEMS>& s, const uint64_t* kin, const uint32_t* vin,
+                                              uint64_t* kout, uint32_t* vout, const FrameState* st, int pass,
+                                              uint64_t* status, uint32_t epoch, uint32_t n, int num_tiles) {
   constexpr int TILE = SORT_THREADS * ITEMS;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t n = st->n;
-  const int num_tiles = (int)((n + TILE - 1) / TILE);
-  if ((int)blockIdx.x >= num_tiles) return;
   const int shift = 8 * pass;
   const uint64_t ep = (uint64_t)epoch << 32;
 
   {  // bin bases of this digit: exclusive scan of the global histogram
-    uint32_t h = st->hist[pass][tid];
+    uint32_t h = __ldcg(&st->hist[pass][tid]);
     uint32_t e = block_excl_scan_256(h, s.scan_tmp, nullptr);
     s.digit_base[tid] = e;
   }
@@ -84,11 +119,17 @@ onesweep_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ v
     const uint32_t tile_base = (uint32_t)tile * TILE;
     // ---- load, warp-striped: item (warp, j, lane) has index tile_base + warp*32*ITEMS + j*32 + lane
     uint64_t key[ITEMS];
+    uint32_t val[ITEMS];
     const uint32_t wbase = tile_base + warp * 32 * ITEMS + lane;
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const uint32_t idx = wbase + j * 32;
-      key[j] = idx < n ? kin[idx] : ~0ull;
+      key[j] = idx < n ? __ldcg(kin + idx) : ~0ull;
+    }
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t idx = wbase + j * 32;
+      val[j] = idx < n ? __ldcg(vin + idx) : 0u;
     }
 #pragma unroll
     for (int w = 0; w < SORT_WARPS; ++w) s.warp_hist[w][tid] = 0;
@@ -119,24 +160,43 @@ onesweep_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ v
       s.warp_hist[w][tid] = count;
       count += c;
     }
+    // ---- publish the aggregate, then scan the tile's counts while the status word travels
+    uint64_t* my = status + (size_t)tile * RADIX + tid;
+    if (tile != 0) st_volatile_u64(my, ep | FLAG_AGG | count);
     const uint32_t toff = block_excl_scan_256(count, s.scan_tmp, nullptr);
     s.tile_off[tid] = toff;
 
     // ---- decoupled look-back for bin `tid`
-    uint64_t* my = status + (size_t)tile * RADIX + tid;
     uint32_t excl;
     if (tile == 0) {
       excl = s.digit_base[tid];
     } else {
-      st_volatile_u64(my, ep | FLAG_AGG | count);
       excl = 0;
+      // LOOKBACK predecessors per round trip: in the one-wave regime (N below a few million)
+      // all tiles publish their aggregates at about the same time, so the walk back to tile 0
+      // is a chain of L2 round trips; independent loads cut it by the batch size.
       int t = tile - 1;
-      while (true) {
-        uint64_t w = ld_volatile_u64(status + (size_t)t * RADIX + tid);
-        if ((w >> 32) != epoch || (w & (FLAG_AGG | FLAG_INC)) == 0) continue;  // not published yet
-        excl += (uint32_t)w & VALUE_MASK;
-        if (w & FLAG_INC) break;
-        --t;
+      bool done = false;
+      while (!done) {
+        uint64_t w[LOOKBACK];
+#pragma unroll
+        for (int k = 0; k < LOOKBACK; ++k)
+          w[k] = t - k >= 0 ? ld_volatile_u64(status + (size_t)(t - k) * RADIX + tid) : 0ull;
+        bool stalled = false;
+        int used = 0;
+#pragma unroll
+        for (int k = 0; k < LOOKBACK; ++k) {
+          if (!done && !stalled) {
+            if ((w[k] >> 32) != epoch || (w[k] & (FLAG_AGG | FLAG_INC)) == 0) {
+              stalled = true;  // not published yet: poll again from this tile
+            } else {
+              excl += (uint32_t)w[k] & VALUE_MASK;
+              ++used;
+              if (w[k] & FLAG_INC) done = true;
+            }
+          }
+        }
+        t -= used;
       }
     }
     st_volatile_u64(my, ep | FLAG_INC | (excl + count));
@@ -161,7 +221,7 @@ onesweep_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ v
       if (k < tile_n) {
         const uint64_t kk = s.stage[k];
         odig[j] = (uint8_t)((kk >> shift) & 0xff);
-        kout[s.bin_base[odig[j]] + k] = kk;
+        __stcg(kout + (s.bin_base[odig[j]] + k), kk);
       }
     }
     __syncthreads();
@@ -170,15 +230,92 @@ onesweep_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ v
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const uint32_t idx = wbase + j * 32;
-      if (idx < n) vstage[slot[j]] = vin[idx];
+      if (idx < n) vstage[slot[j]] = val[j];
     }
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const uint32_t k = tid + j * SORT_THREADS;
-      if (k < tile_n) vout[s.bin_base[odig[j]] + k] = vstage[k];
+      if (k < tile_n) __stcg(vout + (s.bin_base[odig[j]] + k), vstage[k]);
     }
     __syncthreads();
+  }
+}
+
+// SORT_HYBRID, after the passes over bits 32..62: look for neighbours with equal top bits
+// in this block's tiles.  The head of a run of 2..RUN_MAX elements sorts it in place (stable
+// insertion sort by the full code; equal codes keep their order, which is id order); a longer
+// run raises st->sort_fallback.
+template <int ITEMS>
+__device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, int num_tiles) {
+  constexpr int TILE = SORT_THREADS * ITEMS;
+  for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    const uint32_t tile_base = (uint32_t)tile * TILE;
+#pragma unroll 4
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t idx = tile_base + j * SORT_THREADS + threadIdx.x;
+      if (idx >= n) continue;
+      const uint64_t k = __ldcg(key + idx);
+      const uint64_t kn = idx + 1 < n ? __ldcg(key + idx + 1) : ~k;
+      if ((k >> 32) != (kn >> 32)) continue;                       // common case: no run continues here
+      if (idx > 0 && (__ldcg(key + idx - 1) >> 32) == (k >> 32)) continue;  // not the head
+      uint32_t len = 2;
+      while (len <= RUN_MAX && idx + len < n && (__ldcg(key + idx + len) >> 32) == (k >> 32)) ++len;
+      if (len > RUN_MAX) {
+        st->sort_fallback = 1u;
+        continue;
+      }
+      for (uint32_t a = 1; a < len; ++a) {
+        const uint64_t ka = __ldcg(key + idx + a);
+        const uint32_t va = __ldcg(val + idx + a);
+        uint32_t b = a;
+        while (b > 0) {
+          const uint64_t kb = __ldcg(key + idx + b - 1);
+          if (!(kb > ka)) break;
+          __stcg(key + idx + b, kb);
+          __stcg(val + idx + b, __ldcg(val + idx + b - 1));
+          --b;
+        }
+        if (b != a) {
+          __stcg(key + idx + b, ka);
+          __stcg(val + idx + b, va);
+        }
+      }
+    }
+  }
+}
+
+template <int ITEMS>
+__global__ void __launch_bounds__(SORT_THREADS)
+onesweep_kernel(SortArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem<ITEMS>& s = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
+  constexpr int TILE = SORT_THREADS * ITEMS;
+  const uint32_t n = a.st->n;
+  const int num_tiles = (int)((n + TILE - 1) / TILE);
+  const uint32_t nb = min((uint32_t)gridDim.x, (uint32_t)num_tiles);  // blocks that own a tile
+  if (blockIdx.x >= nb) return;
+  uint32_t* bar = &a.st->sort_bar;
+  uint32_t round = 0, epoch = a.epoch0;
+
+  if (a.mode == SORT_SINGLE) {
+    const int in = a.pass & 1;
+    onesweep_pass<ITEMS>(s, a.key[in], a.val[in], a.key[in ^ 1], a.val[in ^ 1], a.st, a.pass, a.status, epoch, n, num_tiles);
+    return;
+  }
+  int buf = 0;
+  if (a.mode == SORT_HYBRID) {
+    for (int pass = 4; pass < 8; ++pass, buf ^= 1) {
+      onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch++, n, num_tiles);
+      grid_barrier(bar, nb, round);
+    }
+    fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles);
+    grid_barrier(bar, nb, round);
+    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) return;
+  }
+  for (int pass = 0; pass < 8; ++pass, buf ^= 1) {
+    onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch++, n, num_tiles);
+    if (pass < 7) grid_barrier(bar, nb, round);
   }
 }
 

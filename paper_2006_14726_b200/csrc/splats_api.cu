@@ -22,6 +22,8 @@ using namespace sw;
 
 constexpr int SORT_ITEMS = 16;
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
+static_assert(SPLATS_SORT_HYBRID == SORT_HYBRID && SPLATS_SORT_LSD8 == SORT_LSD8 && SPLATS_SORT_LSD8_LAUNCHES == SORT_SINGLE,
+              "public sort modes must match onesweep.cuh");
 
 struct Context {
   cudaStream_t stream = nullptr;
@@ -42,6 +44,7 @@ struct Context {
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
   PyramidLayout pyr_layout;
   int refit_mode = SPLATS_REFIT_PYRAMID;
+  int sort_mode = SPLATS_SORT_HYBRID;
   float* stage_color = nullptr;     // staging for the *_host calls
   float* stage_depth = nullptr;
   float* stage_out = nullptr;
@@ -162,10 +165,25 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   if (prof) m[2] = c->mark();
   const int max_sort_tiles = (int)((P + SORT_TILE - 1) / SORT_TILE);
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
-  for (int pass = 0; pass < 8; ++pass) {
-    const int in = pass & 1;
-    onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(
-        c->key[in], c->val[in], c->key[in ^ 1], c->val[in ^ 1], st, pass, c->status, ++c->epoch);
+  SortArgs sa;
+  sa.key[0] = c->key[0]; sa.key[1] = c->key[1];
+  sa.val[0] = c->val[0]; sa.val[1] = c->val[1];
+  sa.st = st;
+  sa.status = c->status;
+  sa.mode = c->sort_mode;
+  int sort_launches = 1;
+  if (c->sort_mode == SORT_SINGLE) {
+    sort_launches = 8;
+    for (int pass = 0; pass < 8; ++pass) {
+      sa.pass = pass;
+      sa.epoch0 = ++c->epoch;
+      onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
+    }
+  } else {
+    sa.pass = 0;
+    sa.epoch0 = c->epoch + 1;
+    c->epoch += 12;
+    onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
   }
   if (prof) m[3] = c->mark();
   const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
@@ -183,7 +201,7 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
     emit_boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->sphere, c->pyr, st, c->nodes);
   }
   if (prof) m[5] = c->mark();
-  c->launches += 12;
+  c->launches += 4 + sort_launches;
   if (prof)
     for (int i = 0; i < 5; ++i) c->spans.push_back({i, m[i], m[i + 1]});
   CU(cudaGetLastError());
@@ -409,6 +427,11 @@ int splats_set_option(int option, int value) {
     case SPLATS_OPT_REFIT:
       if (value != SPLATS_REFIT_PYRAMID && value != SPLATS_REFIT_ATOMIC) return fail(SPLATS_EINVAL, "unknown refit mode");
       g_ctx->refit_mode = value;
+      return SPLATS_OK;
+    case SPLATS_OPT_SORT:
+      if (value != SPLATS_SORT_HYBRID && value != SPLATS_SORT_LSD8 && value != SPLATS_SORT_LSD8_LAUNCHES)
+        return fail(SPLATS_EINVAL, "unknown sort mode");
+      g_ctx->sort_mode = value;
       return SPLATS_OK;
     default:
       return fail(SPLATS_EINVAL, "unknown option");

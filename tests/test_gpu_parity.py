@@ -147,6 +147,46 @@ def test_atomic_refit_mode_gives_the_same_tree():
             sp.splats_set_option(99, 0)
 
 
+def _top_runs(codes):
+    hi = codes >> np.uint64(32)
+    brk = np.flatnonzero(np.r_[True, hi[1:] != hi[:-1], True])
+    return np.diff(brk)
+
+
+@pytest.mark.parametrize("outlier,kind", [(300.0, "short"), (600.0, "short"), (2000.0, "long"), (5000.0, "long")])
+def test_hybrid_sort_fixup_and_fallback(outlier, kind):
+    # The hybrid sort orders by the top 31 code bits and repairs runs that share them: an outlier
+    # stretches the bounds until several splats fall into one cell of the top bits.  Short runs
+    # (<= 32) are fixed in place, longer ones trigger the full 8-pass sort; same result either way.
+    W, H = 64, 64
+    color, depth, cam = synth.random_frame(W, H, seed=21, fill=0.8)
+    depth[depth > 0] = 3.0
+    depth[0, 0] = outlier
+    with Session(W, H) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(4.0)], mode="bvh")
+        L = _top_runs(sc["sorted_codes"])
+        if kind == "short":
+            assert (L > 1).sum() > 100 and L.max() <= 32   # the case really exercises the fix-up
+        else:
+            assert L.max() > 32                             # ... and this one the fallback
+        # a second frame in the same context: the fallback flag and barrier are re-armed
+        c2, d2, cam2 = synth.random_frame(100, 37, seed=77, fill=0.5)
+        check_scene(s, c2, d2, cam2, 100, 37, 1.0, [synth.orbit_camera(4.0)], [(64, 64)], mode="bvh")
+
+
+@pytest.mark.parametrize("mode", ["lsd8", "lsd8_launches"])
+def test_sort_modes_give_the_same_order(mode):
+    cfg = synth.make_config(1)
+    color, depth = synth.source_frame(cfg, 0)
+    with Session(cfg.W, cfg.H) as s:
+        sp.splats_set_option(sp.OPT_SORT, sp.SORT_LSD8 if mode == "lsd8" else sp.SORT_LSD8_LAUNCHES)
+        check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams[:1], mode="bvh")
+        c2, d2, cam2 = synth.random_frame(127, 65, seed=3, fill=0.4)
+        check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
+        with pytest.raises(sp.SplatsError):
+            sp.splats_set_option(sp.OPT_SORT, 9)
+
+
 def test_repeated_updates_and_size_changes():
     # frame-parity double buffering: A, B (other size), A again must reproduce A
     cfg = synth.make_config(0)
