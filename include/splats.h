@@ -81,9 +81,13 @@ int splats_update(const float* color, const float* depth, const wr_camera* src_c
  * Errors: EINVAL as above, ENOBVH if no update was enqueued yet. */
 int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
 
-/* The same two calls with HOST buffers (end-to-end path): the library copies the frame to
- * device staging memory (cudaMemcpyAsync on the stream), runs the same kernels, and for the
- * render copies the image back; splats_render_host returns after the image is in out_rgba. */
+/* The same two calls with HOST buffers (end-to-end path).  Both only ENQUEUE and return: the
+ * frame is uploaded on a copy stream of the library into one of two device staging buffers,
+ * the kernels wait for it on the compute stream, and each rendered image is read back on a
+ * second copy stream from one of three device staging buffers, so the upload of the next
+ * frame and the read-back of the previous image overlap the kernels.  Pinned host memory
+ * makes the copies asynchronous.  The host buffers must stay valid, and out_rgba_host is
+ * complete, only after splats_synchronize().  Results are bit-identical to the device calls. */
 int splats_update_host(const float* color_host, const float* depth_host,
                        const wr_camera* src_camera, int W, int H, float r_scale);
 int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_rgba_host);
@@ -147,7 +151,7 @@ int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls
 /* How many kernels this library has launched since splats_create. */
 unsigned long long splats_launch_count(void);
 
-/* Block until everything enqueued so far has run. */
+/* Block until everything enqueued so far has run (kernels and the *_host copies). */
 int splats_synchronize(void);
 
 const char* splats_last_error(void);

@@ -45,9 +45,16 @@ struct Context {
   PyramidLayout pyr_layout;
   int refit_mode = SPLATS_REFIT_PYRAMID;
   int sort_mode = SPLATS_SORT_HYBRID;
-  float* stage_color = nullptr;     // staging for the *_host calls
-  float* stage_depth = nullptr;
-  float* stage_out = nullptr;
+  // staging for the *_host calls: copies run on their own streams, double / triple buffered,
+  // so the upload of frame f+1 and the read-back of image i-1 overlap the kernels of image i
+  static constexpr int N_IN = 2, N_OUT = 3;
+  cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+  float* stage_color[N_IN] = {nullptr, nullptr};
+  float* stage_depth[N_IN] = {nullptr, nullptr};
+  float* stage_out[N_OUT] = {nullptr, nullptr, nullptr};
+  cudaEvent_t in_uploaded[N_IN] = {}, in_free[N_IN] = {};    // h2d done / kernels done reading
+  cudaEvent_t out_rendered[N_OUT] = {}, out_free[N_OUT] = {};  // render done / d2h done
+  unsigned n_uploads = 0, n_readbacks = 0;
   // frame bookkeeping
   unsigned frame = 0;               // number of updates enqueued
   int parity = 0;                   // FrameState of the latest update
@@ -131,16 +138,38 @@ void free_all(Context* c) {
   cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
-  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->stage_color); cudaFree(c->stage_depth); cudaFree(c->stage_out);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr);
+  for (int i = 0; i < Context::N_IN; ++i) {
+    cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
+    if (c->in_uploaded[i]) cudaEventDestroy(c->in_uploaded[i]);
+    if (c->in_free[i]) cudaEventDestroy(c->in_free[i]);
+  }
+  for (int i = 0; i < Context::N_OUT; ++i) {
+    cudaFree(c->stage_out[i]);
+    if (c->out_rendered[i]) cudaEventDestroy(c->out_rendered[i]);
+    if (c->out_free[i]) cudaEventDestroy(c->out_free[i]);
+  }
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+  if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
   for (auto& e : c->pool)
     if (e) cudaEventDestroy(e);
 }
 
 int ensure_staging(Context* c) {
-  if (!c->stage_color) {
-    CU(dmalloc(&c->stage_color, (size_t)c->cap * 4));
-    CU(dmalloc(&c->stage_depth, (size_t)c->cap));
-    CU(dmalloc(&c->stage_out, (size_t)c->cap * 4));
+  if (!c->h2d_stream) {
+    CU(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < Context::N_IN; ++i) {
+      CU(dmalloc(&c->stage_color[i], (size_t)c->cap * 4));
+      CU(dmalloc(&c->stage_depth[i], (size_t)c->cap));
+      CU(cudaEventCreateWithFlags(&c->in_uploaded[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&c->in_free[i], cudaEventDisableTiming));
+    }
+    for (int i = 0; i < Context::N_OUT; ++i) {
+      CU(dmalloc(&c->stage_out[i], (size_t)c->cap * 4));
+      CU(cudaEventCreateWithFlags(&c->out_rendered[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&c->out_free[i], cudaEventDisableTiming));
+    }
   }
   return SPLATS_OK;
 }
@@ -342,9 +371,17 @@ int splats_update_host(const float* color_host, const float* depth_host, const w
   rc = ensure_staging(c);
   if (rc) return rc;
   const size_t P = (size_t)W * H;
-  CU(cudaMemcpyAsync(c->stage_color, color_host, P * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-  CU(cudaMemcpyAsync(c->stage_depth, depth_host, P * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-  return do_update(c, c->stage_color, c->stage_depth, src_camera, W, H, r_scale);
+  const int u = (int)(c->n_uploads % Context::N_IN);
+  if (c->n_uploads >= (unsigned)Context::N_IN) CU(cudaStreamWaitEvent(c->h2d_stream, c->in_free[u], 0));
+  CU(cudaMemcpyAsync(c->stage_color[u], color_host, P * 4 * sizeof(float), cudaMemcpyHostToDevice, c->h2d_stream));
+  CU(cudaMemcpyAsync(c->stage_depth[u], depth_host, P * sizeof(float), cudaMemcpyHostToDevice, c->h2d_stream));
+  CU(cudaEventRecord(c->in_uploaded[u], c->h2d_stream));
+  CU(cudaStreamWaitEvent(c->stream, c->in_uploaded[u], 0));
+  rc = do_update(c, c->stage_color[u], c->stage_depth[u], src_camera, W, H, r_scale);
+  if (rc) return rc;
+  CU(cudaEventRecord(c->in_free[u], c->stream));
+  c->n_uploads += 1;
+  return SPLATS_OK;
 }
 
 int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_rgba_host) {
@@ -354,10 +391,16 @@ int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_r
   if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_host before any update");
   rc = ensure_staging(c);
   if (rc) return rc;
-  rc = do_render(c, dst_camera, W2, H2, c->stage_out);
+  const int r = (int)(c->n_readbacks % Context::N_OUT);
+  if (c->n_readbacks >= (unsigned)Context::N_OUT) CU(cudaStreamWaitEvent(c->stream, c->out_free[r], 0));
+  rc = do_render(c, dst_camera, W2, H2, c->stage_out[r]);
   if (rc) return rc;
-  CU(cudaMemcpyAsync(out_rgba_host, c->stage_out, (size_t)W2 * H2 * 4 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
-  CU(cudaStreamSynchronize(c->stream));
+  CU(cudaEventRecord(c->out_rendered[r], c->stream));
+  CU(cudaStreamWaitEvent(c->d2h_stream, c->out_rendered[r], 0));
+  CU(cudaMemcpyAsync(out_rgba_host, c->stage_out[r], (size_t)W2 * H2 * 4 * sizeof(float), cudaMemcpyDeviceToHost,
+                     c->d2h_stream));
+  CU(cudaEventRecord(c->out_free[r], c->d2h_stream));
+  c->n_readbacks += 1;
   return SPLATS_OK;
 }
 
@@ -468,6 +511,10 @@ unsigned long long splats_launch_count(void) { return g_ctx ? g_ctx->launches : 
 int splats_synchronize(void) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   CU(cudaStreamSynchronize(g_ctx->stream));
+  if (g_ctx->h2d_stream) {
+    CU(cudaStreamSynchronize(g_ctx->h2d_stream));
+    CU(cudaStreamSynchronize(g_ctx->d2h_stream));
+  }
   return SPLATS_OK;
 }
 
@@ -489,6 +536,7 @@ const char* splats_last_error(void) { return g_err.c_str(); }
 void splats_destroy(void) {
   if (!g_ctx) return;
   cudaStreamSynchronize(g_ctx->stream);
+  if (g_ctx->h2d_stream) { cudaStreamSynchronize(g_ctx->h2d_stream); cudaStreamSynchronize(g_ctx->d2h_stream); }
   free_all(g_ctx);
   delete g_ctx;
   g_ctx = nullptr;

@@ -213,7 +213,31 @@ def test_host_buffer_entry_points_match_device_ones():
         ho = torch.empty((64, 64, 4), dtype=torch.float32).pin_memory()
         sp.splats_update_host(hc, hd, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
         sp.splats_render_host(cfg.dst_cams[0], 64, 64, ho)
+        sp.splats_synchronize()
         assert np.array_equal(ho.numpy(), a)
+
+
+def test_host_pipeline_many_frames_in_flight():
+    # more updates / renders in flight than staging buffers (2 in, 3 out): every image must be
+    # the one its own frame and camera give, whatever the copy streams overlap
+    frames = [synth.random_frame(96, 54, seed=100 + i, fill=0.5 + 0.05 * i) for i in range(5)]
+    cams = [synth.orbit_camera(2.0 * j) for j in range(4)]
+    with Session(96, 54) as s:
+        ref = []
+        for color, depth, cam in frames:
+            s.update(color, depth, cam, 96, 54, 1.5)
+            ref.append([s.render(c, 96, 54) for c in cams])
+        hc = [torch.from_numpy(f[0]).pin_memory() for f in frames]
+        hd = [torch.from_numpy(f[1]).pin_memory() for f in frames]
+        ho = [[torch.empty((54, 96, 4), dtype=torch.float32).pin_memory() for _ in cams] for _ in frames]
+        for i, (color, depth, cam) in enumerate(frames):
+            sp.splats_update_host(hc[i], hd[i], cam, 96, 54, 1.5)
+            for j, c in enumerate(cams):
+                sp.splats_render_host(c, 96, 54, ho[i][j])
+        sp.splats_synchronize()
+        for i in range(len(frames)):
+            for j in range(len(cams)):
+                assert np.array_equal(ho[i][j].numpy(), ref[i][j]), (i, j)
 
 
 def test_error_codes():
