@@ -4,8 +4,8 @@
 Workload (N=1): BASELINE.json configs[3] -- 256^3 volume, 1920x1080 source frames, 60 display
 frames with the camera dollying towards the centre, a splat + BVH rebuild every 4th frame.
 One *step* = one pass of the whole hot path over one source frame: 1 splats_update (bounds,
-unproject+Morton+compaction, 8 onesweep passes, hierarchy+gather, refit) followed by the 4
-splats_render calls of the display frames that use that BVH.  Step k uses source frame k mod 15,
+unproject+Morton+compaction, onesweep sort, gather+box pyramid, hierarchy+node boxes; 5 launches)
+followed by the 4 splats_render calls of the display frames that use that BVH.  Step k uses source frame k mod 15,
 so 15 steps are exactly the scripted 60-frame sequence.  value = display frames / second.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
@@ -40,8 +40,8 @@ FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
 # DRAM bytes per launch from the `ncu --set full` captures summarised under profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum); None until a capture exists for that kernel.
 NCU_TRAFFIC_BYTES = {
-    "render": None,
-    "sort": None,
+    "render": 21.5e6,   # profiles/r01b_ncu_full_summary.txt (source frame 10, cold L2: BVH + splats read once)
+    "sort": 2.9e6,      # the 5 MB working set stays in L2 between the passes
 }
 
 
@@ -81,7 +81,9 @@ def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
     return {
         "bounds": 4 * P + 4 * (P // 2048 + 1),
         "unproject_morton_compact": 4 * P + 12 * N,
-        "sort": 8 * 24 * N,                       # 8 passes x (read 12 N + write 12 N)
+        # hybrid onesweep (default): 4 passes over the top 31 code bits x (read 12 N + write 12 N)
+        # + the neighbour check reading the keys once (8 N); the all-8-pass fallback is not counted
+        "sort": 4 * 24 * N + 8 * N,
         # pyramid mode: gather (perm 4, depth 4, colour 16) -> sphere 16 + rgba 16 + pyramid 32 (N entries)
         "tree_1": (4 + 4 + 16) * N + (16 + 16 + 32) * N,
         # keys 8 + sphere 16 + pyramid 32 read once, 64-byte node records written once
@@ -243,7 +245,7 @@ def run_ours(args):
         if calls == 0:
             continue
         gbs = bytes_sum[name] / (ms_sum * 1e-3) / 1e9 if ms_sum > 0 else 0.0
-        kernels.append({"stage": name, "launches_per_call": 8 if name == "sort" else 1, "calls": calls,
+        kernels.append({"stage": name, "launches_per_call": 1, "calls": calls,
                         "ms_avg": ms_sum / calls, "share": ms_sum / ms_total, "algorithmic_bytes_avg": bytes_sum[name] / calls,
                         "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak})
     dominant = max(kernels, key=lambda r: r["share"])
@@ -276,7 +278,7 @@ def run_ours(args):
                              "the image written once plus BVH and splats read once (DESIGN.md sec. 6)"},
         "roofline_build": {"bound": "hbm", "achieved": build_bytes / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                            "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": build_bytes,
-                           "note": "all build kernels of one splats_update (12 launches), events inside the timed region"},
+                           "note": "all build kernels of one splats_update (5 launches), events inside the timed region"},
         "kernels": kernels,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
