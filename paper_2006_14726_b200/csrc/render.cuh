@@ -184,8 +184,13 @@ render_kernel(RenderParams prm) {
     }
     continue;
   }
-  const int sw = rw >> 1, super = tile >> 2;        // the rectangle is aligned to supertiles
-  const int ty = (super / sw) * 2 + ((tile >> 1) & 1), tx = (super % sw) * 2 + (tile & 1);
+  // The rectangle is aligned to supertiles.  Supertile rows are handed out from the middle of
+  // the rectangle outwards (mid, mid-1, mid+1, ...): the rows that are likely to hold the most
+  // hits start first and the kernel's tail is made of the cheap rows at the top and bottom edge.
+  const int sw = rw >> 1, sh = (ry1 - ry0) >> 1, super = tile >> 2;
+  const int rr = super / sw;
+  const int srow = (sh >> 1) + ((rr & 1) ? -((rr + 1) >> 1) : (rr >> 1));
+  const int ty = srow * 2 + ((tile >> 1) & 1), tx = (super - rr * sw) * 2 + (tile & 1);
   const int x = (rx0 + tx) * 8 + (lane & 7);
   const int y = (ry0 + ty) * 4 + (lane >> 3);
   const bool inside = x < cam.W && y < cam.H;
