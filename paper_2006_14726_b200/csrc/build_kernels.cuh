@@ -138,8 +138,9 @@ __device__ __forceinline__ uint64_t morton63(const float p[3], const float lo[3]
 __global__ void __launch_bounds__(BUILD_THREADS)
 unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevCamera cam,
                  FrameState* __restrict__ st, FrameState* __restrict__ st_next,
-                 const uint32_t* __restrict__ tile_count, uint64_t* __restrict__ keys,
-                 uint32_t* __restrict__ ids) {
+                 const uint32_t* __restrict__ tile_count, uint64_t* __restrict__ keys0,
+                 uint32_t* __restrict__ ids0, uint64_t* __restrict__ keys1, uint32_t* __restrict__ ids1,
+                 int sort_mode) {
   __shared__ uint32_t s_hist[8][256];
   __shared__ uint32_t s_warp[BUILD_THREADS / 32];
   __shared__ uint32_t s_part[BUILD_THREADS / 32];
@@ -158,6 +159,10 @@ unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevC
 #pragma unroll
   for (int d = 0; d < 8; ++d) s_hist[d][tid] = 0u;
 
+  // the sort ping-pongs between two buffers and must end in buffer 0 (onesweep.cuh)
+  const bool odd = sort_input_buffer(sort_mode, st->n) != 0;
+  uint64_t* __restrict__ keys = odd ? keys1 : keys0;
+  uint32_t* __restrict__ ids = odd ? ids1 : ids0;
   float lo[3], ext[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {

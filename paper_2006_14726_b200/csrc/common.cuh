@@ -76,6 +76,18 @@ struct FrameState {
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
 
+// ---- sort modes (onesweep.cuh) and what the producer of the keys must know about them
+constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
+// Which buffer unproject_kernel writes the unsorted pairs to, so that the sorted result always
+// ends in buffer 0: the hybrid mode runs 4 passes (digits 4..7) up to HYBRID5_MIN elements and 5
+// passes (digits 3..7) above it, where the cells of the top 31 bits are coarser than the sample
+// pitch of a dense frame; an odd number of passes starts in buffer 1.
+constexpr uint32_t HYBRID5_MIN = 1u << 21;
+__host__ __device__ __forceinline__ int hybrid_first_digit(uint32_t n) { return n > HYBRID5_MIN ? 3 : 4; }
+__host__ __device__ __forceinline__ int sort_input_buffer(int mode, uint32_t n) {
+  return (mode == SORT_HYBRID && (hybrid_first_digit(n) & 1)) ? 1 : 0;
+}
+
 // 64-byte BVH node: both child boxes live in the parent, so one node fetch (four 16-byte
 // vector loads from one 64-byte-aligned record) tests both children.
 //   b[0..5]  left child box  lo xyz, hi xyz      b[6..11] right child box

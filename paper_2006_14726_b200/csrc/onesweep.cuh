@@ -40,7 +40,6 @@ constexpr uint64_t FLAG_INC = 2ull << 30;  // inclusive prefix available
 constexpr uint32_t VALUE_MASK = (1u << 30) - 1;
 constexpr int LOOKBACK = 8;
 constexpr int RUN_MAX = 32;           // longest run of equal top bits fixed up in place
-constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
 
 struct SortArgs {
   uint64_t* key[2];
@@ -52,14 +51,14 @@ struct SortArgs {
   int pass;          // SORT_SINGLE: the digit; input buffer = pass & 1
 };
 
-template <int ITEMS>
+constexpr int SORT_MAX_ITEMS = 16;
 struct SortSmem {
   uint32_t warp_hist[SORT_WARPS][RADIX];  // per-warp digit counts -> exclusive prefix over warps
   uint32_t tile_off[RADIX];               // exclusive scan of the tile's digit counts
   int64_t bin_base[RADIX];                // global position of local slot 0 of each digit
   uint32_t digit_base[RADIX];             // exclusive scan of the global histogram
   uint32_t scan_tmp[SORT_WARPS];
-  uint64_t stage[SORT_THREADS * ITEMS];   // keys (then values) in tile-sorted order
+  uint64_t stage[SORT_THREADS * SORT_MAX_ITEMS];   // keys (then values) in tile-sorted order
 };
 
 // exclusive scan of one value per thread over the 256-thread block
@@ -101,7 +100,7 @@ __device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t nb, uint32_
 
 // One 8-bit pass over all tiles of this block: in -> out.
 template <int ITEMS>
-__device__ __forceinline__ void onesweep_pass(SortSmem<ITEMS>& s, const uint64_t* kin, const uint32_t* vin,
+__device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, const uint32_t* vin,
                                               uint64_t* kout, uint32_t* vout, const FrameState* st, int pass,
                                               uint64_t* status, uint32_t epoch, uint32_t n, int num_tiles) {
   constexpr int TILE = SORT_THREADS * ITEMS;
@@ -247,7 +246,7 @@ __device__ __forceinline__ void onesweep_pass(SortSmem<ITEMS>& s, const uint64_t
 // insertion sort by the full code; equal codes keep their order, which is id order); a longer
 // run raises st->sort_fallback.
 template <int ITEMS>
-__device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, int num_tiles) {
+__device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, int num_tiles, int low) {
   constexpr int TILE = SORT_THREADS * ITEMS;
   for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
     const uint32_t tile_base = (uint32_t)tile * TILE;
@@ -257,10 +256,10 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
       if (idx >= n) continue;
       const uint64_t k = __ldcg(key + idx);
       const uint64_t kn = idx + 1 < n ? __ldcg(key + idx + 1) : ~k;
-      if ((k >> 32) != (kn >> 32)) continue;                       // common case: no run continues here
-      if (idx > 0 && (__ldcg(key + idx - 1) >> 32) == (k >> 32)) continue;  // not the head
+      if ((k >> low) != (kn >> low)) continue;                     // common case: no run continues here
+      if (idx > 0 && (__ldcg(key + idx - 1) >> low) == (k >> low)) continue;  // not the head
       uint32_t len = 2;
-      while (len <= RUN_MAX && idx + len < n && (__ldcg(key + idx + len) >> 32) == (k >> 32)) ++len;
+      while (len <= RUN_MAX && idx + len < n && (__ldcg(key + idx + len) >> low) == (k >> low)) ++len;
       if (len > RUN_MAX) {
         st->sort_fallback = 1u;
         continue;
@@ -286,37 +285,48 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
 }
 
 template <int ITEMS>
-__global__ void __launch_bounds__(SORT_THREADS)
-onesweep_kernel(SortArgs a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  SortSmem<ITEMS>& s = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
+__device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_t n) {
   constexpr int TILE = SORT_THREADS * ITEMS;
-  const uint32_t n = a.st->n;
   const int num_tiles = (int)((n + TILE - 1) / TILE);
   const uint32_t nb = min((uint32_t)gridDim.x, (uint32_t)num_tiles);  // blocks that own a tile
   if (blockIdx.x >= nb) return;
   uint32_t* bar = &a.st->sort_bar;
   uint32_t round = 0, epoch = a.epoch0;
-
   if (a.mode == SORT_SINGLE) {
     const int in = a.pass & 1;
     onesweep_pass<ITEMS>(s, a.key[in], a.val[in], a.key[in ^ 1], a.val[in ^ 1], a.st, a.pass, a.status, epoch, n, num_tiles);
     return;
   }
-  int buf = 0;
-  if (a.mode == SORT_HYBRID) {
-    for (int pass = 4; pass < 8; ++pass, buf ^= 1) {
-      onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch++, n, num_tiles);
-      grid_barrier(bar, nb, round);
-    }
-    fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles);
-    grid_barrier(bar, nb, round);
-    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) return;
-  }
-  for (int pass = 0; pass < 8; ++pass, buf ^= 1) {
+  int first = a.mode == SORT_HYBRID ? hybrid_first_digit(n) : 0;
+  int buf = sort_input_buffer(a.mode, n);
+  for (int pass = first;;) {
     onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch++, n, num_tiles);
-    if (pass < 7) grid_barrier(bar, nb, round);
+    buf ^= 1;
+    if (++pass < 8) {
+      grid_barrier(bar, nb, round);
+      continue;
+    }
+    if (first == 0) break;  // all 8 digits sorted
+    grid_barrier(bar, nb, round);
+    fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
+    grid_barrier(bar, nb, round);
+    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) break;
+    first = 0;  // a long run of equal top bits: redo the sort with all 8 passes
+    pass = 0;
   }
+}
+
+// The tile size follows N (known on the device only): small frames are latency bound, so they
+// get small tiles (more blocks busy, shorter ranking chains); large ones get 4096-element tiles.
+__global__ void __launch_bounds__(SORT_THREADS)
+onesweep_kernel(SortArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
+  const uint32_t n = a.st->n;
+  const uint32_t slots = gridDim.x * SORT_THREADS;
+  if (n <= slots * 4u) run_sort<4>(s, a, n);
+  else if (n <= slots * 8u) run_sort<8>(s, a, n);
+  else run_sort<16>(s, a, n);
 }
 
 }  // namespace sw

@@ -20,8 +20,7 @@ namespace {
 
 using namespace sw;
 
-constexpr int SORT_ITEMS = 16;
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
+constexpr int SORT_MIN_TILE = SORT_THREADS * 4;  // smallest tile of onesweep_kernel
 static_assert(SPLATS_SORT_HYBRID == SORT_HYBRID && SPLATS_SORT_LSD8 == SORT_LSD8 && SPLATS_SORT_LSD8_LAUNCHES == SORT_SINGLE,
               "public sort modes must match onesweep.cuh");
 
@@ -190,9 +189,10 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   bounds_kernel<<<tiles, BUILD_THREADS, 0, s>>>(depth, P, dc, st, c->tile_count);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
-  unproject_kernel<<<grid2, BUILD_THREADS, 0, s>>>(depth, P, tiles, dc, st, st_next, c->tile_count, c->key[0], c->val[0]);
+  unproject_kernel<<<grid2, BUILD_THREADS, 0, s>>>(depth, P, tiles, dc, st, st_next, c->tile_count, c->key[0], c->val[0],
+                                                  c->key[1], c->val[1], c->sort_mode);
   if (prof) m[2] = c->mark();
-  const int max_sort_tiles = (int)((P + SORT_TILE - 1) / SORT_TILE);
+  const int max_sort_tiles = (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE);
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
   SortArgs sa;
   sa.key[0] = c->key[0]; sa.key[1] = c->key[1];
@@ -206,13 +206,13 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
     for (int pass = 0; pass < 8; ++pass) {
       sa.pass = pass;
       sa.epoch0 = ++c->epoch;
-      onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
+      onesweep_kernel<<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
     }
   } else {
     sa.pass = 0;
     sa.epoch0 = c->epoch + 1;
-    c->epoch += 12;
-    onesweep_kernel<SORT_ITEMS><<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
+    c->epoch += 16;
+    onesweep_kernel<<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
   }
   if (prof) m[3] = c->mark();
   const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
@@ -287,7 +287,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   c->cap = (int64_t)max_W * max_H;
   cudaError_t e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
   const size_t cap = (size_t)c->cap;
-  const size_t max_sort_tiles = (cap + SORT_TILE - 1) / SORT_TILE;
+  const size_t max_sort_tiles = (cap + SORT_MIN_TILE - 1) / SORT_MIN_TILE;
   if (e == cudaSuccess) e = dmalloc(&c->state, 2);
   if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
   if (e == cudaSuccess) e = dmalloc(&c->sched, 2);
@@ -320,12 +320,12 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
       e = cudaMemcpy(c->state + i, &init, sizeof(init), cudaMemcpyHostToDevice);
   }
   if (e == cudaSuccess) {
-    c->sort_smem = sizeof(SortSmem<SORT_ITEMS>);
-    e = cudaFuncSetAttribute(onesweep_kernel<SORT_ITEMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem);
+    c->sort_smem = sizeof(SortSmem);
+    e = cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem);
   }
   int occ = 0;
   if (e == cudaSuccess)
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onesweep_kernel<SORT_ITEMS>, SORT_THREADS, c->sort_smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, onesweep_kernel, SORT_THREADS, c->sort_smem);
   if (e == cudaSuccess && occ < 1) { free_all(c); delete c; return fail(SPLATS_ECUDA, "onesweep kernel does not fit on an SM"); }
   if (e != cudaSuccess) {
     free_all(c);

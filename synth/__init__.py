@@ -228,3 +228,17 @@ def random_frame(W: int, H: int, seed: int, fill: float = 0.6, cam: np.ndarray |
     rgb = rng.uniform(0.0, 1.0, size=(H, W, 3)) * a
     color = np.concatenate([rgb, a], axis=2).astype(np.float32)
     return color, depth, (orbit_camera(0.0) if cam is None else cam)
+
+
+def dense_frame(W: int, H: int, seed: int, cam: np.ndarray | None = None):
+    """A fully covered frame of a smooth undulating surface (every pixel valid, alpha in
+    [0.5, 1]): the N = P upper bound of the build, where the build kernels
+    are bandwidth bound.  Not one of the five configs."""
+    rng = np.random.default_rng(seed)
+    y, x = np.mgrid[0:H, 0:W].astype(np.float32)
+    depth = (3.4 + 0.35 * np.sin(x / W * 9.0) * np.cos(y / H * 7.0)
+             + 0.05 * np.sin(x * 0.05) * np.sin(y * 0.043)).astype(np.float32)
+    a = rng.uniform(0.5, 1.0, size=(H, W, 1))
+    rgb = rng.uniform(0.0, 1.0, size=(H, W, 3)) * a
+    color = np.concatenate([rgb, a], axis=2).astype(np.float32)
+    return color, depth, (orbit_camera(0.0) if cam is None else cam)
