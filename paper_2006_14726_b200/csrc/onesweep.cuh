@@ -38,7 +38,10 @@ constexpr int RADIX = 256;
 constexpr uint64_t FLAG_AGG = 1ull << 30;  // tile aggregate available
 constexpr uint64_t FLAG_INC = 2ull << 30;  // inclusive prefix available
 constexpr uint32_t VALUE_MASK = (1u << 30) - 1;
-constexpr int LOOKBACK = 8;
+#ifndef SPLATS_LOOKBACK
+#define SPLATS_LOOKBACK 8
+#endif
+constexpr int LOOKBACK = SPLATS_LOOKBACK;
 constexpr int RUN_MAX = 32;           // longest run of equal top bits fixed up in place
 
 struct SortArgs {
@@ -58,7 +61,8 @@ struct SortSmem {
   int64_t bin_base[RADIX];                // global position of local slot 0 of each digit
   uint32_t digit_base[RADIX];             // exclusive scan of the global histogram
   uint32_t scan_tmp[SORT_WARPS];
-  uint64_t stage[SORT_THREADS * SORT_MAX_ITEMS];   // keys (then values) in tile-sorted order
+  uint64_t stage[SORT_THREADS * SORT_MAX_ITEMS];   // keys in tile-sorted order
+  uint32_t vstage[SORT_THREADS * SORT_MAX_ITEMS];  // values in tile-sorted order
 };
 
 // exclusive scan of one value per thread over the 256-thread block
@@ -164,6 +168,19 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
     if (tile != 0) st_volatile_u64(my, ep | FLAG_AGG | count);
     const uint32_t toff = block_excl_scan_256(count, s.scan_tmp, nullptr);
     s.tile_off[tid] = toff;
+    __syncthreads();
+
+    // ---- keys and values into tile-sorted order in shared memory: this needs only the tile's
+    // own counts, so it is done before the look-back and frees the registers for it
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t dig = (uint32_t)(key[j] >> shift) & 0xff;
+      if ((wbase + j * 32) < n) {
+        const uint32_t slot = s.tile_off[dig] + s.warp_hist[warp][dig] + rank[j];
+        s.stage[slot] = key[j];
+        s.vstage[slot] = val[j];
+      }
+    }
 
     // ---- decoupled look-back for bin `tid`
     uint32_t excl;
@@ -171,9 +188,9 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
       excl = s.digit_base[tid];
     } else {
       excl = 0;
-      // LOOKBACK predecessors per round trip: in the one-wave regime (N below a few million)
-      // all tiles publish their aggregates at about the same time, so the walk back to tile 0
-      // is a chain of L2 round trips; independent loads cut it by the batch size.
+      // LOOKBACK predecessors per round trip: below a few million elements all tiles of a wave
+      // publish their aggregates at about the same time, so the walk back to an inclusive
+      // prefix is a chain of about tiles / (2 LOOKBACK) L2 round trips.
       int t = tile - 1;
       bool done = false;
       while (!done) {
@@ -202,40 +219,17 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
     s.bin_base[tid] = (int64_t)excl - (int64_t)toff;
     __syncthreads();
 
-    // ---- scatter keys into tile-sorted order in shared memory, then out (coalesced runs)
-    uint32_t slot[ITEMS];
-#pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-      const uint32_t dig = (uint32_t)(key[j] >> shift) & 0xff;
-      const bool valid = (wbase + j * 32) < n;
-      slot[j] = s.tile_off[dig] + s.warp_hist[warp][dig] + rank[j];
-      if (valid) s.stage[slot[j]] = key[j];
-    }
-    __syncthreads();
+    // ---- out: runs of equal digits are contiguous in shared memory and in global memory
     const uint32_t tile_n = min((uint32_t)TILE, n - tile_base);
-    uint8_t odig[ITEMS];
 #pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const uint32_t k = tid + j * SORT_THREADS;
       if (k < tile_n) {
         const uint64_t kk = s.stage[k];
-        odig[j] = (uint8_t)((kk >> shift) & 0xff);
-        __stcg(kout + (s.bin_base[odig[j]] + k), kk);
+        const int64_t pos = s.bin_base[(kk >> shift) & 0xff] + k;
+        __stcg(kout + pos, kk);
+        __stcg(vout + pos, s.vstage[k]);
       }
-    }
-    __syncthreads();
-    // ---- values the same way
-    uint32_t* vstage = reinterpret_cast<uint32_t*>(s.stage);
-#pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-      const uint32_t idx = wbase + j * 32;
-      if (idx < n) vstage[slot[j]] = val[j];
-    }
-    __syncthreads();
-#pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-      const uint32_t k = tid + j * SORT_THREADS;
-      if (k < tile_n) __stcg(vout + (s.bin_base[odig[j]] + k), vstage[k]);
     }
     __syncthreads();
   }
