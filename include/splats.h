@@ -81,6 +81,14 @@ int splats_update(const float* color, const float* depth, const wr_camera* src_c
  * Errors: EINVAL as above, ENOBVH if no update was enqueued yet. */
 int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
 
+/* The paper's own display query (sec. 4: "we render using first-hit ray tracing";
+ * PAPER.md:59 Fig. 2: "a simple first-hit ray tracing query and with no shading other than the
+ * constant sample color"): every destination pixel receives the
+ * stored colour of the sphere whose entry point is nearest along its ray -- order (t, splat
+ * id), same hit definition as splats_render -- and (0,0,0,0) if the ray enters no sphere.
+ * Nothing is composited.  Arguments, layout and errors as splats_render. */
+int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
+
 /* The same two calls with HOST buffers (end-to-end path).  Both only ENQUEUE and return: the
  * frame is uploaded on a copy stream of the library into one of two device staging buffers,
  * the kernels wait for it on the compute stream, and each rendered image is read back on a

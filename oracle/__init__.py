@@ -76,8 +76,8 @@ def lib():
         L.oracle_ray_sphere.restype = _i32
         L.oracle_composite.argtypes = [_i32, _vp, _vp, _vp, _vp]
         L.oracle_composite.restype = _i32
-        L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
-        L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _vp, _vp]
+        L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
+        L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
         _lib = L
     return _lib
 
@@ -187,9 +187,10 @@ def build_scene(color, depth, cam, W, H, r_scale):
                 rgba_sorted=rgba_sorted, children=children, parents=parents, ranges=ranges, aabbs=aabbs)
 
 
-def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False):
+def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False, first_hit=False):
     """O8..O9.  mode 'brute' = L0 (definition), 'bvh' = L1 (walk of the oracle's tree).
-    pixels: optional int64 array of destination pixel indices (y*W2+x)."""
+    pixels: optional int64 array of destination pixel indices (y*W2+x).
+    first_hit: the paper's first-hit query instead of compositing every hit."""
     cam = _f32(cam)
     n = scene["N"]
     if pixels is not None:
@@ -202,10 +203,10 @@ def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False):
     sp, co, ids = scene["sphere_sorted"], scene["rgba_sorted"], scene["sorted_ids"]
     if mode == "brute":
         lib().oracle_render_brute(_ptr(sp), _ptr(co), _ptr(ids), n, _ptr(cam), W2, H2, _ptr(pixels), total,
-                                  _ptr(out), _ptr(used))
+                                  1 if first_hit else 0, _ptr(out), _ptr(used))
     elif mode == "bvh":
         lib().oracle_render_bvh(_ptr(sp), _ptr(co), _ptr(ids), n, _ptr(scene["children"]), _ptr(scene["aabbs"]),
-                                _ptr(cam), W2, H2, _ptr(pixels), total, _ptr(out), _ptr(used))
+                                _ptr(cam), W2, H2, _ptr(pixels), total, 1 if first_hit else 0, _ptr(out), _ptr(used))
     else:
         raise ValueError(mode)
     if pixels is None:

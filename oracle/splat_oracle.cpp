@@ -129,6 +129,21 @@ int composite(std::vector<Hit>& hits, const float* rgba /*[N][4], sorted order*/
   return used;
 }
 
+// First-hit query -- the renderer the paper ships: "a simple first-hit ray tracing query and
+// with no shading other than the constant sample color" (Fig. 2; sec. 4).
+// The nearest accepted hit in (t, id) order supplies the pixel: its stored colour is copied,
+// nothing is composited.  No hit: background (0,0,0,0).  Returns 1 if there was a hit.
+int first_hit(const std::vector<Hit>& hits, const float* rgba /*[N][4], sorted order*/, float out[4]) {
+  out[0] = out[1] = out[2] = out[3] = 0.0f;
+  if (hits.empty()) return 0;
+  const Hit* best = &hits[0];
+  for (const Hit& h : hits)
+    if (hit_less(h, *best)) best = &h;
+  const float* col = rgba + 4 * (size_t)best->leaf;
+  for (int k = 0; k < 4; ++k) out[k] = col[k];
+  return 1;
+}
+
 // Conservative slab test for the BVH-walk renderer (unpinned on purpose): double
 // arithmetic on a box padded by far more than the float32 error of ray_sphere().
 bool ray_box_conservative(const float o[3], const float d[3], const float* box /*lo3,hi3*/) {
@@ -316,10 +331,11 @@ int oracle_composite(int n, const float* t, const uint32_t* id, const float* rgb
 // Arrays are in sorted order (any order gives the same image: hits are ordered by
 // (t, id)).  pixels == nullptr: whole frame into out[H2*W2*4]; otherwise only the
 // n_pixels listed pixel indices, out[n_pixels*4].  hits_used (optional) receives the
-// number of composited hits per output pixel.
+// number of composited hits per output pixel.  first_hit_only != 0: the paper's first-hit
+// query instead of compositing.
 void oracle_render_brute(const float* sphere, const float* rgba, const uint32_t* ids, int64_t N,
                          const float* cam13, int W2, int H2, const int64_t* pixels, int64_t n_pixels,
-                         float* out, int32_t* hits_used) {
+                         int first_hit_only, float* out, int32_t* hits_used) {
   Camera c = load_camera(cam13);
   int64_t total = pixels ? n_pixels : (int64_t)W2 * H2;
   std::vector<Hit> hits;
@@ -333,7 +349,7 @@ void oracle_render_brute(const float* sphere, const float* rgba, const uint32_t*
       float t;
       if (ray_sphere(c.e, dh, sphere + 4 * i, &t)) hits.push_back({t, ids[i], (uint32_t)i});
     }
-    int used = composite(hits, rgba, out + 4 * q);
+    int used = first_hit_only ? first_hit(hits, rgba, out + 4 * q) : composite(hits, rgba, out + 4 * q);
     if (hits_used) hits_used[q] = used;
   }
 }
@@ -356,7 +372,8 @@ void walk(int32_t id, int64_t N, const int32_t* children, const float* aabbs, co
 
 void oracle_render_bvh(const float* sphere, const float* rgba, const uint32_t* ids, int64_t N,
                        const int32_t* children, const float* aabbs, const float* cam13, int W2, int H2,
-                       const int64_t* pixels, int64_t n_pixels, float* out, int32_t* hits_used) {
+                       const int64_t* pixels, int64_t n_pixels, int first_hit_only, float* out,
+                       int32_t* hits_used) {
   Camera c = load_camera(cam13);
   int64_t total = pixels ? n_pixels : (int64_t)W2 * H2;
   std::vector<Hit> hits;
@@ -367,7 +384,7 @@ void oracle_render_bvh(const float* sphere, const float* rgba, const uint32_t* i
     pixel_ray(c, W2, H2, x, y, dh, &len);
     hits.clear();
     if (N > 0) walk(0, N, children, aabbs, sphere, ids, c.e, dh, hits);
-    int used = composite(hits, rgba, out + 4 * q);
+    int used = first_hit_only ? first_hit(hits, rgba, out + 4 * q) : composite(hits, rgba, out + 4 * q);
     if (hits_used) hits_used[q] = used;
   }
 }

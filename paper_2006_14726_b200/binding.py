@@ -49,6 +49,7 @@ def lib() -> ctypes.CDLL:
         L.splats_create.argtypes = [_vp, _ci, _ci]
         L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render_host.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_count.argtypes = [ctypes.POINTER(ctypes.c_uint)]
@@ -112,6 +113,11 @@ def splats_update(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, 
 def splats_render(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
     c = _cam(dst_camera)
     _check(lib().splats_render(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
+
+
+def splats_render_first_hit(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
+    c = _cam(dst_camera)
+    _check(lib().splats_render_first_hit(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
 
 
 def splats_update_host(color, depth, src_camera, W: int, H: int, r_scale: float) -> None:

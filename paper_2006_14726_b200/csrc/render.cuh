@@ -50,6 +50,7 @@ __device__ unsigned long long g_stats[8];  // 0 node visits, 1 sphere tests, 2 h
 
 // The K nearest hits beyond the cursor, sorted by (t, id); alpha rides along so that the
 // traversal knows the distance at which the ray becomes opaque.
+template <int KBUF>
 struct KBuffer {
   float t[KBUF];
   uint32_t leaf[KBUF];
@@ -130,6 +131,11 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 // warp tiles inside the rectangle are handed out dynamically: a warp's first tile is its index
 // in the grid, every further one comes from an atomic ticket; the last block to finish re-arms
 // the ticket for the next launch.
+//
+// FIRST = true is the paper's own query ("a simple first-hit ray tracing query and
+// with no shading other than the constant sample color"): a one-entry buffer keeps the nearest
+// hit in (t, id) order, everything beyond it is culled, and its stored colour is copied out.
+template <int KBUF, bool FIRST>
 __global__ void __launch_bounds__(RENDER_THREADS, 8)
 render_kernel(RenderParams prm) {
   __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
@@ -213,7 +219,7 @@ render_kernel(RenderParams prm) {
   float cur_t = -1.0f;
   uint32_t cur_id = 0;
   bool finished = !inside;
-  KBuffer kb;
+  KBuffer<KBUF> kb;
 
   while (__any_sync(0xffffffffu, !finished)) {
     if (!finished) {
@@ -282,22 +288,34 @@ render_kernel(RenderParams prm) {
               (t > cur_t || (t == cur_t && __ldg(prm.ids + leaf) > cur_id))) {
             STAT_ADD(2, 1);
             kb.insert(t, leaf, __ldg(&prm.rgba[leaf].w), prm.ids);
-            // distance at which the composite below (oracle step O9, same operations in the
-            // same order) reaches alpha >= 0.99: later hits cannot contribute
-            float a = A, t_cut = INF;
+            if (FIRST) {
+              t_hi = kb.t[0];  // nothing beyond the nearest hit so far matters
+            } else {
+              // distance at which the composite below (oracle step O9, same operations in the
+              // same order) reaches alpha >= 0.99: later hits cannot contribute
+              float a = A, t_cut = INF;
 #pragma unroll
-            for (int i = 0; i < KBUF; ++i) {
-              if (kb.leaf[i] != EMPTY_LEAF && t_cut == INF) {
-                a = fma_(sub_(1.0f, a), kb.al[i], a);
-                if (a >= 0.99f) t_cut = kb.t[i];
+              for (int i = 0; i < KBUF; ++i) {
+                if (kb.leaf[i] != EMPTY_LEAF && t_cut == INF) {
+                  a = fma_(sub_(1.0f, a), kb.al[i], a);
+                  if (a >= 0.99f) t_cut = kb.t[i];
+                }
               }
+              t_hi = fminf(kb.t[KBUF - 1], t_cut);
             }
-            t_hi = fminf(kb.t[KBUF - 1], t_cut);
           }
         }
         node = pop();
       }
 
+      if (FIRST) {  // copy the colour of the nearest hit; one traversal is always enough
+        if (kb.leaf[0] != EMPTY_LEAF) {
+          const float4 col = __ldg(prm.rgba + kb.leaf[0]);
+          C[0] = col.x; C[1] = col.y; C[2] = col.z; A = col.w;
+        }
+        finished = true;
+        continue;
+      }
       // ---- oracle step O9: composite the k-buffer front to back, stop at alpha >= 0.99
       bool opaque = false;
 #pragma unroll

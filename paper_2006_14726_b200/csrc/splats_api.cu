@@ -240,7 +240,7 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   return SPLATS_OK;
 }
 
-int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out) {
+int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false) {
   RenderParams prm;
   prm.cam = make_camera(cam, W2, H2);
   prm.nodes = c->nodes;
@@ -255,7 +255,8 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out) {
   const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
-  render_kernel<<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  if (first_hit) render_kernel<1, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  else render_kernel<KBUF, false><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
   if (c->profiling) c->spans.push_back({5, m0, c->mark()});
   c->launches += 1;
   CU(cudaGetLastError());
@@ -334,7 +335,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   }
   c->sort_grid = c->num_sms * occ;  // co-resident persistent grid (see onesweep.cuh)
   int rocc = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rocc, render_kernel, RENDER_THREADS, 0);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rocc, render_kernel<KBUF, false>, RENDER_THREADS, 0);
   if (e != cudaSuccess || rocc < 1) {
     free_all(c);
     delete c;
@@ -360,6 +361,14 @@ int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba) 
   if (reinterpret_cast<uintptr_t>(out_rgba) & 15u) return fail(SPLATS_EINVAL, "out_rgba must be 16-byte aligned");
   if (!g_ctx->has_bvh) return fail(SPLATS_ENOBVH, "splats_render before any splats_update");
   return do_render(g_ctx, dst_camera, W2, H2, out_rgba);
+}
+
+int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* out_rgba) {
+  int rc = check_frame_args(g_ctx, out_rgba, out_rgba, dst_camera, W2, H2);
+  if (rc) return rc;
+  if (reinterpret_cast<uintptr_t>(out_rgba) & 15u) return fail(SPLATS_EINVAL, "out_rgba must be 16-byte aligned");
+  if (!g_ctx->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_first_hit before any splats_update");
+  return do_render(g_ctx, dst_camera, W2, H2, out_rgba, true);
 }
 
 int splats_update_host(const float* color_host, const float* depth_host, const wr_camera* src_camera, int W, int H,

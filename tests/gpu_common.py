@@ -32,9 +32,9 @@ class Session:
         self.d_depth = torch.from_numpy(np.ascontiguousarray(depth, dtype=np.float32)).cuda()
         sp.splats_update(self.d_color, self.d_depth, cam, W, H, r_scale)
 
-    def render(self, cam, W2, H2):
+    def render(self, cam, W2, H2, first_hit=False):
         out = torch.full((H2, W2, 4), -7.0, dtype=torch.float32, device="cuda")
-        sp.splats_render(cam, W2, H2, out)
+        (sp.splats_render_first_hit if first_hit else sp.splats_render)(cam, W2, H2, out)
         torch.cuda.synchronize()
         return out.cpu().numpy()
 

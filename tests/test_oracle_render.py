@@ -162,3 +162,68 @@ def test_single_splat_scene():
     for mode in ("brute", "bvh"):
         out = oracle.render(sc, cam, 3, 3, mode)
         assert np.array_equal(out[1, 1], color[1, 1]) and out[..., 3].sum() == 0.5
+
+
+# ------------------------------------------------------------------ first-hit query
+def _coaxial(ts, ids, cols, radius=0.004):
+    """Spheres centred on the central ray of a 1x1 image at distances ts (array order as given)."""
+    cam = synth.orbit_camera(0.0)
+    e, F = cam[:3].astype(np.float64), cam[9:12].astype(np.float64)
+    sphere = np.array([[*(e + F * t), radius] for t in ts], np.float32)
+    return cam, dict(N=len(ts), sphere_sorted=sphere, rgba_sorted=np.asarray(cols, np.float32),
+                     sorted_ids=np.asarray(ids, np.uint32))
+
+
+def test_first_hit_takes_the_nearest_sphere_and_copies_its_colour():
+    # PAPER.md:59: "a simple first-hit ray tracing query ... no shading other than the constant
+    # sample color": whatever the array order, the nearest entry point wins and nothing behind
+    # it contributes, even when it is almost transparent.
+    cols = [[0.6, 0.0, 0.0, 0.6], [0.0, 0.02, 0.0, 0.05], [0.0, 0.0, 0.9, 1.0]]
+    for order in ([0, 1, 2], [2, 1, 0], [1, 2, 0]):
+        ts = [3.0, 2.0, 4.0]
+        cam, sc = _coaxial([ts[i] for i in order], order, [cols[i] for i in order])
+        for mode in ("brute",):
+            out, used = oracle.render(sc, cam, 1, 1, mode, return_hits=True, first_hit=True)
+            assert used[0, 0] == 1
+            assert np.array_equal(out[0, 0], np.asarray(cols[1], np.float32))
+        # compositing the same stack gives something else: all three contribute
+        allhit = oracle.render(sc, cam, 1, 1, "brute")
+        assert allhit[0, 0, 3] > 0.99 and allhit[0, 0, 2] > 0.3
+
+
+def test_first_hit_equal_t_is_decided_by_id():
+    cols = [[0.5, 0, 0, 0.5], [0, 0.5, 0, 0.5]]
+    for ids, want in (([7, 3], 1), ([3, 7], 0)):
+        cam, sc = _coaxial([2.5, 2.5], ids, cols)
+        out = oracle.render(sc, cam, 1, 1, "brute", first_hit=True)
+        assert np.array_equal(out[0, 0], np.asarray(cols[want], np.float32))
+
+
+@pytest.mark.parametrize("kind,r_scale", [("config0", 1.0), ("wide", 2.0), ("square", 3.0)])
+def test_first_hit_equals_compositing_of_opaque_splats_and_walk_equals_brute(kind, r_scale):
+    # With every alpha = 1 the first composited hit already reaches A >= 0.99, so the all-hit
+    # renderer degenerates to the first-hit query: the two independent code paths must agree.
+    color, depth, cam, W, H = _scene(kind)
+    opaque = color.copy()
+    opaque[..., 3] = 1.0
+    sc = oracle.build_scene(opaque, depth, cam, W, H, r_scale)
+    sc_t = oracle.build_scene(color, depth, cam, W, H, r_scale)   # translucent colours, same geometry
+    for dst in (synth.orbit_camera(5.0), synth.orbit_camera(-20.0, 10.0, 2.5)):
+        a = oracle.render(sc, dst, W, H, "brute")
+        f, used = oracle.render(sc, dst, W, H, "brute", first_hit=True, return_hits=True)
+        assert np.array_equal(a, f) and (a[..., 3] > 0).any()
+        assert set(np.unique(used)) <= {0, 1}
+        fb = oracle.render(sc_t, dst, W, H, "brute", first_hit=True)
+        fw = oracle.render(sc_t, dst, W, H, "bvh", first_hit=True)
+        assert np.array_equal(fb, fw)
+        # same geometry => same winner: the translucent image is the opaque one with the alpha swapped in
+        hit = f[..., 3] > 0
+        assert np.array_equal(fb[..., 3] > 0, hit)
+
+
+def test_first_hit_identity_camera_reproduces_source():
+    color, depth, cam, W, H = _scene("config0")
+    sc = oracle.build_scene(color, depth, cam, W, H, 1.0)
+    out = oracle.render(sc, cam, W, H, "bvh", first_hit=True)
+    v = (sc["valid"] == 1).reshape(H, W)
+    assert np.array_equal(out[v], color[v]) and np.all(out[~v] == 0)
