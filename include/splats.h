@@ -144,6 +144,23 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 #define SPLATS_SORT_LSD8_LAUNCHES  2
 int splats_set_option(int option, int value);
 
+/* How splats_update derives the radius of a splat (takes effect at the next update; SURVEY.md
+ * sec. 8(f) row 3).  r_scale of splats_update multiplies all of them.
+ *   SPLATS_RADIUS_FOOTPRINT (default; param ignored): half the diagonal of the pixel's footprint
+ *     at the splat's view-axis depth (north_star).
+ *   SPLATS_RADIUS_CONSTANT: one radius for every splat, r = r_scale * param; the paper sets it
+ *     "to half the size of a voxel's diagonal", which the caller passes as param
+ *     (object-space length, > 0).
+ *   SPLATS_RADIUS_OPACITY: footprint radius * (param + (1 - param) * alpha), param in [0, 1], alpha
+ *     the pixel's opacity: a reading of the paper's future-work idea of "varying the radius of
+ *     the object space samples according to their opacity"; a splat whose radius
+ *     comes out as 0 is kept (it can never be hit).
+ * Errors: EINVAL for an unknown mode or a param outside its range, ESTATE without a context. */
+#define SPLATS_RADIUS_FOOTPRINT 0
+#define SPLATS_RADIUS_CONSTANT  1
+#define SPLATS_RADIUS_OPACITY   2
+int splats_set_radius(int mode, float param);
+
 /* Per-stage device times, measured with CUDA events recorded on the library's stream around
  * each stage of every update / render issued while profiling is on.  Off by default (the
  * event records cost about a microsecond each).  splats_stage_ms synchronises the stream,

@@ -62,7 +62,7 @@ def lib():
         build()
         L = ctypes.CDLL(str(_LIB))
         L.oracle_pixel_ray.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp, _vp]
-        L.oracle_unproject.argtypes = [_vp, _vp, _i32, _i32, ctypes.c_float, _vp, _vp]
+        L.oracle_unproject.argtypes = [_vp, _vp, _i32, _i32, ctypes.c_float, _i32, ctypes.c_float, _vp, _vp, _vp]
         L.oracle_unproject.restype = _i64
         L.oracle_bounds.argtypes = [_vp, _vp, _i64, _vp, _vp]
         L.oracle_morton_point.argtypes = [_vp, _vp, _vp]
@@ -99,12 +99,17 @@ def pixel_ray(cam, W, H, x, y):
     return d, float(ln[0])
 
 
-def unproject(depth, cam, W, H, r_scale):
+RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
+
+
+def unproject(depth, cam, W, H, r_scale, radius_mode=RADIUS_FOOTPRINT, radius_param=0.0, color=None):
     depth, cam = _f32(depth).reshape(-1), _f32(cam)
     assert depth.size == W * H
     sphere = np.empty((W * H, 4), np.float32)
     valid = np.empty(W * H, np.uint8)
-    n = lib().oracle_unproject(_ptr(depth), _ptr(cam), W, H, float(r_scale), _ptr(sphere), _ptr(valid))
+    col = _f32(color).reshape(W * H, 4) if radius_mode == RADIUS_OPACITY else None
+    n = lib().oracle_unproject(_ptr(depth), _ptr(cam), W, H, float(r_scale), int(radius_mode), float(radius_param),
+                               _ptr(col), _ptr(sphere), _ptr(valid))
     return sphere, valid, int(n)
 
 
@@ -169,10 +174,10 @@ def composite(t, ids, rgba):
 
 
 # ------------------------------------------------------------------ whole path
-def build_scene(color, depth, cam, W, H, r_scale):
+def build_scene(color, depth, cam, W, H, r_scale, radius_mode=RADIUS_FOOTPRINT, radius_param=0.0):
     """O1..O7 on one 2.5D frame.  Returns a dict of numpy arrays (see keys below)."""
     color = _f32(color).reshape(W * H, 4)
-    sphere, valid, n = unproject(depth, cam, W, H, r_scale)
+    sphere, valid, n = unproject(depth, cam, W, H, r_scale, radius_mode, radius_param, color)
     lo, hi = bounds(sphere, valid)
     ids, codes = compact_codes(sphere, valid, lo, hi, n)
     order = sort_codes(codes)

@@ -65,6 +65,22 @@ float radius_factor(const Camera& c, int H, float r_scale) {
   return (r_scale * SQRT_HALF) * ((2.0f * c.tau) / (float)H);
 }
 
+// O2 variants.  mode 0: the footprint radius above.  mode 1: the
+// paper's own choice, one radius for every sample -- "half the size of a voxel's diagonal"
+// (PAPER.md:69); the caller passes that length as `param`, r = r_scale * param.  mode 2: a
+// reading of the future-work idea "varying the radius of the object space samples according to
+// their opacity": the footprint radius times f_min + (1 - f_min) * alpha, with
+// f_min = param in [0, 1], so that opaque samples keep their footprint and faint ones shrink.
+float splat_radius(int mode, float param, float r_scale, float k_r, float z, float alpha) {
+  if (mode == 1) return r_scale * param;
+  float r = k_r * z;
+  if (mode == 2) {
+    float w1 = 1.0f - param;
+    r = r * fmaf(w1, alpha, param);
+  }
+  return r;
+}
+
 // O3 -- PAPER.md:69: samples with zero radius never reach the client.
 bool depth_valid(float t) { return std::isfinite(t) && t > 0.0f; }
 
@@ -183,6 +199,7 @@ void oracle_pixel_ray(const float* cam13, int W, int H, int x, int y, float* dha
 // sphere[p] = (cx, cy, cz, r) and valid[p]; entries of invalid pixels are zeroed.
 // Returns N = number of valid pixels.
 int64_t oracle_unproject(const float* depth, const float* cam13, int W, int H, float r_scale,
+                         int radius_mode, float radius_param, const float* color /*[P][4], mode 2 only*/,
                          float* sphere /*[P][4]*/, uint8_t* valid /*[P]*/) {
   Camera c = load_camera(cam13);
   float k_r = radius_factor(c, H, r_scale);
@@ -197,7 +214,7 @@ int64_t oracle_unproject(const float* depth, const float* cam13, int W, int H, f
       pixel_ray(c, W, H, x, y, dh, &len);
       for (int k = 0; k < 3; ++k) s[k] = fmaf(t, dh[k], c.e[k]);  // Eq. 1
       float z = t / len;                                          // view-axis depth
-      s[3] = k_r * z;
+      s[3] = splat_radius(radius_mode, radius_param, r_scale, k_r, z, radius_mode == 2 ? color[4 * p + 3] : 0.0f);
       valid[p] = 1;
       ++n;
     }

@@ -19,6 +19,7 @@ NUM_STAGES = 6
 STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
+RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
 
 
 class SplatsError(RuntimeError):
@@ -57,6 +58,7 @@ def lib() -> ctypes.CDLL:
         L.splats_export_splats.argtypes = [_vp, _vp, _vp]
         L.splats_set_profiling.argtypes = [_ci]
         L.splats_set_option.argtypes = [_ci, _ci]
+        L.splats_set_radius.argtypes = [_ci, ctypes.c_float]
         L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_uint)]
         L.splats_launch_count.restype = ctypes.c_ulonglong
         L.splats_last_error.restype = ctypes.c_char_p
@@ -165,6 +167,10 @@ def splats_export_splats():
 
 def splats_set_option(option: int, value: int) -> None:
     _check(lib().splats_set_option(int(option), int(value)))
+
+
+def splats_set_radius(mode: int, param: float = 0.0) -> None:
+    _check(lib().splats_set_radius(int(mode), float(param)))
 
 
 def splats_set_profiling(on: bool) -> None:

@@ -53,6 +53,24 @@ __device__ __forceinline__ void splat_centre(const DevCamera& c, int x, int y, f
   for (int k = 0; k < 3; ++k) p[k] = fma_(t, d[k], c.e[k]);
 }
 
+// ---- splat radius (S2 and its variants)
+//   mode 0  footprint: r = k_r * z, k_r = (r_scale sqrt(1/2)) (2 tau / H)   (north_star)
+//   mode 1  constant:  r = r_const = r_scale * param; the paper's choice, param = half a
+//           voxel's diagonal
+//   mode 2  opacity:   r = (k_r * z) * fma(w1, alpha, f_min), f_min = param, w1 = 1 - f_min
+//           (a reading of PAPER.md:109 "varying the radius ... according to their opacity")
+// All constants are computed on the host in float32, one rounding per operation.
+struct RadiusParams {
+  int mode;
+  float k_r, r_const, f_min, w1;
+};
+__device__ __forceinline__ float splat_radius(const RadiusParams& rp, float z, float alpha) {
+  if (rp.mode == 1) return rp.r_const;
+  float r = mul_(rp.k_r, z);
+  if (rp.mode == 2) r = mul_(r, fma_(rp.w1, alpha, rp.f_min));
+  return r;
+}
+
 // ---- order-preserving float <-> uint32 map for atomicMin / atomicMax
 __device__ __forceinline__ uint32_t f2ord(float f) {
   uint32_t u = __float_as_uint(f);

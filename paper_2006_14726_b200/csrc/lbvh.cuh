@@ -24,7 +24,7 @@ __device__ __forceinline__ int delta(const uint64_t* __restrict__ keys, int n, i
 // doubling + binary search, split by binary search.
 __global__ void __launch_bounds__(LBVH_THREADS)
 emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm,
-            const float* __restrict__ depth, const float4* __restrict__ color, DevCamera cam, float k_r,
+            const float* __restrict__ depth, const float4* __restrict__ color, DevCamera cam, RadiusParams rp,
             const FrameState* __restrict__ st, float4* __restrict__ sphere, float4* __restrict__ rgba,
             Node* __restrict__ nodes, int* __restrict__ leaf_parent) {
   const int n = (int)st->n;
@@ -36,8 +36,9 @@ emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm
     float p[3], len;
     splat_centre(cam, x, y, t, p, len);
     const float z = div_(t, len);
-    sphere[i] = make_float4(p[0], p[1], p[2], mul_(k_r, z));
-    rgba[i] = __ldg(color + id);
+    const float4 col = __ldg(color + id);
+    sphere[i] = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
+    rgba[i] = col;
     if (n == 1) leaf_parent[0] = -1;
     if (i >= n - 1) continue;
 
@@ -135,7 +136,7 @@ __device__ __forceinline__ void box_of_sphere(const float4 sp, float lo[3], floa
 
 __global__ void __launch_bounds__(PYR_THREADS)
 leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const float* __restrict__ depth,
-                    const float4* __restrict__ color, DevCamera cam, float k_r, FrameState* st,
+                    const float4* __restrict__ color, DevCamera cam, RadiusParams rp, FrameState* st,
                     float4* __restrict__ sphere, float4* __restrict__ rgba, float4* pyr) {
   __shared__ float s_box[6][PYR_LEAVES];
   __shared__ bool s_last;
@@ -159,9 +160,10 @@ leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const float* __restrict__
       float p[3], len;
       splat_centre(cam, x, y, t, p, len);
       const float z = div_(t, len);
-      const float4 sp = make_float4(p[0], p[1], p[2], mul_(k_r, z));
+      const float4 col = __ldg(color + id);
+      const float4 sp = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
       sphere[i] = sp;
-      rgba[i] = __ldg(color + id);
+      rgba[i] = col;
       box_of_sphere(sp, lo, hi);
     }
 #pragma unroll

@@ -44,6 +44,8 @@ struct Context {
   PyramidLayout pyr_layout;
   int refit_mode = SPLATS_REFIT_PYRAMID;
   int sort_mode = SPLATS_SORT_HYBRID;
+  int radius_mode = SPLATS_RADIUS_FOOTPRINT;
+  float radius_param = 0.0f;
   // staging for the *_host calls: copies run on their own streams, double / triple buffered,
   // so the upload of frame f+1 and the read-back of image i-1 overlap the kernels of image i
   static constexpr int N_IN = 2, N_OUT = 3;
@@ -176,7 +178,16 @@ int ensure_staging(Context* c) {
 int do_update(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale) {
   const int64_t P = (int64_t)W * H;
   const DevCamera dc = make_camera(cam, W, H);
-  const float k_r = radius_factor(cam, H, r_scale);
+  RadiusParams rp;
+  rp.mode = c->radius_mode;
+  rp.k_r = radius_factor(cam, H, r_scale);
+  {
+    volatile float rc = r_scale * c->radius_param;   // separately rounded float32 operations
+    volatile float w1 = 1.0f - c->radius_param;
+    rp.r_const = rc;
+    rp.f_min = c->radius_param;
+    rp.w1 = w1;
+  }
   const int parity = (int)(c->frame & 1u);
   FrameState* st = c->state + parity;
   FrameState* st_next = c->state + (parity ^ 1);
@@ -219,12 +230,12 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
   if (c->refit_mode == SPLATS_REFIT_ATOMIC) {
     emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
-                                               k_r, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
+                                               rp, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
     if (prof) m[4] = c->mark();
     refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
   } else {
     const int pgrid = (int)((P + PYR_LEAVES - 1) / PYR_LEAVES);
-    leaf_pyramid_kernel<<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], depth, reinterpret_cast<const float4*>(color), dc, k_r,
+    leaf_pyramid_kernel<<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], depth, reinterpret_cast<const float4*>(color), dc, rp,
                                                       st, c->sphere, c->rgba, c->pyr);
     if (prof) m[4] = c->mark();
     emit_boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->sphere, c->pyr, st, c->nodes);
@@ -488,6 +499,19 @@ int splats_set_option(int option, int value) {
     default:
       return fail(SPLATS_EINVAL, "unknown option");
   }
+}
+
+int splats_set_radius(int mode, float param) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  if (mode != SPLATS_RADIUS_FOOTPRINT && mode != SPLATS_RADIUS_CONSTANT && mode != SPLATS_RADIUS_OPACITY)
+    return fail(SPLATS_EINVAL, "unknown radius mode");
+  if (mode == SPLATS_RADIUS_CONSTANT && !(param > 0.0f && std::isfinite(param)))
+    return fail(SPLATS_EINVAL, "constant radius must be finite and > 0");
+  if (mode == SPLATS_RADIUS_OPACITY && !(param >= 0.0f && param <= 1.0f))
+    return fail(SPLATS_EINVAL, "opacity radius floor must be in [0, 1]");
+  g_ctx->radius_mode = mode;
+  g_ctx->radius_param = mode == SPLATS_RADIUS_FOOTPRINT ? 0.0f : param;
+  return SPLATS_OK;
 }
 
 int splats_set_profiling(int on) {

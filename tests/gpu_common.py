@@ -70,9 +70,12 @@ def assert_rgba_close(got, ref, what=""):
     return float(err.max()), bad
 
 
-def check_scene(sess, color, depth, cam, W, H, r_scale, dst_cams, dst_sizes=None, mode="bvh", sample=None, seed=0):
-    """update + export parity + one render per destination camera."""
-    sc = oracle.build_scene(color, depth, cam, W, H, r_scale)
+def check_scene(sess, color, depth, cam, W, H, r_scale, dst_cams, dst_sizes=None, mode="bvh", sample=None, seed=0,
+                radius=(0, 0.0)):
+    """update + export parity + one render per destination camera.  radius = (mode, param) of
+    splats_set_radius / oracle.build_scene."""
+    sc = oracle.build_scene(color, depth, cam, W, H, r_scale, radius[0], radius[1])
+    sp.splats_set_radius(radius[0], radius[1])
     sess.update(color, depth, cam, W, H, r_scale)
     assert_bvh_bit_exact(sc)
     stats = []
