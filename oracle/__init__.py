@@ -64,6 +64,9 @@ def lib():
         L.oracle_pixel_ray.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp, _vp]
         L.oracle_unproject.argtypes = [_vp, _vp, _i32, _i32, ctypes.c_float, _i32, ctypes.c_float, _vp, _vp, _vp]
         L.oracle_unproject.restype = _i64
+        L.oracle_pack.argtypes = [_vp, _vp, _vp, _i32, _i32, ctypes.c_float, _i32, ctypes.c_float, _vp, _vp, _vp]
+        L.oracle_pack.restype = _i64
+        L.oracle_decode.argtypes = [_vp, _vp, _i64, _vp, _vp, _vp, _vp]
         L.oracle_bounds.argtypes = [_vp, _vp, _i64, _vp, _vp]
         L.oracle_morton_point.argtypes = [_vp, _vp, _vp]
         L.oracle_morton_point.restype = ctypes.c_uint64
@@ -111,6 +114,31 @@ def unproject(depth, cam, W, H, r_scale, radius_mode=RADIUS_FOOTPRINT, radius_pa
     n = lib().oracle_unproject(_ptr(depth), _ptr(cam), W, H, float(r_scale), int(radius_mode), float(radius_param),
                                _ptr(col), _ptr(sphere), _ptr(valid))
     return sphere, valid, int(n)
+
+
+def pack(color, depth, cam, W, H, r_scale, quant, radius_mode=RADIUS_FOOTPRINT, radius_param=0.0):
+    """Server side of the wire format: (samples uint64[n], colours uint32[n]).
+    quant = (lo xyz, hi xyz, r_max)."""
+    color, depth, cam, quant = _f32(color).reshape(W * H, 4), _f32(depth).reshape(-1), _f32(cam), _f32(quant)
+    assert quant.size == 7
+    samples = np.empty(W * H, np.uint64)
+    colours = np.empty(W * H, np.uint32)
+    n = lib().oracle_pack(_ptr(color), _ptr(depth), _ptr(cam), W, H, float(r_scale), int(radius_mode), float(radius_param),
+                          _ptr(quant), _ptr(samples), _ptr(colours))
+    return samples[:n].copy(), colours[:n].copy()
+
+
+def decode(samples, colours, quant):
+    """Client side: (sphere float32[n,4], rgba float32[n,4], valid uint8[n])."""
+    samples = np.ascontiguousarray(samples, dtype=np.uint64)
+    colours = np.ascontiguousarray(colours, dtype=np.uint32)
+    quant = _f32(quant)
+    n = samples.size
+    sphere = np.empty((n, 4), np.float32)
+    rgba = np.empty((n, 4), np.float32)
+    valid = np.empty(n, np.uint8)
+    lib().oracle_decode(_ptr(samples), _ptr(colours), n, _ptr(quant), _ptr(sphere), _ptr(rgba), _ptr(valid))
+    return sphere, rgba, valid
 
 
 def bounds(sphere, valid):
@@ -188,6 +216,24 @@ def build_scene(color, depth, cam, W, H, r_scale, radius_mode=RADIUS_FOOTPRINT, 
     children, parents, ranges = tree(sorted_codes)
     aabbs = refit(sphere_sorted, children)
     return dict(N=n, W=W, H=H, sphere=sphere, valid=valid, lo=lo, hi=hi, ids=ids, codes=codes, order=order,
+                sorted_ids=sorted_ids, sorted_codes=sorted_codes, sphere_sorted=sphere_sorted,
+                rgba_sorted=rgba_sorted, children=children, parents=parents, ranges=ranges, aabbs=aabbs)
+
+
+def build_scene_packed(samples, colours, quant):
+    """O4..O7 on a received buffer of packed samples (ids = position in the buffer)."""
+    sphere, rgba, valid = decode(samples, colours, quant)
+    n = int(valid.sum())
+    lo, hi = bounds(sphere, valid)
+    ids, codes = compact_codes(sphere, valid, lo, hi, n)
+    order = sort_codes(codes)
+    sorted_ids = ids[order]
+    sorted_codes = codes[order]
+    sphere_sorted = np.ascontiguousarray(sphere[sorted_ids])
+    rgba_sorted = np.ascontiguousarray(rgba[sorted_ids])
+    children, parents, ranges = tree(sorted_codes)
+    aabbs = refit(sphere_sorted, children)
+    return dict(N=n, sphere=sphere, valid=valid, lo=lo, hi=hi, ids=ids, codes=codes, order=order,
                 sorted_ids=sorted_ids, sorted_codes=sorted_codes, sphere_sorted=sphere_sorted,
                 rgba_sorted=rgba_sorted, children=children, parents=parents, ranges=ranges, aabbs=aabbs)
 

@@ -221,6 +221,82 @@ int64_t oracle_unproject(const float* depth, const float* cam13, int W, int H, f
   return n;
 }
 
+// ---- Wire format.  PAPER.md:69: "We quantize the object space
+// coordinate and pack it together with the radius into 64 bits ... Before sending we compact
+// that buffer by moving all the samples with zero radius to one side and send only those object
+// space samples with non-zero radius"; "32 bits per color and 64 bits per object
+// space sample (position and radius)".  The paper does not give the bit split; the reading taken
+// (DESIGN.md sec. 2): four 16-bit fields, x | y << 16 | z << 32 | radius << 48; positions are
+// fixed point over a quantisation box q = (lo[3], hi[3], r_max) that travels with the frame
+// (cell = ext / 65536, decoded at the cell centre), the radius is fixed point over [0, r_max],
+// rounded UP (a splat never shrinks) and never 0 for a kept sample; colour is RGBA8, rounded to
+// nearest.  Compaction keeps ascending pixel order.
+uint32_t quant_pos(float p, float lo, float ext) {
+  float s = ((p - lo) / ext) * 65536.0f;
+  if (!(s > 0.0f)) return 0u;
+  if (s >= 65535.0f) return 65535u;
+  return (uint32_t)s;
+}
+uint32_t quant_radius(float r, float r_max) {
+  float u = ceilf((r / r_max) * 65535.0f);
+  if (!(u > 1.0f)) return 1u;
+  if (u >= 65535.0f) return 65535u;
+  return (uint32_t)u;
+}
+uint32_t quant_colour(float c) {
+  float x = fminf(fmaxf(c, 0.0f), 1.0f);
+  return (uint32_t)(x * 255.0f + 0.5f);
+}
+
+// Server side: Eq. 1 + radius (as oracle_unproject) -> quantise -> pack -> compact.
+// quant7 = lo xyz, hi xyz, r_max.  Returns the number of samples written.
+int64_t oracle_pack(const float* color, const float* depth, const float* cam13, int W, int H, float r_scale,
+                    int radius_mode, float radius_param, const float* quant7, uint64_t* samples /*[<=P]*/,
+                    uint32_t* colours /*[<=P]*/) {
+  size_t P = (size_t)W * H;
+  std::vector<float> sphere(4 * P);
+  std::vector<uint8_t> valid(P);
+  oracle_unproject(depth, cam13, W, H, r_scale, radius_mode, radius_param, color, sphere.data(), valid.data());
+  float ext[3];
+  for (int k = 0; k < 3; ++k) ext[k] = quant7[3 + k] - quant7[k];
+  int64_t n = 0;
+  for (size_t p = 0; p < P; ++p) {
+    const float* sp = sphere.data() + 4 * p;
+    if (!valid[p] || !(sp[3] > 0.0f)) continue;   // zero radius: never sent
+    uint64_t w = 0;
+    for (int k = 0; k < 3; ++k) w |= (uint64_t)quant_pos(sp[k], quant7[k], ext[k]) << (16 * k);
+    w |= (uint64_t)quant_radius(sp[3], quant7[6]) << 48;
+    samples[n] = w;
+    uint32_t c8 = 0;
+    for (int k = 0; k < 4; ++k) c8 |= quant_colour(color[4 * p + k]) << (8 * k);
+    colours[n] = c8;
+    ++n;
+  }
+  return n;
+}
+
+// Client side: samples -> spheres (cx, cy, cz, r) and float colours, in the order received.
+// A sample whose radius field is 0 is not a legal sample: valid[i] = 0 and it is dropped later.
+void oracle_decode(const uint64_t* samples, const uint32_t* colours, int64_t n, const float* quant7,
+                   float* sphere /*[n][4]*/, float* rgba /*[n][4]*/, uint8_t* valid /*[n]*/) {
+  float cell[3];
+  for (int k = 0; k < 3; ++k) cell[k] = (quant7[3 + k] - quant7[k]) / 65536.0f;
+  float rstep = quant7[6] / 65535.0f;
+  for (int64_t i = 0; i < n; ++i) {
+    uint64_t w = samples[i];
+    float* s = sphere + 4 * i;
+    for (int k = 0; k < 3; ++k) {
+      float q = (float)(uint32_t)((w >> (16 * k)) & 0xffffu);
+      s[k] = fmaf(q + 0.5f, cell[k], quant7[k]);
+    }
+    uint32_t qr = (uint32_t)(w >> 48);
+    s[3] = (float)qr * rstep;
+    valid[i] = qr != 0u;
+    if (!valid[i]) s[0] = s[1] = s[2] = s[3] = 0.0f;
+    for (int k = 0; k < 4; ++k) rgba[4 * i + k] = (float)((colours[i] >> (8 * k)) & 0xffu) / 255.0f;
+  }
+}
+
 // ---- O4 (bounds): component-wise min / max of the valid centres.
 void oracle_bounds(const float* sphere, const uint8_t* valid, int64_t P, float* lo3, float* hi3) {
   bool any = false;
