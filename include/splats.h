@@ -89,6 +89,49 @@ int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
  * Nothing is composited.  Arguments, layout and errors as splats_render. */
 int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
 
+/* ---- The paper's wire format -------------------------------------
+ * the server sends "object space samples ... comprised of the coordinates from
+ * Equation 1 and a footprint radius.  We quantize the object space coordinate and pack it
+ * together with the radius into 64 bits", compacted so that only samples with non-zero radius
+ * travel; "32 bits per color and 64 bits per object space sample".  The paper
+ * does not print the bit split; this library's reading:
+ *   sample  uint64 = qx | qy << 16 | qz << 32 | qr << 48, four unsigned 16-bit fields;
+ *           q_k = clamp(floor((p_k - lo_k) / (hi_k - lo_k) * 65536), 0, 65535), decoded at the cell
+ *           centre lo_k + (q_k + 0.5) * (hi_k - lo_k) / 65536;
+ *           qr = clamp(ceil(r / r_max * 65535), 1, 65535), decoded as qr * (r_max / 65535): the
+ *           radius is rounded up, and a field of 0 never occurs in a sample that is sent
+ *   colour  uint32 = R | G << 8 | B << 16 | A << 24, round(255 * clamp(c, 0, 1)), decoded c / 255
+ * wr_quant (host memory) is the frame header both sides must agree on: the quantisation box
+ * (e.g. the volume's bounding box) and the largest representable radius. */
+typedef struct {
+  float lo[3];
+  float hi[3];
+  float r_max;
+} wr_quant;
+
+/* Server side: Eq. 1 + radius (mode of splats_set_radius) for every pixel of the 2.5D frame,
+ * quantise, pack, and compact in ascending pixel order (the step the paper runs serially on
+ * the CPU: 23 ms at 1024 x 1024).  Only enqueues.
+ *   color, depth, src_camera, W, H, r_scale   as splats_update
+ *   samples  dev, room for W*H uint64; colors  dev, room for W*H uint32; 16-byte aligned
+ *   count    dev, one uint32: the number of samples written (pixels with a valid depth and a
+ *            radius > 0)
+ * Uses scratch of the context (W*H <= capacity).  Errors: EINVAL as splats_update, or for a
+ * box with hi <= lo / non-finite values / r_max <= 0. */
+int splats_pack(const float* color, const float* depth, const wr_camera* src_camera, int W, int H,
+                float r_scale, const wr_quant* quant, unsigned long long* samples, unsigned* colors,
+                unsigned* count);
+
+/* Client side, the paper's literal entry point ("The client upon receiving the
+ * data will build an LBVH"): build the splats and the BVH from n received samples.  Splat ids are
+ * positions in the buffer; a sample whose radius field is 0 is dropped.  The buffers must stay
+ * valid until the enqueued work has run.  n = 0 is allowed (the next render writes zeros).
+ *   samples  dev, n uint64, 16-byte aligned;  colors  dev, n uint32;  n <= capacity
+ * Afterwards splats_render / splats_render_first_hit / splats_export work as after
+ * splats_update.  Errors: EINVAL (null pointers with n > 0, n > capacity, bad quant). */
+int splats_update_packed(const unsigned long long* samples, const unsigned* colors, unsigned n,
+                         const wr_quant* quant);
+
 /* The same two calls with HOST buffers (end-to-end path).  Both only ENQUEUE and return: the
  * frame is uploaded on a copy stream of the library into one of two device staging buffers,
  * the kernels wait for it on the compute stream, and each rendered image is read back on a
@@ -168,8 +211,9 @@ int splats_set_radius(int mode, float param);
  * since profiling was switched on or since the previous query, and clears the record.
  * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 first tree kernel
  * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 second tree
- * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render.  calls may be NULL. */
-#define SPLATS_NUM_STAGES 6
+ * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render (either query),
+ * 6 splats_pack (both launches).  calls may be NULL. */
+#define SPLATS_NUM_STAGES 7
 int splats_set_profiling(int on);
 int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);
 

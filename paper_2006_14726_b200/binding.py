@@ -15,8 +15,8 @@ import torch
 
 from . import build as _build
 
-NUM_STAGES = 6
-STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render")
+NUM_STAGES = 7
+STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
@@ -26,6 +26,10 @@ class SplatsError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"splats error {code}: {msg}")
         self.code = code
+
+
+class wr_quant(ctypes.Structure):
+    _fields_ = [("lo", ctypes.c_float * 3), ("hi", ctypes.c_float * 3), ("r_max", ctypes.c_float)]
 
 
 class wr_camera(ctypes.Structure):
@@ -51,6 +55,8 @@ def lib() -> ctypes.CDLL:
         L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
+        L.splats_update_packed.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render_host.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_count.argtypes = [ctypes.POINTER(ctypes.c_uint)]
@@ -120,6 +126,29 @@ def splats_render(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
 def splats_render_first_hit(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
     c = _cam(dst_camera)
     _check(lib().splats_render_first_hit(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
+
+
+def _quant(q) -> wr_quant:
+    a = np.ascontiguousarray(np.asarray(q, dtype=np.float32).reshape(7))
+    out = wr_quant()
+    ctypes.memmove(ctypes.byref(out), a.ctypes.data, 7 * 4)
+    return out
+
+
+def splats_pack(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, H: int, r_scale: float, quant,
+                samples: torch.Tensor, colors: torch.Tensor, count: torch.Tensor) -> None:
+    """samples: int64 CUDA tensor (uint64 words) of >= W*H, colors: int32 of >= W*H, count: int32 of 1."""
+    c, q = _cam(src_camera), _quant(quant)
+    _check(lib().splats_pack(_dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H),
+                             ctypes.byref(c), int(W), int(H), float(r_scale), ctypes.byref(q),
+                             _dev_ptr(samples, torch.int64, W * H), _dev_ptr(colors, torch.int32, W * H),
+                             _dev_ptr(count, torch.int32, 1)))
+
+
+def splats_update_packed(samples: torch.Tensor, colors: torch.Tensor, n: int, quant) -> None:
+    q = _quant(quant)
+    _check(lib().splats_update_packed(_dev_ptr(samples, torch.int64, n) if n else None,
+                                      _dev_ptr(colors, torch.int32, n) if n else None, int(n), ctypes.byref(q)))
 
 
 def splats_update_host(color, depth, src_camera, W: int, H: int, r_scale: float) -> None:

@@ -27,12 +27,50 @@ __device__ __forceinline__ void load_depth8(const float* __restrict__ depth, int
   }
 }
 
+// Where the splat centres come from.  FrameSource: the 2.5D frame itself (splats_update; Eq. 1
+// per valid pixel).  PackedSource: a received buffer of quantised samples (splats_update_packed;
+// every element is a splat unless its radius field is 0).  Element index = splat id.
+struct FrameSource {
+  const float* __restrict__ depth;
+  DevCamera cam;
+  using Raw = float;
+  __device__ __forceinline__ int width() const { return cam.W; }
+  __device__ __forceinline__ void load8(int64_t base, int64_t P, Raw t[8]) const { load_depth8(depth, base, P, t); }
+  __device__ __forceinline__ bool valid(Raw t) const { return depth_valid(t); }
+  __device__ __forceinline__ void centre(Raw t, int x, int y, float p[3]) const {
+    float len;
+    splat_centre(cam, x, y, t, p, len);
+  }
+};
+struct PackedSource {
+  const uint64_t* __restrict__ samples;
+  QuantParams q;
+  using Raw = uint64_t;
+  __device__ __forceinline__ int width() const { return 0x7fffffff; }  // one long row: x = index
+  __device__ __forceinline__ void load8(int64_t base, int64_t P, Raw w[8]) const {
+    if (base + 8 <= P) {
+      const ulonglong2* v = reinterpret_cast<const ulonglong2*>(samples + base);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const ulonglong2 a = __ldg(v + k);
+        w[2 * k] = a.x;
+        w[2 * k + 1] = a.y;
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) w[k] = (base + k < P) ? __ldg(samples + base + k) : 0ull;
+    }
+  }
+  __device__ __forceinline__ bool valid(Raw w) const { return (w >> 48) != 0ull; }
+  __device__ __forceinline__ void centre(Raw w, int, int, float p[3]) const { decode_centre(w, q, p); }
+};
+
 // ------------------------------------------------------------------------------------ a1
 // Scene bounds = component-wise min/max of the valid splat centres (Eq. 1),
 // number of valid pixels per tile (for the compaction) and in total.
+template <class Src>
 __global__ void __launch_bounds__(BUILD_THREADS)
-bounds_kernel(const float* __restrict__ depth, int64_t P, DevCamera cam, FrameState* __restrict__ st,
-              uint32_t* __restrict__ tile_count) {
+bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* __restrict__ tile_count) {
   __shared__ float s_red[6][BUILD_THREADS / 32];
   __shared__ uint32_t s_cnt[BUILD_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -41,19 +79,20 @@ bounds_kernel(const float* __restrict__ depth, int64_t P, DevCamera cam, FrameSt
   float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
   uint32_t cnt = 0;
   if (base < P) {
-    float t[8];
-    load_depth8(depth, base, P, t);
-    int y = (int)(base / cam.W), x = (int)(base - (int64_t)y * cam.W);
+    typename Src::Raw t[8];
+    src.load8(base, P, t);
+    const int W = src.width();
+    int y = (int)(base / W), x = (int)(base - (int64_t)y * W);
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      if (depth_valid(t[k])) {
-        float p[3], len;
-        splat_centre(cam, x, y, t[k], p, len);
+      if (src.valid(t[k])) {
+        float p[3];
+        src.centre(t[k], x, y, p);
 #pragma unroll
         for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], p[a]); hi[a] = fmaxf(hi[a], p[a]); }
         ++cnt;
       }
-      if (++x == cam.W) { x = 0; ++y; }
+      if (++x == W) { x = 0; ++y; }
     }
   }
 #pragma unroll
@@ -135,8 +174,9 @@ __device__ __forceinline__ uint64_t morton63(const float p[3], const float lo[3]
 // digit histograms of the radix sort are accumulated in shared memory on the way (the keys
 // are in registers anyway) and flushed once per block.  Block 0 also re-arms the other
 // parity's FrameState for the next frame.
+template <class Src>
 __global__ void __launch_bounds__(BUILD_THREADS)
-unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevCamera cam,
+unproject_kernel(const Src src, int64_t P, int num_tiles,
                  FrameState* __restrict__ st, FrameState* __restrict__ st_next,
                  const uint32_t* __restrict__ tile_count, uint64_t* __restrict__ keys0,
                  uint32_t* __restrict__ ids0, uint64_t* __restrict__ keys1, uint32_t* __restrict__ ids1,
@@ -183,18 +223,19 @@ unproject_kernel(const float* __restrict__ depth, int64_t P, int num_tiles, DevC
     uint64_t code[8];
     uint32_t vmask = 0;
     if (base < P && tile_count[tile] != 0) {
-      float t[8];
-      load_depth8(depth, base, P, t);
-      int y = (int)(base / cam.W), x = (int)(base - (int64_t)y * cam.W);
+      typename Src::Raw t[8];
+      src.load8(base, P, t);
+      const int W = src.width();
+      int y = (int)(base / W), x = (int)(base - (int64_t)y * W);
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
-        if (depth_valid(t[k])) {
-          float p[3], len;
-          splat_centre(cam, x, y, t[k], p, len);
+        if (src.valid(t[k])) {
+          float p[3];
+          src.centre(t[k], x, y, p);
           code[k] = morton63(p, lo, ext);
           vmask |= 1u << k;
         }
-        if (++x == cam.W) { x = 0; ++y; }
+        if (++x == W) { x = 0; ++y; }
       }
     }
     // block exclusive scan of popc(vmask)

@@ -71,6 +71,50 @@ __device__ __forceinline__ float splat_radius(const RadiusParams& rp, float z, f
   return r;
 }
 
+// ---- wire format (include/splats.h, wr_quant): 64-bit sample =
+// x | y << 16 | z << 32 | radius << 48, four 16-bit fixed-point fields; colour = RGBA8.
+struct QuantParams {
+  float lo[3], ext[3];   // quantisation box and its extent hi - lo
+  float cell[3];         // ext / 65536
+  float r_max, rstep;    // radius of code 65535, r_max / 65535
+};
+__device__ __forceinline__ uint32_t quant_pos(float p, float lo, float ext) {
+  const float s = mul_(div_(sub_(p, lo), ext), 65536.0f);
+  if (!(s > 0.0f)) return 0u;
+  if (s >= 65535.0f) return 65535u;
+  return __float2uint_rz(s);
+}
+__device__ __forceinline__ uint32_t quant_radius(float r, float r_max) {  // rounded up, never 0
+  const float u = ceilf(mul_(div_(r, r_max), 65535.0f));
+  if (!(u > 1.0f)) return 1u;
+  if (u >= 65535.0f) return 65535u;
+  return __float2uint_rz(u);
+}
+__device__ __forceinline__ uint32_t quant_colour(float c) {
+  const float x = fminf(fmaxf(c, 0.0f), 1.0f);
+  return __float2uint_rz(add_(mul_(x, 255.0f), 0.5f));
+}
+__device__ __forceinline__ uint64_t pack_sample(const float p[3], float r, const QuantParams& q) {
+  return (uint64_t)quant_pos(p[0], q.lo[0], q.ext[0]) | ((uint64_t)quant_pos(p[1], q.lo[1], q.ext[1]) << 16) |
+         ((uint64_t)quant_pos(p[2], q.lo[2], q.ext[2]) << 32) | ((uint64_t)quant_radius(r, q.r_max) << 48);
+}
+__device__ __forceinline__ uint32_t pack_colour(const float4 c) {
+  return quant_colour(c.x) | (quant_colour(c.y) << 8) | (quant_colour(c.z) << 16) | (quant_colour(c.w) << 24);
+}
+// centre of the sample's cell (a radius field of 0 marks a sample that must be dropped)
+__device__ __forceinline__ void decode_centre(uint64_t w, const QuantParams& q, float p[3]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    p[k] = fma_(add_(__uint2float_rn((uint32_t)(w >> (16 * k)) & 0xffffu), 0.5f), q.cell[k], q.lo[k]);
+}
+__device__ __forceinline__ float decode_radius(uint64_t w, const QuantParams& q) {
+  return mul_(__uint2float_rn((uint32_t)(w >> 48)), q.rstep);
+}
+__device__ __forceinline__ float4 decode_colour(uint32_t c) {
+  return make_float4(div_(__uint2float_rn(c & 0xffu), 255.0f), div_(__uint2float_rn((c >> 8) & 0xffu), 255.0f),
+                     div_(__uint2float_rn((c >> 16) & 0xffu), 255.0f), div_(__uint2float_rn(c >> 24), 255.0f));
+}
+
 // ---- order-preserving float <-> uint32 map for atomicMin / atomicMax
 __device__ __forceinline__ uint32_t f2ord(float f) {
   uint32_t u = __float_as_uint(f);

@@ -8,6 +8,39 @@ namespace sw {
 
 constexpr int LBVH_THREADS = 256;
 
+// Splat `id` (= source pixel index, or position in a received sample buffer) as sphere + colour.
+// FrameGather recomputes the sphere from the depth buffer with exactly the arithmetic of the
+// bounds / Morton kernels (Eq. 1; radius per RadiusParams) and copies the colour
+// ("no shading other than the constant sample color"); PackedGather decodes the
+// 64-bit sample and the RGBA8 colour.
+struct FrameGather {
+  const float* __restrict__ depth;
+  const float4* __restrict__ color;
+  DevCamera cam;
+  RadiusParams rp;
+  __device__ __forceinline__ void get(uint32_t id, float4& sp, float4& col) const {
+    const int y = (int)(id / (uint32_t)cam.W), x = (int)(id - (uint32_t)y * (uint32_t)cam.W);
+    const float t = __ldg(depth + id);
+    float p[3], len;
+    splat_centre(cam, x, y, t, p, len);
+    const float z = div_(t, len);
+    col = __ldg(color + id);
+    sp = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
+  }
+};
+struct PackedGather {
+  const uint64_t* __restrict__ samples;
+  const uint32_t* __restrict__ colours;
+  QuantParams q;
+  __device__ __forceinline__ void get(uint32_t id, float4& sp, float4& col) const {
+    const uint64_t w = __ldg(samples + id);
+    float p[3];
+    decode_centre(w, q, p);
+    sp = make_float4(p[0], p[1], p[2], decode_radius(w, q));
+    col = decode_colour(__ldg(colours + id));
+  }
+};
+
 // Common-prefix length of the keys at sorted positions i and j; ties broken by the sorted
 // position itself (equivalent to concatenating key and index); -1 outside the array.
 __device__ __forceinline__ int delta(const uint64_t* __restrict__ keys, int n, int i, uint64_t ki, int j) {
@@ -22,22 +55,17 @@ __device__ __forceinline__ int delta(const uint64_t* __restrict__ keys, int n, i
 // ("no shading other than the constant sample color"); (b) emits internal
 // node i of the binary radix tree over the sorted keys: direction, range end by
 // doubling + binary search, split by binary search.
+template <class Gather>
 __global__ void __launch_bounds__(LBVH_THREADS)
-emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm,
-            const float* __restrict__ depth, const float4* __restrict__ color, DevCamera cam, RadiusParams rp,
+emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src,
             const FrameState* __restrict__ st, float4* __restrict__ sphere, float4* __restrict__ rgba,
             Node* __restrict__ nodes, int* __restrict__ leaf_parent) {
   const int n = (int)st->n;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     // ---- (a) gather
-    const uint32_t id = __ldg(perm + i);
-    const int y = (int)(id / (uint32_t)cam.W), x = (int)(id - (uint32_t)y * (uint32_t)cam.W);
-    const float t = __ldg(depth + id);
-    float p[3], len;
-    splat_centre(cam, x, y, t, p, len);
-    const float z = div_(t, len);
-    const float4 col = __ldg(color + id);
-    sphere[i] = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
+    float4 sp, col;
+    src.get(__ldg(perm + i), sp, col);
+    sphere[i] = sp;
     rgba[i] = col;
     if (n == 1) leaf_parent[0] = -1;
     if (i >= n - 1) continue;
@@ -134,9 +162,9 @@ __device__ __forceinline__ void box_of_sphere(const float4 sp, float lo[3], floa
   hi[0] = add_(sp.x, sp.w); hi[1] = add_(sp.y, sp.w); hi[2] = add_(sp.z, sp.w);
 }
 
+template <class Gather>
 __global__ void __launch_bounds__(PYR_THREADS)
-leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const float* __restrict__ depth,
-                    const float4* __restrict__ color, DevCamera cam, RadiusParams rp, FrameState* st,
+leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
                     float4* __restrict__ sphere, float4* __restrict__ rgba, float4* pyr) {
   __shared__ float s_box[6][PYR_LEAVES];
   __shared__ bool s_last;
@@ -154,14 +182,8 @@ leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const float* __restrict__
     const uint32_t i = base + l;
     float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
     if (i < n) {
-      const uint32_t id = __ldg(perm + i);
-      const int y = (int)(id / (uint32_t)cam.W), x = (int)(id - (uint32_t)y * (uint32_t)cam.W);
-      const float t = __ldg(depth + id);
-      float p[3], len;
-      splat_centre(cam, x, y, t, p, len);
-      const float z = div_(t, len);
-      const float4 col = __ldg(color + id);
-      const float4 sp = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
+      float4 sp, col;
+      src.get(__ldg(perm + i), sp, col);
       sphere[i] = sp;
       rgba[i] = col;
       box_of_sphere(sp, lo, hi);

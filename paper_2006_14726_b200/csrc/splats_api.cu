@@ -14,6 +14,7 @@
 #include "common.cuh"
 #include "lbvh.cuh"
 #include "onesweep.cuh"
+#include "pack.cuh"
 #include "render.cuh"
 
 namespace {
@@ -175,35 +176,57 @@ int ensure_staging(Context* c) {
   return SPLATS_OK;
 }
 
-int do_update(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale) {
-  const int64_t P = (int64_t)W * H;
-  const DevCamera dc = make_camera(cam, W, H);
+// Quantisation constants of the wire format, each operation rounded to float32 on its own.
+bool make_quant(const wr_quant* q, QuantParams* out) {
+  for (int k = 0; k < 3; ++k) {
+    if (!std::isfinite(q->lo[k]) || !std::isfinite(q->hi[k]) || !(q->hi[k] > q->lo[k])) return false;
+    volatile float ext = q->hi[k] - q->lo[k];
+    volatile float cell = ext / 65536.0f;
+    if (!std::isfinite(ext)) return false;
+    out->lo[k] = q->lo[k];
+    out->ext[k] = ext;
+    out->cell[k] = cell;
+  }
+  if (!(q->r_max > 0.0f) || !std::isfinite(q->r_max)) return false;
+  volatile float rstep = q->r_max / 65535.0f;
+  out->r_max = q->r_max;
+  out->rstep = rstep;
+  return true;
+}
+
+RadiusParams make_radius(const Context* c, const wr_camera* cam, int H, float r_scale) {
   RadiusParams rp;
   rp.mode = c->radius_mode;
   rp.k_r = radius_factor(cam, H, r_scale);
-  {
-    volatile float rc = r_scale * c->radius_param;   // separately rounded float32 operations
-    volatile float w1 = 1.0f - c->radius_param;
-    rp.r_const = rc;
-    rp.f_min = c->radius_param;
-    rp.w1 = w1;
-  }
+  volatile float rc = r_scale * c->radius_param;   // separately rounded float32 operations
+  volatile float w1 = 1.0f - c->radius_param;
+  rp.r_const = rc;
+  rp.f_min = c->radius_param;
+  rp.w1 = w1;
+  return rp;
+}
+
+// The launch sequence of one update: a1 bounds, a2 keys + compaction, a3 sort, a4/a5 tree.
+// Src yields the splat centres of elements [0, P) (build_kernels.cuh), Gather the sphere and
+// colour of a splat id (lbvh.cuh).
+template <class Src, class Gather>
+int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
   const int parity = (int)(c->frame & 1u);
   FrameState* st = c->state + parity;
   FrameState* st_next = c->state + (parity ^ 1);
-  const int tiles = (int)((P + TILE_PX - 1) / TILE_PX);
+  const int tiles = P > 0 ? (int)((P + TILE_PX - 1) / TILE_PX) : 1;
   cudaStream_t s = c->stream;
   const bool prof = c->profiling;
 
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
-  bounds_kernel<<<tiles, BUILD_THREADS, 0, s>>>(depth, P, dc, st, c->tile_count);
+  bounds_kernel<Src><<<tiles, BUILD_THREADS, 0, s>>>(src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
-  unproject_kernel<<<grid2, BUILD_THREADS, 0, s>>>(depth, P, tiles, dc, st, st_next, c->tile_count, c->key[0], c->val[0],
-                                                  c->key[1], c->val[1], c->sort_mode);
+  unproject_kernel<Src><<<grid2, BUILD_THREADS, 0, s>>>(src, P, tiles, st, st_next, c->tile_count, c->key[0], c->val[0],
+                                                       c->key[1], c->val[1], c->sort_mode);
   if (prof) m[2] = c->mark();
-  const int max_sort_tiles = (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE);
+  const int max_sort_tiles = P > 0 ? (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE) : 1;
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
   SortArgs sa;
   sa.key[0] = c->key[0]; sa.key[1] = c->key[1];
@@ -226,17 +249,16 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
     onesweep_kernel<<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
   }
   if (prof) m[3] = c->mark();
-  const int lgrid_max = (int)((P + LBVH_THREADS - 1) / LBVH_THREADS);
+  const int lgrid_max = P > 0 ? (int)((P + LBVH_THREADS - 1) / LBVH_THREADS) : 1;
   const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
   if (c->refit_mode == SPLATS_REFIT_ATOMIC) {
-    emit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], depth, reinterpret_cast<const float4*>(color), dc,
-                                               rp, st, c->sphere, c->rgba, c->nodes, c->leaf_parent);
+    emit_kernel<Gather><<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], gather, st, c->sphere, c->rgba, c->nodes,
+                                                       c->leaf_parent);
     if (prof) m[4] = c->mark();
     refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
   } else {
-    const int pgrid = (int)((P + PYR_LEAVES - 1) / PYR_LEAVES);
-    leaf_pyramid_kernel<<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], depth, reinterpret_cast<const float4*>(color), dc, rp,
-                                                      st, c->sphere, c->rgba, c->pyr);
+    const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
+    leaf_pyramid_kernel<Gather><<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], gather, st, c->sphere, c->rgba, c->pyr);
     if (prof) m[4] = c->mark();
     emit_boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->sphere, c->pyr, st, c->nodes);
   }
@@ -249,6 +271,18 @@ int do_update(Context* c, const float* color, const float* depth, const wr_camer
   c->frame += 1;
   c->has_bvh = true;
   return SPLATS_OK;
+}
+
+int do_update_frame(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale) {
+  FrameSource src;
+  src.depth = depth;
+  src.cam = make_camera(cam, W, H);
+  FrameGather g;
+  g.depth = depth;
+  g.color = reinterpret_cast<const float4*>(color);
+  g.cam = src.cam;
+  g.rp = make_radius(c, cam, H, r_scale);
+  return do_update(c, src, g, (int64_t)W * H);
 }
 
 int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false) {
@@ -363,7 +397,7 @@ int splats_update(const float* color, const float* depth, const wr_camera* src_c
   if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
   if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
     return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
-  return do_update(g_ctx, color, depth, src_camera, W, H, r_scale);
+  return do_update_frame(g_ctx, color, depth, src_camera, W, H, r_scale);
 }
 
 int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba) {
@@ -382,6 +416,49 @@ int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* 
   return do_render(g_ctx, dst_camera, W2, H2, out_rgba, true);
 }
 
+int splats_pack(const float* color, const float* depth, const wr_camera* src_camera, int W, int H, float r_scale,
+                const wr_quant* quant, unsigned long long* samples, unsigned* colors, unsigned* count) {
+  int rc = check_frame_args(g_ctx, color, depth, src_camera, W, H);
+  if (rc) return rc;
+  if (!quant || !samples || !colors || !count) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
+  if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
+    return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
+  Context* c = g_ctx;
+  PackArgs a;
+  if (!make_quant(quant, &a.q)) return fail(SPLATS_EINVAL, "quantisation box must be finite with hi > lo, r_max finite and > 0");
+  a.color = reinterpret_cast<const float4*>(color);
+  a.depth = depth;
+  a.cam = make_camera(src_camera, W, H);
+  a.rp = make_radius(c, src_camera, H, r_scale);
+  a.P = (int64_t)W * H;
+  a.num_tiles = (int)((a.P + TILE_PX - 1) / TILE_PX);
+  size_t m0 = 0;
+  if (c->profiling) m0 = c->mark();
+  pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count);
+  const int grid2 = a.num_tiles < c->num_sms * 4 ? a.num_tiles : c->num_sms * 4;
+  pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
+  if (c->profiling) c->spans.push_back({6, m0, c->mark()});
+  c->launches += 2;
+  CU(cudaGetLastError());
+  return SPLATS_OK;
+}
+
+int splats_update_packed(const unsigned long long* samples, const unsigned* colors, unsigned n, const wr_quant* quant) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context: call splats_create first");
+  if (!quant || ((!samples || !colors) && n != 0)) return fail(SPLATS_EINVAL, "null pointer argument");
+  if ((int64_t)n > g_ctx->cap) return fail(SPLATS_EINVAL, "n exceeds the capacity given to splats_create");
+  if (reinterpret_cast<uintptr_t>(samples) & 15u) return fail(SPLATS_EINVAL, "samples must be 16-byte aligned");
+  PackedSource src;
+  if (!make_quant(quant, &src.q)) return fail(SPLATS_EINVAL, "quantisation box must be finite with hi > lo, r_max finite and > 0");
+  src.samples = reinterpret_cast<const uint64_t*>(samples);
+  PackedGather g;
+  g.samples = src.samples;
+  g.colours = colors;
+  g.q = src.q;
+  return do_update(g_ctx, src, g, (int64_t)n);
+}
+
 int splats_update_host(const float* color_host, const float* depth_host, const wr_camera* src_camera, int W, int H,
                        float r_scale) {
   int rc = check_frame_args(g_ctx, color_host, depth_host, src_camera, W, H);
@@ -397,7 +474,7 @@ int splats_update_host(const float* color_host, const float* depth_host, const w
   CU(cudaMemcpyAsync(c->stage_depth[u], depth_host, P * sizeof(float), cudaMemcpyHostToDevice, c->h2d_stream));
   CU(cudaEventRecord(c->in_uploaded[u], c->h2d_stream));
   CU(cudaStreamWaitEvent(c->stream, c->in_uploaded[u], 0));
-  rc = do_update(c, c->stage_color[u], c->stage_depth[u], src_camera, W, H, r_scale);
+  rc = do_update_frame(c, c->stage_color[u], c->stage_depth[u], src_camera, W, H, r_scale);
   if (rc) return rc;
   CU(cudaEventRecord(c->in_free[u], c->stream));
   c->n_uploads += 1;
