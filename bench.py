@@ -225,6 +225,37 @@ def run_ours(args):
     torch.cuda.synchronize()
     first_ms = sum(a.elapsed_time(b) for a, b, _ in first_events) / max(1, sum(n for _, _, n in first_events))
 
+    # ---- the paper's wire format: server-side pack + compaction and the
+    # client-side build from packed samples, once per source frame; reported beside the headline
+    import math
+    half_diag = math.sqrt(3.0) / cfg.vol_n / 2          # half a voxel's diagonal
+    quant = [0.0, 0.0, 0.0, 1.0, 1.0, 1.0, 4 * half_diag]
+    w_samples = torch.empty(P, dtype=torch.int64, device="cuda")
+    w_colors = torch.empty(P, dtype=torch.int32, device="cuda")
+    w_count = torch.zeros(1, dtype=torch.int32, device="cuda")
+    sp.splats_set_radius(sp.RADIUS_CONSTANT, half_diag)
+    pack_ms, upd_ms, wire_n = [], [], []
+    for rep in range(2):                                # first pass warms up
+        for g in range(G):
+            f = frames[g]
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            ev[0].record()
+            sp.splats_pack(d_color[g], d_depth[g], f["src_cam"], W, H, cfg.r_scale, quant, w_samples, w_colors, w_count)
+            ev[1].record()
+            n_s = int(w_count.item())                   # the count travels with the frame
+            ev[3].record()
+            sp.splats_update_packed(w_samples, w_colors, n_s, quant)
+            ev[2].record()
+            sp.splats_render_first_hit(f["dst_cams"][-1], W, H, d_out[0])
+            torch.cuda.synchronize()
+            if rep:
+                pack_ms.append(ev[0].elapsed_time(ev[1]))
+                upd_ms.append(ev[3].elapsed_time(ev[2]))
+                wire_n.append(n_s)
+    sp.splats_set_radius(sp.RADIUS_FOOTPRINT, 0.0)
+    pack_avg, upd_avg, n_avg = sum(pack_ms) / len(pack_ms), sum(upd_ms) / len(upd_ms), sum(wire_n) / len(wire_n)
+    pack_bytes = 8 * P + 28 * n_avg                     # depth read twice, colour read + 12 B written per sample
+
     # ---- end-to-end through the host-buffer entry points (H2D of the frame, D2H of every image)
     h_color = [torch.from_numpy(f["color"]).pin_memory() for f in frames]
     h_depth = [torch.from_numpy(f["depth"]).pin_memory() for f in frames]
@@ -299,6 +330,12 @@ def run_ours(args):
                            "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": build_bytes,
                            "note": "all build kernels of one splats_update (5 launches), events inside the timed region"},
         "kernels": kernels,
+        "wire_format": {"pack_ms": pack_avg, "pack_gbs": pack_bytes / (pack_avg * 1e-3) / 1e9,
+                        "pack_frac_of_hbm_peak": pack_bytes / (pack_avg * 1e-3) / 1e9 / peak,
+                        "update_packed_ms": upd_avg, "samples_avg": n_avg, "payload_bytes_avg": 12 * n_avg,
+                        "note": "splats_pack (Eq. 1, constant half-voxel-diagonal radius, 64-bit samples + RGBA8, GPU "
+                                "compaction; the paper's serial CPU compaction takes 23 ms at 1024x1024, PAPER.md:79) and "
+                                "splats_update_packed on the same source frames"},
         "first_hit": {"render_ms": first_ms, "mrays_per_s": P / (first_ms * 1e-3) / 1e6,
                       "note": "splats_render_first_hit (the paper's own query, PAPER.md:53,59) on the same frames and cameras"},
     }
