@@ -81,6 +81,7 @@ def lib():
         L.oracle_composite.restype = _i32
         L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
         L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
+        L.oracle_render_points.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _i32, _vp]
         _lib = L
     return _lib
 
@@ -264,3 +265,13 @@ def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False, first
         out = out.reshape(H2, W2, 4)
         used = used.reshape(H2, W2)
     return (out, used) if return_hits else out
+
+
+def render_points(scene, cam, W2, H2, point_px=1):
+    """The [ZAL12] point-primitive warp the paper compares against: splat
+    centres as fixed-size points with a per-point depth test.  Returns float32 [H2, W2, 4]."""
+    cam = _f32(cam)
+    out = np.zeros((H2, W2, 4), np.float32)
+    lib().oracle_render_points(_ptr(scene["sphere_sorted"]), _ptr(scene["rgba_sorted"]), _ptr(scene["sorted_ids"]),
+                               scene["N"], _ptr(cam), W2, H2, int(point_px), _ptr(out))
+    return out

@@ -482,4 +482,48 @@ void oracle_render_bvh(const float* sphere, const float* rgba, const uint32_t* i
   }
 }
 
+// ---- Comparison renderer: the 2.5D point rendering of [ZAL12] that
+// the paper compares against -- "the authors render the image pixels as point primitives"
+// (PAPER.md:37), object space coordinate -> "window coordinates by applying the viewing and
+// camera transforms as well as viewport transform", "the point primitives' size is
+// fixed to a certain number of pixels", depth test "not performed per fragment but
+// per vertex".  Restated without a graphics API: every splat centre is projected
+// with the destination camera; it covers the point_px x point_px pixels whose centres lie in the
+// square (w - size/2, w + size/2] of that side around its window position (the OpenGL point
+// rasterisation rule: odd sizes centre on floor(w) + 1/2, even sizes on floor(w + 1/2)); each
+// pixel shows the stored colour of the covering point with the smallest view-axis depth (ties:
+// smaller splat id); no blending; points at or behind the eye plane are culled.
+void oracle_render_points(const float* sphere, const float* rgba, const uint32_t* ids, int64_t N,
+                          const float* cam13, int W2, int H2, int point_px, float* out /*[H2*W2*4]*/) {
+  Camera c = load_camera(cam13);
+  size_t P2 = (size_t)W2 * H2;
+  std::vector<float> zbuf(P2, 0.0f);
+  std::vector<int64_t> owner(P2, -1);
+  float ta = (c.tau * (float)W2) / (float)H2;
+  float hW = 0.5f * (float)W2, hH = 0.5f * (float)H2;
+  float off = 0.5f * (float)point_px + 0.5f;
+  for (int64_t i = 0; i < N; ++i) {
+    const float* s = sphere + 4 * i;
+    float v[3] = {s[0] - c.e[0], s[1] - c.e[1], s[2] - c.e[2]};
+    float zc = fmaf(v[2], c.F[2], fmaf(v[1], c.F[1], v[0] * c.F[0]));
+    if (!(zc > 0.0f)) continue;
+    float xr = fmaf(v[2], c.R[2], fmaf(v[1], c.R[1], v[0] * c.R[0]));
+    float yu = fmaf(v[2], c.U[2], fmaf(v[1], c.U[1], v[0] * c.U[0]));
+    float ndx = xr / (zc * ta), ndy = yu / (zc * c.tau);
+    float wx = fmaf(ndx, hW, hW), wy = fmaf(-ndy, hH, hH);
+    float fx0 = floorf(wx - off) + 1.0f, fy0 = floorf(wy - off) + 1.0f;
+    if (!(fx0 > -1e9f && fx0 < 1e9f && fy0 > -1e9f && fy0 < 1e9f)) continue;   // far off screen / not finite
+    long x0 = (long)fx0, y0 = (long)fy0;
+    for (long y = y0; y < y0 + point_px; ++y)
+      for (long x = x0; x < x0 + point_px; ++x) {
+        if (x < 0 || y < 0 || x >= W2 || y >= H2) continue;
+        size_t p = (size_t)y * W2 + x;
+        bool wins = owner[p] < 0 || zc < zbuf[p] || (zc == zbuf[p] && ids[i] < ids[owner[p]]);
+        if (wins) { zbuf[p] = zc; owner[p] = i; }
+      }
+  }
+  for (size_t p = 0; p < P2; ++p)
+    for (int k = 0; k < 4; ++k) out[4 * p + k] = owner[p] < 0 ? 0.0f : rgba[4 * (size_t)owner[p] + k];
+}
+
 }  // extern "C"
