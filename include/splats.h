@@ -89,6 +89,17 @@ int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
  * Nothing is composited.  Arguments, layout and errors as splats_render. */
 int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* out_rgba);
 
+/* The renderer the paper compares against ("we implemented the reference method by
+ * Zellmann et al. using OpenGL point rendering"), restated as CUDA
+ * kernels because no graphics API exists on this machine: the centres of the splats of the
+ * latest update are projected with dst_camera to window coordinates and drawn as
+ * square points of point_px x point_px pixels (a size "fixed to a certain number of
+ * pixels"; OpenGL's rule: pixel centres in (w - size/2, w + size/2]), depth-tested per point
+ * on the view-axis depth, ties to the smaller splat id, no blending: each pixel
+ * shows the stored colour of its nearest point, background (0,0,0,0).  Points at or behind the
+ * eye plane are culled.  point_px in [1, 64].  Arguments, layout, errors as splats_render. */
+int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_px, float* out_rgba);
+
 /* ---- The paper's wire format -------------------------------------
  * the server sends "object space samples ... comprised of the coordinates from
  * Equation 1 and a footprint radius.  We quantize the object space coordinate and pack it
@@ -212,8 +223,8 @@ int splats_set_radius(int mode, float param);
  * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 first tree kernel
  * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 second tree
  * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render (either query),
- * 6 splats_pack (both launches).  calls may be NULL. */
-#define SPLATS_NUM_STAGES 7
+ * 6 splats_pack (both launches), 7 splats_render_points (three launches).  calls may be NULL. */
+#define SPLATS_NUM_STAGES 8
 int splats_set_profiling(int on);
 int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);
 

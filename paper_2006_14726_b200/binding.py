@@ -15,8 +15,8 @@ import torch
 
 from . import build as _build
 
-NUM_STAGES = 7
-STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack")
+NUM_STAGES = 8
+STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack", "points")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
@@ -55,6 +55,7 @@ def lib() -> ctypes.CDLL:
         L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_render_points.argtypes = [cam_p, _ci, _ci, _ci, _vp]
         L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
         L.splats_update_packed.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
@@ -126,6 +127,12 @@ def splats_render(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
 def splats_render_first_hit(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:
     c = _cam(dst_camera)
     _check(lib().splats_render_first_hit(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
+
+
+def splats_render_points(dst_camera, W2: int, H2: int, point_px: int, out_rgba: torch.Tensor) -> None:
+    c = _cam(dst_camera)
+    _check(lib().splats_render_points(ctypes.byref(c), int(W2), int(H2), int(point_px),
+                                      _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
 
 
 def _quant(q) -> wr_quant:

@@ -15,6 +15,7 @@
 #include "lbvh.cuh"
 #include "onesweep.cuh"
 #include "pack.cuh"
+#include "points.cuh"
 #include "render.cuh"
 
 namespace {
@@ -40,6 +41,7 @@ struct Context {
   float4* sphere = nullptr;
   float4* rgba = nullptr;
   Node* nodes = nullptr;
+  uint64_t* zkey = nullptr;         // depth buffer of splats_render_points, all ones between calls
   int* leaf_parent = nullptr;
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
   PyramidLayout pyr_layout;
@@ -140,7 +142,7 @@ void free_all(Context* c) {
   cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
-  cudaFree(c->leaf_parent); cudaFree(c->pyr);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->zkey);
   for (int i = 0; i < Context::N_IN; ++i) {
     cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
     if (c->in_uploaded[i]) cudaEventDestroy(c->in_uploaded[i]);
@@ -347,6 +349,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (e == cudaSuccess) e = dmalloc(&c->rgba, cap);
   if (e == cudaSuccess) e = dmalloc(&c->nodes, cap);
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->zkey, cap);
+  if (e == cudaSuccess) e = cudaMemset(c->zkey, 0xff, cap * sizeof(uint64_t));
   {  // pyramid levels 1.. : ceil(cap / 2^k) entries each
     size_t off = 0;
     c->pyr_layout.off[0] = 0;
@@ -414,6 +418,37 @@ int splats_render_first_hit(const wr_camera* dst_camera, int W2, int H2, float* 
   if (reinterpret_cast<uintptr_t>(out_rgba) & 15u) return fail(SPLATS_EINVAL, "out_rgba must be 16-byte aligned");
   if (!g_ctx->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_first_hit before any splats_update");
   return do_render(g_ctx, dst_camera, W2, H2, out_rgba, true);
+}
+
+int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_px, float* out_rgba) {
+  int rc = check_frame_args(g_ctx, out_rgba, out_rgba, dst_camera, W2, H2);
+  if (rc) return rc;
+  if (reinterpret_cast<uintptr_t>(out_rgba) & 15u) return fail(SPLATS_EINVAL, "out_rgba must be 16-byte aligned");
+  if (point_px < 1 || point_px > 64) return fail(SPLATS_EINVAL, "point_px outside [1, 64]");
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_points before any update");
+  PointParams p;
+  p.cam = make_camera(dst_camera, W2, H2);
+  p.sphere = c->sphere;
+  p.rgba = c->rgba;
+  p.ids = c->val[0];
+  p.st = c->state + c->parity;
+  p.zkey = c->zkey;
+  p.out = reinterpret_cast<float4*>(out_rgba);
+  p.point_px = point_px;
+  p.hW = 0.5f * (float)W2;
+  p.hH = 0.5f * (float)H2;
+  p.off = 0.5f * (float)point_px + 0.5f;
+  const int grid = c->num_sms * 8;
+  size_t m0 = 0;
+  if (c->profiling) m0 = c->mark();
+  points_kernel<false><<<grid, POINT_THREADS, 0, c->stream>>>(p);
+  points_kernel<true><<<grid, POINT_THREADS, 0, c->stream>>>(p);
+  points_background_kernel<<<grid, POINT_THREADS, 0, c->stream>>>(p);
+  if (c->profiling) c->spans.push_back({7, m0, c->mark()});
+  c->launches += 3;
+  CU(cudaGetLastError());
+  return SPLATS_OK;
 }
 
 int splats_pack(const float* color, const float* depth, const wr_camera* src_camera, int W, int H, float r_scale,
