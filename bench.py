@@ -218,12 +218,19 @@ def run_ours(args):
                 sp.splats_render_first_hit(cam, W, H, d_out[j])
             e1.record()
             first_events.append((e0, e1, len(f["dst_cams"])))
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record()
+            for j, cam in enumerate(f["dst_cams"]):
+                sp.splats_render_points(cam, W, H, 2, d_out[j])
+            p1.record()
+            point_events.append((p0, p1, len(f["dst_cams"])))
 
-    first_events = []
+    first_events, point_events = [], []
     for k in range(min(K, G)):
         step_first(k)
     torch.cuda.synchronize()
     first_ms = sum(a.elapsed_time(b) for a, b, _ in first_events) / max(1, sum(n for _, _, n in first_events))
+    points_ms = sum(a.elapsed_time(b) for a, b, _ in point_events) / max(1, sum(n for _, _, n in point_events))
 
     # ---- the paper's wire format: server-side pack + compaction and the
     # client-side build from packed samples, once per source frame; reported beside the headline
@@ -336,6 +343,9 @@ def run_ours(args):
                         "note": "splats_pack (Eq. 1, constant half-voxel-diagonal radius, 64-bit samples + RGBA8, GPU "
                                 "compaction; the paper's serial CPU compaction takes 23 ms at 1024x1024, PAPER.md:79) and "
                                 "splats_update_packed on the same source frames"},
+        "point_baseline": {"render_ms": points_ms,
+                           "note": "splats_render_points, 2x2-pixel points: CUDA restatement of the OpenGL point rendering of "
+                                   "[ZAL12] that the paper compares against (PAPER.md:37,89); GL itself is unavailable on this box"},
         "first_hit": {"render_ms": first_ms, "mrays_per_s": P / (first_ms * 1e-3) / 1e6,
                       "note": "splats_render_first_hit (the paper's own query, PAPER.md:53,59) on the same frames and cameras"},
     }
