@@ -312,7 +312,10 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
 
 // The tile size follows N (known on the device only): small frames are latency bound, so they
 // get small tiles (more blocks busy, shorter ranking chains); large ones get 4096-element tiles.
-__global__ void __launch_bounds__(SORT_THREADS)
+#ifndef SPLATS_SORT_BLOCKS
+#define SPLATS_SORT_BLOCKS 2
+#endif
+__global__ void __launch_bounds__(SORT_THREADS, SPLATS_SORT_BLOCKS)
 onesweep_kernel(SortArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);

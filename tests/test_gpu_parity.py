@@ -188,14 +188,14 @@ def test_sort_modes_give_the_same_order(mode):
 
 
 def test_dense_frame_five_pass_hybrid_sort_and_all_tile_sizes():
-    # N > 2^21: the hybrid sort runs 5 passes (top 39 bits) starting from the second buffer;
+    # N > 2^20: the hybrid sort runs 5 passes (top 39 bits) starting from the second buffer;
     # then smaller frames in the same context walk through the 4096/2048/1024-element tile paths.
     W, H = 2304, 1000
     color, depth, cam = synth.dense_frame(W, H, seed=5)
     with Session(W, H) as s:
         sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(2.0)], mode="bvh", sample=4096)
-        assert sc["N"] == W * H > (1 << 21)
-        for (w, h) in ((1400, 700), (900, 500), (640, 360)):
+        assert sc["N"] == W * H > (1 << 20)
+        for (w, h) in ((1500, 800), (1400, 700), (900, 500), (640, 360)):
             c2, d2, cam2 = synth.dense_frame(w, h, seed=w)
             check_scene(s, c2, d2, cam2, w, h, 1.0, [synth.orbit_camera(-2.0)], mode="bvh", sample=2048)
 
