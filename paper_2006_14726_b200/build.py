@@ -38,7 +38,8 @@ def nvcc_path() -> str:
 def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None) -> Path:
     if not force and LIB.exists() and LIB.stat().st_mtime >= _newest_source_mtime():
         return LIB
-    cmd = [nvcc_path(), *NVCC_FLAGS, *(extra or []), f"-I{INCLUDE}", *map(str, sources()), "-o", str(LIB)]
+    extra = list(extra or []) + os.environ.get("SPLATS_NVCC_EXTRA", "").split()   # e.g. -DSPLATS_STATS (debug builds)
+    cmd = [nvcc_path(), *NVCC_FLAGS, *extra, f"-I{INCLUDE}", *map(str, sources()), "-o", str(LIB)]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))
