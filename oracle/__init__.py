@@ -81,6 +81,7 @@ def lib():
         L.oracle_composite.restype = _i32
         L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
         L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
+        L.oracle_march.argtypes = [_vp, _i32, _vp, _vp, _vp, _i32, _i32, _vp, _vp]
         L.oracle_render_points.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _i32, _vp]
         _lib = L
     return _lib
@@ -275,3 +276,31 @@ def render_points(scene, cam, W2, H2, point_px=1):
     lib().oracle_render_points(_ptr(scene["sphere_sorted"]), _ptr(scene["rgba_sorted"]), _ptr(scene["sorted_ids"]),
                                scene["N"], _ptr(cam), W2, H2, int(point_px), _ptr(out))
     return out
+
+
+def make_transfer(tents, half_width=0.05, shade=0.45, depth_alpha=0.5, stop_alpha=0.999):
+    """wr_transfer as (int32[1], float32[24]): tents = [(iso, alpha_max, (r, g, b)), ...] (<= 4)."""
+    assert 1 <= len(tents) <= 4
+    f = np.zeros(24, np.float32)
+    for i, (iso, a, rgb) in enumerate(tents):
+        f[i], f[4 + i] = iso, a
+        f[8 + 3 * i: 11 + 3 * i] = rgb
+    f[20:24] = (half_width, shade, depth_alpha, stop_alpha)
+    return np.array([len(tents)], np.int32), f
+
+
+# BASELINE.json configs[0]: "opacity peaks 0.8 at iso 0.35 and 0.95 at iso 0.7"; colours as in synth/
+BASELINE_TENTS = [(0.35, 0.8, (0.95, 0.55, 0.15)), (0.70, 0.95, (0.25, 0.60, 0.95))]
+
+
+def march(volume, cam, W, H, transfer=None):
+    """Server-side ray marcher: (color float32 [H,W,4] premultiplied, depth float32 [H,W])."""
+    vol = _f32(volume)
+    n = vol.shape[0]
+    assert vol.shape == (n, n, n)
+    tn, tf = transfer if transfer is not None else make_transfer(BASELINE_TENTS)
+    cam = _f32(cam)
+    color = np.empty((H, W, 4), np.float32)
+    depth = np.empty((H, W), np.float32)
+    lib().oracle_march(_ptr(vol), n, _ptr(tn), _ptr(tf), _ptr(cam), W, H, _ptr(color), _ptr(depth))
+    return color, depth

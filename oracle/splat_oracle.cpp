@@ -482,6 +482,94 @@ void oracle_render_bvh(const float* sphere, const float* rgba, const uint32_t* i
   }
 }
 
+// ---- Server-side volume ray marcher (first half).  PAPER.md:63 sec. 4.1:
+// "we render the volume using a ray marcher that employs one of the heuristics presented by
+// Zellmann et al. to estimate which depth value represents the volume best.  We march rays
+// r = o + d t"; it "writes out colors and t values to an off-screen buffer".  The
+// paper gives neither its transfer function nor the heuristic's formula; the reading is
+// BASELINE.json's server pass: unit cube, n^3 float32 densities at voxel
+// centres, trilinear, clamp to edge, samples at t0 + (s + 1/2) * step with step = 0.5 / n,
+// opacity tents, premultiplied front-to-back compositing, depth = t of the first sample at which
+// the accumulated alpha reaches depth_alpha (0 if never: dropped), stop at stop_alpha.  float32
+// with the operation order of DESIGN.md S12.  tf = n_tents, then iso[4], alpha[4], rgb[4][3],
+// half_width, shade, depth_alpha, stop_alpha (all float32; layout of wr_transfer).
+static inline float lerp1(float a, float b, float f) { return fmaf(f, b - a, a); }
+
+void oracle_march(const float* vol, int n, const int32_t* tf_n, const float* tf, const float* cam13, int W, int H,
+                  float* color /*[H*W*4]*/, float* depth /*[H*W]*/) {
+  Camera c = load_camera(cam13);
+  const int nt = *tf_n;
+  const float* iso = tf; const float* amax = tf + 4; const float* rgb = tf + 8;
+  const float hw = tf[20], shade = tf[21], depth_alpha = tf[22], stop_alpha = tf[23];
+  const float one_minus_shade = 1.0f - shade;
+  const float fn = (float)n, step = 0.5f / fn;
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      size_t p = (size_t)y * W + x;
+      float d[3], len;
+      pixel_ray(c, W, H, x, y, d, &len);
+      float t0 = 0.0f, t1 = INFINITY;
+      bool miss = false;
+      for (int k = 0; k < 3; ++k) {
+        if (fabsf(d[k]) < 1e-30f) {
+          if (c.e[k] < 0.0f || c.e[k] > 1.0f) miss = true;
+          continue;
+        }
+        float a = (0.0f - c.e[k]) / d[k], b = (1.0f - c.e[k]) / d[k];
+        if (a > b) { float s = a; a = b; b = s; }
+        t0 = fmaxf(t0, a);
+        t1 = fminf(t1, b);
+      }
+      float C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f, tdepth = 0.0f;
+      if (!miss && t0 < t1) {
+        for (int s = 0;; ++s) {
+          float t = fmaf((float)s + 0.5f, step, t0);
+          if (!(t < t1)) break;
+          float P[3], f[3];
+          int i0[3], i1[3];
+          for (int k = 0; k < 3; ++k) {
+            P[k] = fmaf(t, d[k], c.e[k]);
+            float g = fmaf(P[k], fn, -0.5f);
+            float fl = floorf(g);
+            f[k] = g - fl;
+            int a = (int)fl, b = a + 1;
+            a = a < 0 ? 0 : (a > n - 1 ? n - 1 : a);
+            b = b < 0 ? 0 : (b > n - 1 ? n - 1 : b);
+            i0[k] = a; i1[k] = b;
+          }
+          auto V = [&](int i, int j, int k) -> float { return vol[((size_t)k * n + j) * n + i]; };
+          float c00 = lerp1(V(i0[0], i0[1], i0[2]), V(i1[0], i0[1], i0[2]), f[0]);
+          float c10 = lerp1(V(i0[0], i1[1], i0[2]), V(i1[0], i1[1], i0[2]), f[0]);
+          float c01 = lerp1(V(i0[0], i0[1], i1[2]), V(i1[0], i0[1], i1[2]), f[0]);
+          float c11 = lerp1(V(i0[0], i1[1], i1[2]), V(i1[0], i1[1], i1[2]), f[0]);
+          float dens = lerp1(lerp1(c00, c10, f[1]), lerp1(c01, c11, f[1]), f[2]);
+          float alpha = 0.0f;
+          int ci = -1;
+          for (int i = 0; i < nt; ++i) {
+            float w = 1.0f - fabsf(dens - iso[i]) / hw;
+            if (w > 0.0f) {
+              alpha = fmaf(amax[i], w, alpha);
+              if (ci < 0) ci = i;
+            }
+          }
+          if (alpha > 0.0f) {
+            float T = 1.0f - A, Ta = T * alpha;
+            for (int k = 0; k < 3; ++k) {
+              float pc = fminf(fmaxf(P[k], 0.0f), 1.0f);
+              float mod = fmaf(shade, pc, one_minus_shade);
+              C[k] = fmaf(Ta, rgb[3 * ci + k] * mod, C[k]);
+            }
+            A = fmaf(T, alpha, A);
+            if (tdepth == 0.0f && A >= depth_alpha) tdepth = t;
+            if (A >= stop_alpha) break;
+          }
+        }
+      }
+      color[4 * p + 0] = C[0]; color[4 * p + 1] = C[1]; color[4 * p + 2] = C[2]; color[4 * p + 3] = A;
+      depth[p] = tdepth;
+    }
+}
+
 // ---- Comparison renderer: the 2.5D point rendering of [ZAL12] that
 // the paper compares against -- "the authors render the image pixels as point primitives"
 // (PAPER.md:37), object space coordinate -> "window coordinates by applying the viewing and
