@@ -120,7 +120,37 @@ typedef struct {
   float r_max;
 } wr_quant;
 
-/* Server side: Eq. 1 + radius (mode of splats_set_radius) for every pixel of the 2.5D frame,
+/* Server side, first half: the volume ray marcher (sec. 4.1 "we render the volume
+ * using a ray marcher that employs one of the heuristics presented by Zellmann et al. to estimate
+ * which depth value represents the volume best.  We march rays r = o + d t"; PAPER.md:85 it
+ * "writes out colors and t values to an off-screen buffer").  The paper prints neither its
+ * transfer function nor the heuristic; the reading is BASELINE.json's server pass:
+ *   volume   dev, n*n*n float32 densities, x fastest, at the voxel centres of the unit cube
+ *            [0,1]^3; sampled trilinearly, clamped to the edge, at t0 + (s + 1/2) * 0.5/n
+ *   tf       host; opacity = sum over tents of alpha[i] * max(0, 1 - |density - iso[i]| /
+ *            half_width); colour = rgb of the lowest tent with a positive weight, times
+ *            (1 - shade + shade * clamp(position, 0, 1)) per channel; no opacity correction
+ *   color    dev out, H*W*4 float32: premultiplied front-to-back composite, 16-byte aligned
+ *   depth    dev out, H*W float32: ray parameter t (unit direction) of the first sample at which
+ *            the accumulated alpha is >= depth_alpha, 0 if never (a dropped pixel); the march
+ *            stops once the accumulated alpha is >= stop_alpha
+ * The outputs are exactly what splats_update / splats_pack take.  Only enqueues.  Errors:
+ * EINVAL (null pointers, n outside [1, 2048], n_tents outside [1, 4], half_width <= 0, W*H
+ * outside [1, capacity], bad camera). */
+typedef struct {
+  int n_tents;
+  float iso[4];
+  float alpha[4];
+  float rgb[4][3];
+  float half_width;
+  float shade;
+  float depth_alpha;
+  float stop_alpha;
+} wr_transfer;
+int splats_march(const float* volume, int n, const wr_transfer* tf, const wr_camera* camera, int W,
+                 int H, float* color, float* depth);
+
+/* Server side, second half: Eq. 1 + radius (mode of splats_set_radius) for every pixel of the 2.5D frame,
  * quantise, pack, and compact in ascending pixel order (the step the paper runs serially on
  * the CPU: 23 ms at 1024 x 1024).  Only enqueues.
  *   color, depth, src_camera, W, H, r_scale   as splats_update
@@ -223,8 +253,9 @@ int splats_set_radius(int mode, float param);
  * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 first tree kernel
  * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 second tree
  * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render (either query),
- * 6 splats_pack (both launches), 7 splats_render_points (three launches).  calls may be NULL. */
-#define SPLATS_NUM_STAGES 8
+ * 6 splats_pack (both launches), 7 splats_render_points (three launches), 8 splats_march.
+ * calls may be NULL. */
+#define SPLATS_NUM_STAGES 9
 int splats_set_profiling(int on);
 int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);
 

@@ -15,8 +15,8 @@ import torch
 
 from . import build as _build
 
-NUM_STAGES = 8
-STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack", "points")
+NUM_STAGES = 9
+STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack", "points", "march")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
@@ -30,6 +30,12 @@ class SplatsError(RuntimeError):
 
 class wr_quant(ctypes.Structure):
     _fields_ = [("lo", ctypes.c_float * 3), ("hi", ctypes.c_float * 3), ("r_max", ctypes.c_float)]
+
+
+class wr_transfer(ctypes.Structure):
+    _fields_ = [("n_tents", ctypes.c_int), ("iso", ctypes.c_float * 4), ("alpha", ctypes.c_float * 4),
+                ("rgb", (ctypes.c_float * 3) * 4), ("half_width", ctypes.c_float), ("shade", ctypes.c_float),
+                ("depth_alpha", ctypes.c_float), ("stop_alpha", ctypes.c_float)]
 
 
 class wr_camera(ctypes.Structure):
@@ -56,6 +62,7 @@ def lib() -> ctypes.CDLL:
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_points.argtypes = [cam_p, _ci, _ci, _ci, _vp]
+        L.splats_march.argtypes = [_vp, _ci, ctypes.POINTER(wr_transfer), cam_p, _ci, _ci, _vp, _vp]
         L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
         L.splats_update_packed.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
@@ -133,6 +140,25 @@ def splats_render_points(dst_camera, W2: int, H2: int, point_px: int, out_rgba: 
     c = _cam(dst_camera)
     _check(lib().splats_render_points(ctypes.byref(c), int(W2), int(H2), int(point_px),
                                       _dev_ptr(out_rgba, torch.float32, W2 * H2 * 4)))
+
+
+def make_transfer(tents, half_width=0.05, shade=0.45, depth_alpha=0.5, stop_alpha=0.999) -> wr_transfer:
+    """tents = [(iso, alpha_max, (r, g, b)), ...] (at most 4)."""
+    t = wr_transfer()
+    t.n_tents = len(tents)
+    for i, (iso, a, rgb) in enumerate(tents):
+        t.iso[i], t.alpha[i] = iso, a
+        for k in range(3):
+            t.rgb[i][k] = rgb[k]
+    t.half_width, t.shade, t.depth_alpha, t.stop_alpha = half_width, shade, depth_alpha, stop_alpha
+    return t
+
+
+def splats_march(volume: torch.Tensor, n: int, tf: wr_transfer, camera, W: int, H: int, color: torch.Tensor,
+                 depth: torch.Tensor) -> None:
+    c = _cam(camera)
+    _check(lib().splats_march(_dev_ptr(volume, torch.float32, n * n * n), int(n), ctypes.byref(tf), ctypes.byref(c),
+                              int(W), int(H), _dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H)))
 
 
 def _quant(q) -> wr_quant:

@@ -13,6 +13,7 @@
 #include "build_kernels.cuh"
 #include "common.cuh"
 #include "lbvh.cuh"
+#include "march.cuh"
 #include "onesweep.cuh"
 #include "pack.cuh"
 #include "points.cuh"
@@ -447,6 +448,49 @@ int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_
   points_background_kernel<<<grid, POINT_THREADS, 0, c->stream>>>(p);
   if (c->profiling) c->spans.push_back({7, m0, c->mark()});
   c->launches += 3;
+  CU(cudaGetLastError());
+  return SPLATS_OK;
+}
+
+int splats_march(const float* volume, int n, const wr_transfer* tf, const wr_camera* camera, int W, int H, float* color,
+                 float* depth) {
+  int rc = check_frame_args(g_ctx, color, depth, camera, W, H);
+  if (rc) return rc;
+  if (!volume || !tf) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (n < 1 || n > 2048) return fail(SPLATS_EINVAL, "volume size outside [1, 2048]");
+  if (tf->n_tents < 1 || tf->n_tents > 4) return fail(SPLATS_EINVAL, "n_tents outside [1, 4]");
+  if (!(tf->half_width > 0.0f) || !std::isfinite(tf->half_width)) return fail(SPLATS_EINVAL, "half_width must be finite and > 0");
+  if (reinterpret_cast<uintptr_t>(color) & 15u) return fail(SPLATS_EINVAL, "color must be 16-byte aligned");
+  Context* c = g_ctx;
+  MarchParams p;
+  p.vol = volume;
+  p.n = n;
+  p.fn = (float)n;
+  volatile float step = 0.5f / p.fn;
+  p.step = step;
+  p.n_tents = tf->n_tents;
+  for (int i = 0; i < 4; ++i) {
+    p.iso[i] = tf->iso[i];
+    p.amax[i] = tf->alpha[i];
+    for (int k = 0; k < 3; ++k) p.rgb[i][k] = tf->rgb[i][k];
+  }
+  p.hw = tf->half_width;
+  p.shade = tf->shade;
+  volatile float oms = 1.0f - tf->shade;
+  p.one_minus_shade = oms;
+  p.depth_alpha = tf->depth_alpha;
+  p.stop_alpha = tf->stop_alpha;
+  p.cam = make_camera(camera, W, H);
+  p.color = reinterpret_cast<float4*>(color);
+  p.depth = depth;
+  const int tiles = ((W + 7) / 8) * ((H + 3) / 4);
+  const int blocks_needed = (tiles + MARCH_THREADS / 32 - 1) / (MARCH_THREADS / 32);
+  const int grid = blocks_needed < c->num_sms * 16 ? blocks_needed : c->num_sms * 16;
+  size_t m0 = 0;
+  if (c->profiling) m0 = c->mark();
+  march_kernel<<<grid, MARCH_THREADS, 0, c->stream>>>(p);
+  if (c->profiling) c->spans.push_back({8, m0, c->mark()});
+  c->launches += 1;
   CU(cudaGetLastError());
   return SPLATS_OK;
 }
