@@ -76,6 +76,11 @@ def make_workload(config_index: int, n_groups: int | None):
     return cfg, frames
 
 
+def synth_volume(cfg):
+    import synth
+    return synth.volume(cfg)
+
+
 def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
     """Compulsory DRAM traffic per launch for the layout in DESIGN.md sec. 5 (bytes)."""
     return {
@@ -240,6 +245,21 @@ def run_ours(args):
     w_samples = torch.empty(P, dtype=torch.int64, device="cuda")
     w_colors = torch.empty(P, dtype=torch.int32, device="cuda")
     w_count = torch.zeros(1, dtype=torch.int32, device="cuda")
+    d_vol = torch.from_numpy(synth_volume(cfg)).cuda()
+    m_color = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    m_depth = torch.empty((H, W), dtype=torch.float32, device="cuda")
+    tf = sp.make_transfer([(0.35, 0.8, (0.95, 0.55, 0.15)), (0.70, 0.95, (0.25, 0.60, 0.95))])
+    march_ms = []
+    for rep in range(2):
+        for g in range(0, G, max(1, G // 4)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sp.splats_march(d_vol, cfg.vol_n, tf, frames[g]["src_cam"], W, H, m_color, m_depth)
+            e1.record()
+            torch.cuda.synchronize()
+            if rep:
+                march_ms.append(e0.elapsed_time(e1))
+    del d_vol
     sp.splats_set_radius(sp.RADIUS_CONSTANT, half_diag)
     pack_ms, upd_ms, wire_n = [], [], []
     for rep in range(2):                                # first pass warms up
@@ -337,10 +357,11 @@ def run_ours(args):
                            "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": build_bytes,
                            "note": "all build kernels of one splats_update (5 launches), events inside the timed region"},
         "kernels": kernels,
-        "wire_format": {"pack_ms": pack_avg, "pack_gbs": pack_bytes / (pack_avg * 1e-3) / 1e9,
+        "wire_format": {"march_ms": sum(march_ms) / len(march_ms), "pack_ms": pack_avg, "pack_gbs": pack_bytes / (pack_avg * 1e-3) / 1e9,
                         "pack_frac_of_hbm_peak": pack_bytes / (pack_avg * 1e-3) / 1e9 / peak,
                         "update_packed_ms": upd_avg, "samples_avg": n_avg, "payload_bytes_avg": 12 * n_avg,
-                        "note": "splats_pack (Eq. 1, constant half-voxel-diagonal radius, 64-bit samples + RGBA8, GPU "
+                        "note": "splats_march (the server's ray marcher on this config's volume, a few source cameras), "
+                                "splats_pack (Eq. 1, constant half-voxel-diagonal radius, 64-bit samples + RGBA8, GPU "
                                 "compaction; the paper's serial CPU compaction takes 23 ms at 1024x1024, PAPER.md:79) and "
                                 "splats_update_packed on the same source frames"},
         "point_baseline": {"render_ms": points_ms,
