@@ -27,6 +27,14 @@ constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 
 constexpr uint32_t EMPTY_LEAF = 0xffffffffu;
 constexpr uint32_t STACK_DONE = 0xffffffffu;  // not a legal leaf-range code (first < 2^26 - 1)
 
+// the image is written once and not read again by this library: streaming stores keep it from
+// displacing the BVH in L2
+#ifdef SPLATS_OUT_PLAIN
+#define OUT_STORE(p, v) (*(p) = (v))
+#else
+#define OUT_STORE(p, v) __stcs((p), (v))
+#endif
+
 struct RenderParams {
   DevCamera cam;
   const Node* nodes;
@@ -186,7 +194,7 @@ render_kernel(RenderParams prm) {
       const int idx = base + k;
       const int yy = idx / cam.W, xx = idx - yy * cam.W;
       if (idx < total_px && !(xx >= px0 && xx < px1 && yy >= py0 && yy < py1))
-        prm.out[idx] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        OUT_STORE(prm.out + idx, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
     }
     continue;
   }
@@ -338,7 +346,7 @@ render_kernel(RenderParams prm) {
       }
     }
   }
-  if (inside) prm.out[(size_t)y * cam.W + x] = make_float4(C[0], C[1], C[2], A);
+  if (inside) OUT_STORE(prm.out + (size_t)y * cam.W + x, make_float4(C[0], C[1], C[2], A));
   }  // tile loop
   __syncthreads();
   if (tid == 0) {
