@@ -302,6 +302,19 @@ def run_ours(args):
     ms_e2e_dev = timed(step_e2e, K, fin=sp.splats_synchronize)
     wall_e2e = (time.perf_counter() - t0) * 1e3
     ms_e2e = max(ms_e2e_dev, 0.0)
+    # ---- the same end-to-end steps with the 8-bit display image read back (extra key, not the e2e)
+    h_out8 = [torch.empty((H, W), dtype=torch.int32).pin_memory() for _ in range(renders_per_step)]
+
+    def step_e2e8(k: int):
+        f = frames[k % G]
+        sp.splats_update_host(h_color[k % G], h_depth[k % G], f["src_cam"], W, H, cfg.r_scale)
+        for j, cam in enumerate(f["dst_cams"]):
+            sp.splats_render_host_rgba8(cam, W, H, h_out8[j])
+
+    for k in range(min(Wm, 3)):
+        step_e2e8(k)
+    sp.splats_synchronize()
+    ms_e2e8 = timed(step_e2e8, K, fin=sp.splats_synchronize)
     clocks = sampler.stop()
     clocks["samples_in_timed_region"] = n_in_region
 
@@ -345,6 +358,9 @@ def run_ours(args):
         "e2e": {"value": frames_done / (ms_e2e * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": P * 20, "d2h_bytes_per_step": P * 16 * renders_per_step,
                 "wall_ms_per_step": wall_e2e / K},
+        "e2e_rgba8": {"value": frames_done / (ms_e2e8 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": P * 20,
+                      "d2h_bytes_per_step": P * 4 * renders_per_step,
+                      "note": "same steps with splats_render_host_rgba8 (8-bit display image read back instead of float32)"},
         "gpu_launches": int(launches),
         "value_without_stage_events": frames_done / (ms_plain * 1e-3),
         "build_ms": build_ms, "render_ms": render_ms, "mrays_per_s": P / (render_ms * 1e-3) / 1e6,

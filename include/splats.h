@@ -184,6 +184,14 @@ int splats_update_host(const float* color_host, const float* depth_host,
                        const wr_camera* src_camera, int W, int H, float r_scale);
 int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_rgba_host);
 
+/* splats_render with an 8-bit image: every pixel is written as one uint32 R | G << 8 | B << 16 |
+ * A << 24 with round(255 * clamp(c, 0, 1)) per channel of the composited premultiplied colour
+ * (the colour format of the wire, "32 bits per color") -- what a client that only
+ * displays the warped frame needs, at a quarter of the bytes.  out_rgba8: dev (or host for the
+ * _host variant, same pipelining as splats_render_host), H2*W2 uint32.  Errors as splats_render. */
+int splats_render_rgba8(const wr_camera* dst_camera, int W2, int H2, unsigned* out_rgba8);
+int splats_render_host_rgba8(const wr_camera* dst_camera, int W2, int H2, unsigned* out_rgba8_host);
+
 /* Number of splats N of the latest update.  Synchronises the stream.  Parity/debug only. */
 int splats_count(unsigned* n_host);
 

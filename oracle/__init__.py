@@ -81,6 +81,7 @@ def lib():
         L.oracle_composite.restype = _i32
         L.oracle_render_brute.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
         L.oracle_render_bvh.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _i32, _i32, _vp, _i64, _i32, _vp, _vp]
+        L.oracle_quantise_image.argtypes = [_vp, _i64, _vp]
         L.oracle_march.argtypes = [_vp, _i32, _vp, _vp, _vp, _i32, _i32, _vp, _vp]
         L.oracle_render_points.argtypes = [_vp, _vp, _vp, _i64, _vp, _i32, _i32, _i32, _vp]
         _lib = L
@@ -304,3 +305,11 @@ def march(volume, cam, W, H, transfer=None):
     depth = np.empty((H, W), np.float32)
     lib().oracle_march(_ptr(vol), n, _ptr(tn), _ptr(tf), _ptr(cam), W, H, _ptr(color), _ptr(depth))
     return color, depth
+
+
+def quantise_image(rgba):
+    """RGBA8 words (uint32, R | G<<8 | B<<16 | A<<24) of a float image, rounding as the wire's colours."""
+    a = _f32(rgba)
+    out = np.empty(a.shape[:-1], np.uint32)
+    lib().oracle_quantise_image(_ptr(a), out.size, _ptr(out))
+    return out

@@ -275,6 +275,16 @@ int64_t oracle_pack(const float* color, const float* depth, const float* cam13, 
   return n;
 }
 
+// RGBA8 form of a float image (the display format of splats_render_rgba8): the wire's colour
+// quantisation applied to every pixel.
+void oracle_quantise_image(const float* rgba, int64_t n_pixels, uint32_t* out) {
+  for (int64_t p = 0; p < n_pixels; ++p) {
+    uint32_t c8 = 0;
+    for (int k = 0; k < 4; ++k) c8 |= quant_colour(rgba[4 * p + k]) << (8 * k);
+    out[p] = c8;
+  }
+}
+
 // Client side: samples -> spheres (cx, cy, cz, r) and float colours, in the order received.
 // A sample whose radius field is 0 is not a legal sample: valid[i] = 0 and it is dropped later.
 void oracle_decode(const uint64_t* samples, const uint32_t* colours, int64_t n, const float* quant7,

@@ -61,6 +61,8 @@ def lib() -> ctypes.CDLL:
         L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_render_rgba8.argtypes = [cam_p, _ci, _ci, _vp]
+        L.splats_render_host_rgba8.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_points.argtypes = [cam_p, _ci, _ci, _ci, _vp]
         L.splats_march.argtypes = [_vp, _ci, ctypes.POINTER(wr_transfer), cam_p, _ci, _ci, _vp, _vp]
         L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
@@ -193,6 +195,21 @@ def splats_update_host(color, depth, src_camera, W: int, H: int, r_scale: float)
 def splats_render_host(dst_camera, W2: int, H2: int, out_rgba) -> None:
     c = _cam(dst_camera)
     _check(lib().splats_render_host(ctypes.byref(c), int(W2), int(H2), _host_ptr(out_rgba, W2 * H2 * 4)))
+
+
+def splats_render_rgba8(dst_camera, W2: int, H2: int, out_rgba8: torch.Tensor) -> None:
+    """out_rgba8: int32 CUDA tensor of >= W2*H2 (uint32 words R | G<<8 | B<<16 | A<<24)."""
+    c = _cam(dst_camera)
+    _check(lib().splats_render_rgba8(ctypes.byref(c), int(W2), int(H2), _dev_ptr(out_rgba8, torch.int32, W2 * H2)))
+
+
+def splats_render_host_rgba8(dst_camera, W2: int, H2: int, out_rgba8) -> None:
+    """out_rgba8: contiguous int32 host tensor (pinned for asynchronous copies) of >= W2*H2."""
+    if not (isinstance(out_rgba8, torch.Tensor) and not out_rgba8.is_cuda and out_rgba8.is_contiguous()
+            and out_rgba8.dtype == torch.int32 and out_rgba8.numel() >= W2 * H2):
+        raise TypeError("expected a contiguous int32 host tensor of sufficient size")
+    c = _cam(dst_camera)
+    _check(lib().splats_render_host_rgba8(ctypes.byref(c), int(W2), int(H2), out_rgba8.data_ptr()))
 
 
 def splats_count() -> int:

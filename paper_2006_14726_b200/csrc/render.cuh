@@ -42,7 +42,8 @@ struct RenderParams {
   const float4* rgba;
   const uint32_t* ids;
   const FrameState* st;
-  float4* out;
+  float4* out;       // float32 RGBA image ...
+  uint32_t* out8;    // ... or RGBA8 (OUT8 instances): exactly one of the two is used
   unsigned* sched;  // [0] tile ticket, [1] blocks done (both zero between launches)
 };
 
@@ -143,7 +144,9 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 // FIRST = true is the paper's own query ("a simple first-hit ray tracing query and
 // with no shading other than the constant sample color"): a one-entry buffer keeps the nearest
 // hit in (t, id) order, everything beyond it is culled, and its stored colour is copied out.
-template <int KBUF, bool FIRST>
+// OUT8 = true writes the pixel as RGBA8 (round(255 c), the colour format of the wire, S10) instead
+// of four float32: a quarter of the bytes for a client that only displays the image.
+template <int KBUF, bool FIRST, bool OUT8 = false>
 __global__ void __launch_bounds__(RENDER_THREADS, 8)
 render_kernel(RenderParams prm) {
   __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
@@ -194,7 +197,8 @@ render_kernel(RenderParams prm) {
       const int idx = base + k;
       const int yy = idx / cam.W, xx = idx - yy * cam.W;
       if (idx < total_px && !(xx >= px0 && xx < px1 && yy >= py0 && yy < py1))
-        OUT_STORE(prm.out + idx, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
+        if (OUT8) __stcs(prm.out8 + idx, 0u);
+        else OUT_STORE(prm.out + idx, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
     }
     continue;
   }
@@ -346,7 +350,10 @@ render_kernel(RenderParams prm) {
       }
     }
   }
-  if (inside) OUT_STORE(prm.out + (size_t)y * cam.W + x, make_float4(C[0], C[1], C[2], A));
+  if (inside) {
+    if (OUT8) __stcs(prm.out8 + (size_t)y * cam.W + x, pack_colour(make_float4(C[0], C[1], C[2], A)));
+    else OUT_STORE(prm.out + (size_t)y * cam.W + x, make_float4(C[0], C[1], C[2], A));
+  }
   }  // tile loop
   __syncthreads();
   if (tid == 0) {

@@ -288,7 +288,7 @@ int do_update_frame(Context* c, const float* color, const float* depth, const wr
   return do_update(c, src, g, (int64_t)W * H);
 }
 
-int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false) {
+int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false, bool rgba8 = false) {
   RenderParams prm;
   prm.cam = make_camera(cam, W2, H2);
   prm.nodes = c->nodes;
@@ -297,13 +297,15 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   prm.ids = c->val[0];
   prm.st = c->state + c->parity;
   prm.out = reinterpret_cast<float4*>(out);
+  prm.out8 = reinterpret_cast<uint32_t*>(out);
   prm.sched = c->sched;
   const int tiles = ((W2 + 7) / 8) * ((H2 + 3) / 4);
   const int blocks_needed = (tiles + RENDER_THREADS / 32 - 1) / (RENDER_THREADS / 32);
   const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
-  if (first_hit) render_kernel<1, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  if (rgba8) render_kernel<KBUF, false, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  else if (first_hit) render_kernel<1, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
   else render_kernel<KBUF, false><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
   if (c->profiling) c->spans.push_back({5, m0, c->mark()});
   c->launches += 1;
@@ -575,6 +577,33 @@ int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_r
   CU(cudaStreamWaitEvent(c->d2h_stream, c->out_rendered[r], 0));
   CU(cudaMemcpyAsync(out_rgba_host, c->stage_out[r], (size_t)W2 * H2 * 4 * sizeof(float), cudaMemcpyDeviceToHost,
                      c->d2h_stream));
+  CU(cudaEventRecord(c->out_free[r], c->d2h_stream));
+  c->n_readbacks += 1;
+  return SPLATS_OK;
+}
+
+int splats_render_rgba8(const wr_camera* dst_camera, int W2, int H2, unsigned* out_rgba8) {
+  int rc = check_frame_args(g_ctx, out_rgba8, out_rgba8, dst_camera, W2, H2);
+  if (rc) return rc;
+  if (reinterpret_cast<uintptr_t>(out_rgba8) & 3u) return fail(SPLATS_EINVAL, "out_rgba8 must be 4-byte aligned");
+  if (!g_ctx->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_rgba8 before any update");
+  return do_render(g_ctx, dst_camera, W2, H2, reinterpret_cast<float*>(out_rgba8), false, true);
+}
+
+int splats_render_host_rgba8(const wr_camera* dst_camera, int W2, int H2, unsigned* out_rgba8_host) {
+  int rc = check_frame_args(g_ctx, out_rgba8_host, out_rgba8_host, dst_camera, W2, H2);
+  if (rc) return rc;
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_host_rgba8 before any update");
+  rc = ensure_staging(c);
+  if (rc) return rc;
+  const int r = (int)(c->n_readbacks % Context::N_OUT);
+  if (c->n_readbacks >= (unsigned)Context::N_OUT) CU(cudaStreamWaitEvent(c->stream, c->out_free[r], 0));
+  rc = do_render(c, dst_camera, W2, H2, c->stage_out[r], false, true);
+  if (rc) return rc;
+  CU(cudaEventRecord(c->out_rendered[r], c->stream));
+  CU(cudaStreamWaitEvent(c->d2h_stream, c->out_rendered[r], 0));
+  CU(cudaMemcpyAsync(out_rgba8_host, c->stage_out[r], (size_t)W2 * H2 * sizeof(unsigned), cudaMemcpyDeviceToHost, c->d2h_stream));
   CU(cudaEventRecord(c->out_free[r], c->d2h_stream));
   c->n_readbacks += 1;
   return SPLATS_OK;

@@ -288,3 +288,26 @@ def test_error_codes():
         sp.splats_render(cam, 64, 64, out)
         torch.cuda.synchronize()
         assert "context" in sp.splats_last_error() or sp.splats_last_error() != ""
+
+
+def test_rgba8_output_device_and_host():
+    # splats_render_rgba8 / splats_render_host_rgba8: the composited image rounded to 8 bit per channel
+    cfg = synth.make_config(0)
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
+    c2, d2, cam2 = synth.random_frame(130, 50, seed=8, fill=0.6)
+    sc2 = oracle.build_scene(c2, d2, cam2, 130, 50, 2.0)
+    with Session(130, 64) as s:
+        for (scn, col, dep, cam, W, H, rs, dst, W2, H2) in ((sc, color, depth, cfg.src_cams[0], cfg.W, cfg.H, 1.0, cfg.dst_cams[0], 64, 64),
+                                                            (sc2, c2, d2, cam2, 130, 50, 2.0, synth.orbit_camera(7.0), 97, 33)):
+            s.update(col, dep, cam, W, H, rs)
+            want = oracle.quantise_image(oracle.render(scn, dst, W2, H2, "brute"))
+            out = torch.full((H2, W2), 0x5a5a5a5a, dtype=torch.int32, device="cuda")
+            sp.splats_render_rgba8(dst, W2, H2, out)
+            torch.cuda.synchronize()
+            np.testing.assert_array_equal(out.cpu().numpy().view(np.uint32), want)
+            host = torch.zeros((H2, W2), dtype=torch.int32).pin_memory()
+            sp.splats_render_host_rgba8(dst, W2, H2, host)
+            sp.splats_synchronize()
+            np.testing.assert_array_equal(host.numpy().view(np.uint32), want)
+            assert (want != 0).mean() > 0.02

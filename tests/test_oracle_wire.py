@@ -108,3 +108,11 @@ def test_scene_from_packed_samples_renders_like_the_float_scene():
     assert np.array_equal(a, b)
     ref = oracle.render(sc, cfg.dst_cams[0], 64, 64, "brute")
     assert ((a[..., 3] > 0) == (ref[..., 3] > 0)).mean() > 0.99
+
+
+def test_image_quantisation_hand_values():
+    # the display format of splats_render_rgba8 = the wire's colour rounding, per channel
+    img = np.array([[[0.25, 0.5, 1.0, 0.5], [0, 0, 0, 0]], [[2.0, -1.0, 0.999, 0.002], [1 / 255, 0.5 / 255, 0.49 / 255, 254.5 / 255]]], np.float32)
+    q = oracle.quantise_image(img)
+    assert q.shape == (2, 2) and q.dtype == np.uint32
+    assert q.tolist() == [[0x80FF8040, 0], [0x01FF00FF, (255 << 24) | (0 << 16) | (1 << 8) | 1]]
