@@ -173,6 +173,12 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
 int splats_update_packed(const unsigned long long* samples, const unsigned* colors, unsigned n,
                          const wr_quant* quant);
 
+/* splats_update_packed with HOST buffers: what the paper's client does when a frame arrives from
+ * the network -- 12 bytes per sample cross PCIe instead of 20 bytes per pixel.
+ * Pipelined like splats_update_host (the buffers must stay valid until splats_synchronize). */
+int splats_update_packed_host(const unsigned long long* samples_host, const unsigned* colors_host,
+                              unsigned n, const wr_quant* quant);
+
 /* The same two calls with HOST buffers (end-to-end path).  Both only ENQUEUE and return: the
  * frame is uploaded on a copy stream of the library into one of two device staging buffers,
  * the kernels wait for it on the compute stream, and each rendered image is read back on a

@@ -67,6 +67,7 @@ def lib() -> ctypes.CDLL:
         L.splats_march.argtypes = [_vp, _ci, ctypes.POINTER(wr_transfer), cam_p, _ci, _ci, _vp, _vp]
         L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
         L.splats_update_packed.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
+        L.splats_update_packed_host.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render_host.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_count.argtypes = [ctypes.POINTER(ctypes.c_uint)]
@@ -184,6 +185,16 @@ def splats_update_packed(samples: torch.Tensor, colors: torch.Tensor, n: int, qu
     q = _quant(quant)
     _check(lib().splats_update_packed(_dev_ptr(samples, torch.int64, n) if n else None,
                                       _dev_ptr(colors, torch.int32, n) if n else None, int(n), ctypes.byref(q)))
+
+
+def splats_update_packed_host(samples: torch.Tensor, colors: torch.Tensor, n: int, quant) -> None:
+    """samples: int64 host tensor (uint64 words), colors: int32 host tensor; pinned for asynchronous copies."""
+    for t, dt in ((samples, torch.int64), (colors, torch.int32)):
+        if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and t.dtype == dt and t.numel() >= n):
+            raise TypeError(f"expected a contiguous host tensor of dtype {dt} with >= {n} elements")
+    q = _quant(quant)
+    _check(lib().splats_update_packed_host(samples.data_ptr() if n else None, colors.data_ptr() if n else None, int(n),
+                                           ctypes.byref(q)))
 
 
 def splats_update_host(color, depth, src_camera, W: int, H: int, r_scale: float) -> None:

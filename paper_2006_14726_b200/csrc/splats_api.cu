@@ -540,6 +540,37 @@ int splats_update_packed(const unsigned long long* samples, const unsigned* colo
   return do_update(g_ctx, src, g, (int64_t)n);
 }
 
+int splats_update_packed_host(const unsigned long long* samples_host, const unsigned* colors_host, unsigned n,
+                              const wr_quant* quant) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context: call splats_create first");
+  if (!quant || ((!samples_host || !colors_host) && n != 0)) return fail(SPLATS_EINVAL, "null pointer argument");
+  if ((int64_t)n > g_ctx->cap) return fail(SPLATS_EINVAL, "n exceeds the capacity given to splats_create");
+  Context* c = g_ctx;
+  PackedSource src;
+  if (!make_quant(quant, &src.q)) return fail(SPLATS_EINVAL, "quantisation box must be finite with hi > lo, r_max finite and > 0");
+  int rc = ensure_staging(c);
+  if (rc) return rc;
+  // the frame staging buffers are reused: 16 bytes per pixel hold the 8-byte samples, 4 the colours
+  const int u = (int)(c->n_uploads % Context::N_IN);
+  if (c->n_uploads >= (unsigned)Context::N_IN) CU(cudaStreamWaitEvent(c->h2d_stream, c->in_free[u], 0));
+  if (n) {
+    CU(cudaMemcpyAsync(c->stage_color[u], samples_host, (size_t)n * sizeof(uint64_t), cudaMemcpyHostToDevice, c->h2d_stream));
+    CU(cudaMemcpyAsync(c->stage_depth[u], colors_host, (size_t)n * sizeof(uint32_t), cudaMemcpyHostToDevice, c->h2d_stream));
+  }
+  CU(cudaEventRecord(c->in_uploaded[u], c->h2d_stream));
+  CU(cudaStreamWaitEvent(c->stream, c->in_uploaded[u], 0));
+  src.samples = reinterpret_cast<const uint64_t*>(c->stage_color[u]);
+  PackedGather g;
+  g.samples = src.samples;
+  g.colours = reinterpret_cast<const uint32_t*>(c->stage_depth[u]);
+  g.q = src.q;
+  rc = do_update(c, src, g, (int64_t)n);
+  if (rc) return rc;
+  CU(cudaEventRecord(c->in_free[u], c->stream));
+  c->n_uploads += 1;
+  return SPLATS_OK;
+}
+
 int splats_update_host(const float* color_host, const float* depth_host, const wr_camera* src_camera, int W, int H,
                        float r_scale) {
   int rc = check_frame_args(g_ctx, color_host, depth_host, src_camera, W, H);

@@ -131,3 +131,28 @@ def test_config2_paper_shape_constant_radius_round_trip():
         px = rng.choice(cfg.W * cfg.H, size=100_000, replace=False).astype(np.int64)
         assert_rgba_close(s.render(cam, cfg.W, cfg.H).reshape(-1, 4)[px], oracle.render(sc, cam, cfg.W, cfg.H, "bvh", pixels=px), "all-hit")
         sp.splats_set_radius(0, 0.0)
+
+
+def test_packed_host_entry_point_pipelined():
+    # several received frames in flight through splats_update_packed_host + splats_render_host_rgba8
+    cfg = synth.make_config(1)
+    quant = BOX
+    frames = []
+    for b, (W, H) in enumerate(((512, 512), (300, 200), (512, 512), (64, 64))):
+        color, depth, cam = synth.random_frame(W, H, seed=40 + b, fill=0.5) if b % 2 else (*synth.source_frame(cfg, 0), cfg.src_cams[0])
+        rs, rc = oracle.pack(color, depth, cam, W, H, 1.0, quant)
+        frames.append((rs, rc, torch.from_numpy(rs.view(np.int64).copy()).pin_memory(), torch.from_numpy(rc.view(np.int32).copy()).pin_memory()))
+    dst = cfg.dst_cams[1]
+    with Session(512, 512):
+        outs = []
+        for rs, rc, hs, hc in frames:
+            sp.splats_update_packed_host(hs, hc, len(rs), quant)
+            o = torch.zeros((120, 160), dtype=torch.int32).pin_memory()
+            sp.splats_render_host_rgba8(dst, 160, 120, o)
+            outs.append(o)
+        sp.splats_synchronize()
+        for (rs, rc, _, _), o in zip(frames, outs):
+            sc = oracle.build_scene_packed(rs, rc, quant)
+            want = oracle.quantise_image(oracle.render(sc, dst, 160, 120, "bvh"))
+            np.testing.assert_array_equal(o.numpy().view(np.uint32), want)
+        assert_bvh_bit_exact(oracle.build_scene_packed(frames[-1][0], frames[-1][1], quant))
