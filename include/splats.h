@@ -232,7 +232,11 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *       redo the sort with all 8 passes.
  *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
  *     SPLATS_SORT_LSD8_LAUNCHES: one launch per pass.
+ *   SPLATS_OPT_PDL (default 1): launch the kernels of splats_update / splats_render as
+ *     programmatic dependent launches (each kernel waits on its predecessor at its first
+ *     instruction; only the launch latency overlaps).  0 = ordinary stream launches.
  * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
+#define SPLATS_OPT_PDL         2
 #define SPLATS_OPT_REFIT       0
 #define SPLATS_REFIT_PYRAMID   0
 #define SPLATS_REFIT_ATOMIC    1

@@ -71,6 +71,8 @@ struct PackedSource {
 template <class Src>
 __global__ void __launch_bounds__(BUILD_THREADS)
 bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* __restrict__ tile_count) {
+  pdl_wait();
+  pdl_trigger();
   __shared__ float s_red[6][BUILD_THREADS / 32];
   __shared__ uint32_t s_cnt[BUILD_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -181,6 +183,8 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
                  const uint32_t* __restrict__ tile_count, uint64_t* __restrict__ keys0,
                  uint32_t* __restrict__ ids0, uint64_t* __restrict__ keys1, uint32_t* __restrict__ ids1,
                  int sort_mode) {
+  pdl_wait();
+  pdl_trigger();
   __shared__ uint32_t s_hist[8][256];
   __shared__ uint32_t s_warp[BUILD_THREADS / 32];
   __shared__ uint32_t s_part[BUILD_THREADS / 32];

@@ -18,6 +18,16 @@ __device__ __forceinline__ float sub_(float a, float b) { return __fsub_rn(a, b)
 __device__ __forceinline__ float div_(float a, float b) { return __fdiv_rn(a, b); }
 __device__ __forceinline__ float sqrt_(float a) { return __fsqrt_rn(a); }
 
+// ---- programmatic dependent launch (sm_90+): a kernel launched with the stream-serialisation
+// attribute may be scheduled while its predecessor in the stream is still draining; pdl_wait()
+// blocks until that predecessor has completed and its writes are visible, so it must come
+// before the first access to anything the predecessor produced.  Without the attribute both
+// are no-ops.  pdl_trigger() lets the successor's blocks be scheduled once every block of this
+// grid has started (they then sit in pdl_wait), which hides the launch latency between the
+// short dependent kernels of one update.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- camera as kernel parameter (host fills the derived constants in float32)
 struct DevCamera {
   float e[3], R[3], U[3], F[3];

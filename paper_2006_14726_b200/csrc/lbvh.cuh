@@ -166,6 +166,8 @@ template <class Gather>
 __global__ void __launch_bounds__(PYR_THREADS)
 leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
                     float4* __restrict__ sphere, float4* __restrict__ rgba, float4* pyr) {
+  pdl_wait();
+  pdl_trigger();
   __shared__ float s_box[6][PYR_LEAVES];
   __shared__ bool s_last;
   const uint32_t n = st->n;
@@ -355,6 +357,8 @@ __device__ __forceinline__ int descend4(const uint64_t* __restrict__ keys, int n
 __global__ void __launch_bounds__(LBVH_THREADS)
 emit_boxes_kernel(const uint64_t* __restrict__ keys, const float4* __restrict__ sphere,
                   const float4* __restrict__ pyr, FrameState* st, Node* __restrict__ nodes) {
+  pdl_wait();
+  pdl_trigger();
   const int n = (int)st->n;
   if (n == 1 && blockIdx.x == 0 && threadIdx.x == 0) {  // the single leaf is the root
     float lo[3], hi[3];

@@ -317,6 +317,8 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
 #endif
 __global__ void __launch_bounds__(SORT_THREADS, SPLATS_SORT_BLOCKS)
 onesweep_kernel(SortArgs a) {
+  pdl_wait();
+  pdl_trigger();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
   const uint32_t n = a.st->n;

@@ -149,6 +149,8 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 template <int KBUF, bool FIRST, bool OUT8 = false>
 __global__ void __launch_bounds__(RENDER_THREADS, 8)
 render_kernel(RenderParams prm) {
+  pdl_wait();
+  pdl_trigger();
   __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
   __shared__ float s_tn[SSTACK][RENDER_THREADS];
   __shared__ int s_rect[4];

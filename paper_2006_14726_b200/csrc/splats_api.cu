@@ -49,6 +49,7 @@ struct Context {
   int refit_mode = SPLATS_REFIT_PYRAMID;
   int sort_mode = SPLATS_SORT_HYBRID;
   int radius_mode = SPLATS_RADIUS_FOOTPRINT;
+  bool pdl = true;                  // programmatic dependent launches between the hot-path kernels
   float radius_param = 0.0f;
   // staging for the *_host calls: copies run on their own streams, double / triple buffered,
   // so the upload of frame f+1 and the read-back of image i-1 overlap the kernels of image i
@@ -132,6 +133,22 @@ float radius_factor(const wr_camera* c, int H, float r_scale) {
   volatile float b = 2.0f * c->tan_half_fovy;
   volatile float q = b / (float)H;
   return a * q;
+}
+
+// Launch on the context's stream, optionally as a programmatic dependent launch (common.cuh).
+template <typename... KArgs, typename... Args>
+void launch(bool pdl, void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
 template <typename T>
@@ -223,11 +240,12 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
 
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
-  bounds_kernel<Src><<<tiles, BUILD_THREADS, 0, s>>>(src, P, st, c->tile_count);
+  const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
+  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
-  unproject_kernel<Src><<<grid2, BUILD_THREADS, 0, s>>>(src, P, tiles, st, st_next, c->tile_count, c->key[0], c->val[0],
-                                                       c->key[1], c->val[1], c->sort_mode);
+  launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
+         c->val[0], c->key[1], c->val[1], c->sort_mode);
   if (prof) m[2] = c->mark();
   const int max_sort_tiles = P > 0 ? (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE) : 1;
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
@@ -249,7 +267,7 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
     sa.pass = 0;
     sa.epoch0 = c->epoch + 1;
     c->epoch += 16;
-    onesweep_kernel<<<sgrid, SORT_THREADS, c->sort_smem, s>>>(sa);
+    launch(pdl, onesweep_kernel, sgrid, SORT_THREADS, c->sort_smem, s, sa);
   }
   if (prof) m[3] = c->mark();
   const int lgrid_max = P > 0 ? (int)((P + LBVH_THREADS - 1) / LBVH_THREADS) : 1;
@@ -261,9 +279,9 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
     refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
-    leaf_pyramid_kernel<Gather><<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], gather, st, c->sphere, c->rgba, c->pyr);
+    launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, c->sphere, c->rgba, c->pyr);
     if (prof) m[4] = c->mark();
-    emit_boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->sphere, c->pyr, st, c->nodes);
+    launch(pdl, emit_boxes_kernel, lgrid, LBVH_THREADS, 0, s, c->key[0], c->sphere, c->pyr, st, c->nodes);
   }
   if (prof) m[5] = c->mark();
   c->launches += 4 + sort_launches;
@@ -304,9 +322,10 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
-  if (rgba8) render_kernel<KBUF, false, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
-  else if (first_hit) render_kernel<1, true><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
-  else render_kernel<KBUF, false><<<grid, RENDER_THREADS, 0, c->stream>>>(prm);
+  const bool pdl = c->pdl && !c->profiling;
+  if (rgba8) launch(pdl, render_kernel<KBUF, false, true>, grid, RENDER_THREADS, 0, c->stream, prm);
+  else if (first_hit) launch(pdl, render_kernel<1, true, false>, grid, RENDER_THREADS, 0, c->stream, prm);
+  else launch(pdl, render_kernel<KBUF, false, false>, grid, RENDER_THREADS, 0, c->stream, prm);
   if (c->profiling) c->spans.push_back({5, m0, c->mark()});
   c->launches += 1;
   CU(cudaGetLastError());
@@ -711,6 +730,10 @@ int splats_set_option(int option, int value) {
       if (value != SPLATS_SORT_HYBRID && value != SPLATS_SORT_LSD8 && value != SPLATS_SORT_LSD8_LAUNCHES)
         return fail(SPLATS_EINVAL, "unknown sort mode");
       g_ctx->sort_mode = value;
+      return SPLATS_OK;
+    case SPLATS_OPT_PDL:
+      if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_PDL takes 0 or 1");
+      g_ctx->pdl = value != 0;
       return SPLATS_OK;
     default:
       return fail(SPLATS_EINVAL, "unknown option");
