@@ -6,7 +6,11 @@ frames with the camera dollying towards the centre, a splat + BVH rebuild every 
 One *step* = one pass of the whole hot path over one source frame: 1 splats_update (bounds,
 unproject+Morton+compaction, onesweep sort, gather+box pyramid, hierarchy+node boxes; 5 launches)
 followed by the 4 splats_render calls of the display frames that use that BVH.  Step k uses source frame k mod 15,
-so 15 steps are exactly the scripted 60-frame sequence.  value = display frames / second.
+so 15 steps are exactly the scripted 60-frame sequence.  value = display frames / second, timed
+with CUDA events around exactly K steps of the library as a user runs it (programmatic dependent
+launches; the four renders of a step write four images and may overlap, SPLATS_OPT_OVERLAP).  The
+per-kernel table and the roofline come from a second pass over the same K steps with per-stage
+events on the library's stream (which serialises the stages; its rate is value_with_stage_events).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
@@ -194,22 +198,25 @@ def run_ours(args):
         return replicas.max_over_ranks(e0.elapsed_time(e1))
 
     K, Wm = args.steps, args.warmup
+    # the four renders of a step go to four different images: let them overlap (include/splats.h)
+    sp.splats_set_option(sp.OPT_OVERLAP, 1)
     for k in range(Wm):
         step(k)
     barrier()
 
     sampler = ClockSampler(local_rank)
     sampler.start()
-    # ---- timed region: K steps, per-stage CUDA events recorded inside it (library stream)
-    sp.splats_set_profiling(True)
+    # ---- timed region: exactly K steps, the library as a user runs it (no per-stage events)
     launches0 = sp.splats_launch_count()
     ms_total = timed(step, K)
     launches = sp.splats_launch_count() - launches0
+    n_in_region = len(sampler.samples)
+    # ---- the same K steps again with per-stage CUDA events on the library's stream (the events
+    # serialise the stages, so this pass is a little slower; kernels / roofline come from it)
+    sp.splats_set_profiling(True)
+    ms_staged = timed(step, K)
     stage = sp.splats_stage_ms()
     sp.splats_set_profiling(False)
-    n_in_region = len(sampler.samples)
-    # ---- same K steps without the per-stage events (reported beside the headline)
-    ms_plain = timed(step, K)
 
     # ---- the paper's first-hit query on the same sequence: renders only,
     # reported beside the headline, not part of it
@@ -358,7 +365,7 @@ def run_ours(args):
             continue
         gbs = bytes_sum[name] / (ms_sum * 1e-3) / 1e9 if ms_sum > 0 else 0.0
         kernels.append({"stage": name, "launches_per_call": 1, "calls": calls,
-                        "ms_avg": ms_sum / calls, "share": ms_sum / ms_total, "algorithmic_bytes_avg": bytes_sum[name] / calls,
+                        "ms_avg": ms_sum / calls, "share": ms_sum / ms_staged, "algorithmic_bytes_avg": bytes_sum[name] / calls,
                         "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak})
     dominant = max(kernels, key=lambda r: r["share"])
     build = [r for r in kernels if r["stage"] != "render"]
@@ -375,6 +382,9 @@ def run_ours(args):
                                f"r_scale {cfg.r_scale}, dolly x0.5 over the sequence",
                    "splats_per_frame_min_max": [min(steps_N), max(steps_N)],
                    "l2_policy": f"inputs larger than L2: {G} source frames x {P * 20 / 1e6:.1f} MB cycled",
+                   "launch_mode": "programmatic dependent launches, consecutive renders of a step overlap "
+                                  "(SPLATS_OPT_PDL, SPLATS_OPT_OVERLAP); kernels / roofline from a second pass of the same "
+                                  "steps with per-stage events, stages serialised",
                    "parallelism": "replicas" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": frames_done / (ms_e2e * 1e-3), "unit": UNIT,
@@ -388,7 +398,7 @@ def run_ours(args):
                              "note": "splats_update_packed_host (64-bit samples + RGBA8 colours from pinned host memory, "
                                      "constant half-voxel-diagonal radius) + 4 x splats_render_host_rgba8 per step"},
         "gpu_launches": int(launches),
-        "value_without_stage_events": frames_done / (ms_plain * 1e-3),
+        "value_with_stage_events": frames_done / (ms_staged * 1e-3), "ms_per_step_with_stage_events": ms_staged / K,
         "build_ms": build_ms, "render_ms": render_ms, "mrays_per_s": P / (render_ms * 1e-3) / 1e6,
         "roofline": {"kernel": dominant["stage"], "bound": "hbm", "achieved": dominant["achieved_gbs"], "peak": peak,
                      "unit": "GB/s", "frac": dominant["achieved_gbs"] / peak,

@@ -235,8 +235,18 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *   SPLATS_OPT_PDL (default 1): launch the kernels of splats_update / splats_render as
  *     programmatic dependent launches (each kernel waits on its predecessor at its first
  *     instruction; only the launch latency overlaps).  0 = ordinary stream launches.
+ *   SPLATS_OPT_OVERLAP (default 0; needs SPLATS_OPT_PDL): consecutive splats_render* calls that
+ *     use the same BVH and write disjoint images do not depend on each other, so up to four of
+ *     them are allowed to execute concurrently: the next render's blocks fill the SMs that the
+ *     tail of the previous one leaves idle.  Results are unchanged.  Stream order is kept towards
+ *     everything else (updates, other calls of this library, later work of the caller), and a
+ *     render whose image overlaps one that may still be in flight is serialised.  The one thing
+ *     given up: work that the CALLER enqueues between two such render calls is not guaranteed to
+ *     be complete before the second render starts writing its image (the render reads nothing
+ *     of the caller's, so this only matters if that work writes the same image).
  * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
 #define SPLATS_OPT_PDL         2
+#define SPLATS_OPT_OVERLAP     3
 #define SPLATS_OPT_REFIT       0
 #define SPLATS_REFIT_PYRAMID   0
 #define SPLATS_REFIT_ATOMIC    1

@@ -21,6 +21,7 @@ OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC = 0, 0, 1
 OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
 OPT_PDL = 2
+OPT_OVERLAP = 3
 
 
 class SplatsError(RuntimeError):

@@ -44,7 +44,8 @@ struct RenderParams {
   const FrameState* st;
   float4* out;       // float32 RGBA image ...
   uint32_t* out8;    // ... or RGBA8 (OUT8 instances): exactly one of the two is used
-  unsigned* sched;  // [0] tile ticket, [1] blocks done (both zero between launches)
+  unsigned* sched;  // [0] tile ticket, [1] blocks done (both zero between launches); one pair per render in flight
+  int wait_prev;    // 0: this render does not depend on the kernel before it in the stream (see do_render)
 };
 
 #ifdef SPLATS_STATS
@@ -149,7 +150,7 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 template <int KBUF, bool FIRST, bool OUT8 = false>
 __global__ void __launch_bounds__(RENDER_THREADS, 8)
 render_kernel(RenderParams prm) {
-  pdl_wait();
+  if (prm.wait_prev) pdl_wait();
   pdl_trigger();
   __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
   __shared__ float s_tn[SSTACK][RENDER_THREADS];

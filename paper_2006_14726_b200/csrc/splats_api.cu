@@ -35,7 +35,12 @@ struct Context {
   // device memory
   FrameState* state = nullptr;      // [2], by frame parity
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
-  unsigned* sched = nullptr;        // render tile ticket + done counter
+  unsigned* sched = nullptr;        // render tile ticket + done counter, one pair per render in flight
+  // renders launched since the last fully serialising launch on the stream (see do_render)
+  static constexpr int MAX_OVERLAP = 4;
+  int render_streak = 0;
+  const char* inflight_lo[MAX_OVERLAP] = {};
+  const char* inflight_hi[MAX_OVERLAP] = {};
   uint64_t* key[2] = {nullptr, nullptr};
   uint32_t* val[2] = {nullptr, nullptr};
   uint64_t* status = nullptr;       // [max sort tiles][256]
@@ -50,6 +55,7 @@ struct Context {
   int sort_mode = SPLATS_SORT_HYBRID;
   int radius_mode = SPLATS_RADIUS_FOOTPRINT;
   bool pdl = true;                  // programmatic dependent launches between the hot-path kernels
+  bool overlap = false;             // consecutive independent renders may run concurrently (SPLATS_OPT_OVERLAP)
   float radius_param = 0.0f;
   // staging for the *_host calls: copies run on their own streams, double / triple buffered,
   // so the upload of frame f+1 and the read-back of image i-1 overlap the kernels of image i
@@ -241,7 +247,9 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
   const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
-  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
+  c->render_streak = 0;
+  // an ordinary launch: everything before it in the stream, overlapping renders included, is complete
+  launch(false, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
   launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
@@ -316,13 +324,41 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   prm.st = c->state + c->parity;
   prm.out = reinterpret_cast<float4*>(out);
   prm.out8 = reinterpret_cast<uint32_t*>(out);
-  prm.sched = c->sched;
   const int tiles = ((W2 + 7) / 8) * ((H2 + 3) / 4);
   const int blocks_needed = (tiles + RENDER_THREADS / 32 - 1) / (RENDER_THREADS / 32);
   const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
-  const bool pdl = c->pdl && !c->profiling;
+  // Renders of one BVH into disjoint images do not depend on each other, so up to MAX_OVERLAP
+  // consecutive ones are launched as programmatic dependents that do NOT wait for their
+  // predecessor: the next render's blocks fill the SMs that the tail of the previous one leaves
+  // idle.  The first render after anything else waits (the BVH must be complete; everything
+  // before it in the stream is ordered), every MAX_OVERLAP-th one and any render whose image
+  // overlaps one that may still be in flight is an ordinary launch (full stream order), and so
+  // is the first kernel of whatever follows (bounds_kernel, pack, points, ...).  Each render in
+  // flight has its own pair of ticket counters.
+  const char* out_lo = reinterpret_cast<const char*>(out);
+  const char* out_hi = out_lo + (size_t)W2 * H2 * (rgba8 ? 4 : 16);
+  bool pdl = c->pdl && !c->profiling;
+  int wait_prev = 1;
+  if (!(pdl && c->overlap)) {
+    c->render_streak = 0;   // every render waits for its predecessor; one pair of ticket counters
+  } else if (c->render_streak > 0) {
+    bool independent = c->render_streak < Context::MAX_OVERLAP;
+    for (int i = 0; i < c->render_streak && independent; ++i)
+      if (out_lo < c->inflight_hi[i] && c->inflight_lo[i] < out_hi) independent = false;
+    if (independent) {
+      wait_prev = 0;
+    } else {
+      pdl = false;          // an ordinary launch: serialised against everything before it
+      c->render_streak = 0;
+    }
+  }
+  prm.wait_prev = wait_prev;
+  prm.sched = c->sched + 2 * c->render_streak;
+  c->inflight_lo[c->render_streak] = out_lo;
+  c->inflight_hi[c->render_streak] = out_hi;
+  c->render_streak = (pdl && c->overlap) ? c->render_streak + 1 : 0;
   if (rgba8) launch(pdl, render_kernel<KBUF, false, true>, grid, RENDER_THREADS, 0, c->stream, prm);
   else if (first_hit) launch(pdl, render_kernel<1, true, false>, grid, RENDER_THREADS, 0, c->stream, prm);
   else launch(pdl, render_kernel<KBUF, false, false>, grid, RENDER_THREADS, 0, c->stream, prm);
@@ -360,8 +396,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   const size_t max_sort_tiles = (cap + SORT_MIN_TILE - 1) / SORT_MIN_TILE;
   if (e == cudaSuccess) e = dmalloc(&c->state, 2);
   if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
-  if (e == cudaSuccess) e = dmalloc(&c->sched, 2);
-  if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * sizeof(unsigned));
+  if (e == cudaSuccess) e = dmalloc(&c->sched, 2 * Context::MAX_OVERLAP);
+  if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * Context::MAX_OVERLAP * sizeof(unsigned));
   for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
     e = dmalloc(&c->key[i], cap);
     if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
@@ -464,6 +500,7 @@ int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_
   const int grid = c->num_sms * 8;
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
+  c->render_streak = 0;
   points_kernel<false><<<grid, POINT_THREADS, 0, c->stream>>>(p);
   points_kernel<true><<<grid, POINT_THREADS, 0, c->stream>>>(p);
   points_background_kernel<<<grid, POINT_THREADS, 0, c->stream>>>(p);
@@ -509,6 +546,7 @@ int splats_march(const float* volume, int n, const wr_transfer* tf, const wr_cam
   const int grid = blocks_needed < c->num_sms * 16 ? blocks_needed : c->num_sms * 16;
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
+  c->render_streak = 0;
   march_kernel<<<grid, MARCH_THREADS, 0, c->stream>>>(p);
   if (c->profiling) c->spans.push_back({8, m0, c->mark()});
   c->launches += 1;
@@ -535,6 +573,7 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
   a.num_tiles = (int)((a.P + TILE_PX - 1) / TILE_PX);
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
+  c->render_streak = 0;
   pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count);
   const int grid2 = a.num_tiles < c->num_sms * 4 ? a.num_tiles : c->num_sms * 4;
   pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
@@ -730,6 +769,11 @@ int splats_set_option(int option, int value) {
       if (value != SPLATS_SORT_HYBRID && value != SPLATS_SORT_LSD8 && value != SPLATS_SORT_LSD8_LAUNCHES)
         return fail(SPLATS_EINVAL, "unknown sort mode");
       g_ctx->sort_mode = value;
+      return SPLATS_OK;
+    case SPLATS_OPT_OVERLAP:
+      if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_OVERLAP takes 0 or 1");
+      g_ctx->overlap = value != 0;
+      g_ctx->render_streak = 0;
       return SPLATS_OK;
     case SPLATS_OPT_PDL:
       if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_PDL takes 0 or 1");

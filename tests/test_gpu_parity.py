@@ -311,3 +311,53 @@ def test_rgba8_output_device_and_host():
             sp.splats_synchronize()
             np.testing.assert_array_equal(host.numpy().view(np.uint32), want)
             assert (want != 0).mean() > 0.02
+
+
+def test_overlapping_renders_option():
+    # SPLATS_OPT_OVERLAP: consecutive renders of one BVH into disjoint images may run concurrently.
+    # Eleven renders in a row (every fourth is serialised), two of them into the same buffer, an
+    # update in between, first-hit / rgba8 / points mixed in: every image equals the serial result.
+    cfg = synth.make_config(1)
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, 1.0)
+    c2, d2, cam2 = synth.random_frame(300, 200, seed=12, fill=0.7)
+    sc2 = oracle.build_scene(c2, d2, cam2, 300, 200, 2.0)
+    W, H = cfg.W, cfg.H
+    cams = [synth.orbit_camera(2.0 * i, 1.0 * i) for i in range(11)]
+    with Session(W, H) as s:
+        sp.splats_set_option(sp.OPT_OVERLAP, 1)
+        s.update(color, depth, cfg.src_cams[0], W, H, 1.0)
+        outs = [torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda") for _ in range(11)]
+        for i, cam in enumerate(cams):
+            sp.splats_render(cam, W, H, outs[i])
+        shared = torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda")
+        sp.splats_render(cams[0], W, H, shared)
+        sp.splats_render(cams[5], W, H, shared)             # same image twice: the second one must win
+        fh = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        sp.splats_render_first_hit(cams[3], W, H, fh)
+        o8 = torch.empty((H, W), dtype=torch.int32, device="cuda")
+        sp.splats_render_rgba8(cams[4], W, H, o8)
+        pts = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        sp.splats_render_points(cams[2], W, H, 2, pts)
+        # a new frame while the renders above may still be in flight, then renders of the new BVH
+        dc2, dd2 = torch.from_numpy(c2).cuda(), torch.from_numpy(d2).cuda()
+        sp.splats_update(dc2, dd2, cam2, 300, 200, 2.0)
+        new = [torch.empty((120, 160, 4), dtype=torch.float32, device="cuda") for _ in range(3)]
+        for i in range(3):
+            sp.splats_render(cams[i + 1], 160, 120, new[i])
+        torch.cuda.synchronize()
+        for i in (0, 3, 4, 7, 10):
+            assert_rgba_close(outs[i].cpu().numpy(), oracle.render(sc, cams[i], W, H, "bvh"), f"render {i}")
+        ref5 = oracle.render(sc, cams[5], W, H, "bvh")
+        assert_rgba_close(shared.cpu().numpy(), ref5, "aliased image")
+        assert np.array_equal(fh.cpu().numpy(), oracle.render(sc, cams[3], W, H, "bvh", first_hit=True))
+        np.testing.assert_array_equal(o8.cpu().numpy().view(np.uint32), oracle.quantise_image(oracle.render(sc, cams[4], W, H, "bvh")))
+        assert np.array_equal(pts.cpu().numpy(), oracle.render_points(sc, cams[2], W, H, 2))
+        for i in range(3):
+            assert_rgba_close(new[i].cpu().numpy(), oracle.render(sc2, cams[i + 1], 160, 120, "bvh"), f"new frame render {i}")
+        # serial and overlapped executions give identical bits
+        sp.splats_set_option(sp.OPT_OVERLAP, 0)
+        serial = torch.empty((120, 160, 4), dtype=torch.float32, device="cuda")
+        sp.splats_render(cams[2], 160, 120, serial)
+        torch.cuda.synchronize()
+        assert torch.equal(serial, new[1])
