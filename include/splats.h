@@ -236,7 +236,7 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *     programmatic dependent launches (each kernel waits on its predecessor at its first
  *     instruction; only the launch latency overlaps).  0 = ordinary stream launches.
  *   SPLATS_OPT_OVERLAP (default 0; needs SPLATS_OPT_PDL): consecutive splats_render* calls that
- *     use the same BVH and write disjoint images do not depend on each other, so up to four of
+ *     use the same BVH and write disjoint images do not depend on each other, so up to eight of
  *     them are allowed to execute concurrently: the next render's blocks fill the SMs that the
  *     tail of the previous one leaves idle.  Results are unchanged.  Stream order is kept towards
  *     everything else (updates, other calls of this library, later work of the caller), and a

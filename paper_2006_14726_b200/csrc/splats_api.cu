@@ -37,7 +37,7 @@ struct Context {
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
   unsigned* sched = nullptr;        // render tile ticket + done counter, one pair per render in flight
   // renders launched since the last fully serialising launch on the stream (see do_render)
-  static constexpr int MAX_OVERLAP = 4;
+  static constexpr int MAX_OVERLAP = 8;
   int render_streak = 0;
   const char* inflight_lo[MAX_OVERLAP] = {};
   const char* inflight_hi[MAX_OVERLAP] = {};

@@ -315,7 +315,7 @@ def test_rgba8_output_device_and_host():
 
 def test_overlapping_renders_option():
     # SPLATS_OPT_OVERLAP: consecutive renders of one BVH into disjoint images may run concurrently.
-    # Eleven renders in a row (every fourth is serialised), two of them into the same buffer, an
+    # Eleven renders in a row (the ninth is serialised), two of them into the same buffer, an
     # update in between, first-hit / rgba8 / points mixed in: every image equals the serial result.
     cfg = synth.make_config(1)
     color, depth = synth.source_frame(cfg, 0)
