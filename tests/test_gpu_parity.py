@@ -361,3 +361,37 @@ def test_overlapping_renders_option():
         sp.splats_render(cams[2], 160, 120, serial)
         torch.cuda.synchronize()
         assert torch.equal(serial, new[1])
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_seeded_fuzz_whole_path(seed):
+    # random sizes, fills, radii, source kinds (frame / packed) and options; everything bit-exact
+    rng = np.random.default_rng(1000 + seed)
+    W, H = int(rng.integers(1, 400)), int(rng.integers(1, 300))
+    fill = float(rng.choice([0.02, 0.3, 0.7, 1.0]))
+    r_scale = float(rng.choice([0.5, 1.0, 1.0, 2.0, 3.5]))
+    radius = [(0, 0.0), (0, 0.0), (1, 0.006), (2, 0.3)][int(rng.integers(4))]
+    color, depth, cam = synth.random_frame(W, H, seed=seed, fill=fill, cam=synth.orbit_camera(float(rng.uniform(-40, 40)), float(rng.uniform(-20, 20))))
+    if seed % 3 == 0:
+        depth[depth > 0] = np.float32(3.0 + 0.01 * (seed % 5))        # coplanar: many equal codes / equal t
+    W2, H2 = int(rng.integers(1, 200)), int(rng.integers(1, 150))
+    dst = synth.orbit_camera(float(rng.uniform(-30, 30)), float(rng.uniform(-15, 15)), float(rng.uniform(2.0, 5.0)))
+    with Session(max(W, 200), max(H, 150)) as s:
+        sp.splats_set_option(sp.OPT_OVERLAP, seed % 2)
+        sp.splats_set_option(sp.OPT_SORT, [sp.SORT_HYBRID, sp.SORT_HYBRID, sp.SORT_LSD8][seed % 3])
+        sc, _ = check_scene(s, color, depth, cam, W, H, r_scale, [dst, cam], [(W2, H2), (W2, H2)], mode="bvh", radius=radius)
+        fh = s.render(dst, W2, H2, first_hit=True)
+        assert np.array_equal(fh, oracle.render(sc, dst, W2, H2, "bvh", first_hit=True))
+        pts = torch.empty((H2, W2, 4), dtype=torch.float32, device="cuda")
+        sp.splats_render_points(dst, W2, H2, 1 + seed % 3, pts)
+        assert np.array_equal(pts.cpu().numpy(), oracle.render_points(sc, dst, W2, H2, 1 + seed % 3))
+        # the same frame through the wire format
+        quant = np.array([-4, -4, -4, 5, 5, 5, 0.05], np.float32)
+        rs, rc = oracle.pack(color, depth, cam, W, H, r_scale, quant, radius[0], radius[1])
+        scp = oracle.build_scene_packed(rs, rc, quant)
+        ws = torch.from_numpy(np.ascontiguousarray(rs.view(np.int64) if len(rs) else np.zeros(1, np.int64))).cuda()
+        cs = torch.from_numpy(np.ascontiguousarray(rc.view(np.int32) if len(rc) else np.zeros(1, np.int32))).cuda()
+        sp.splats_update_packed(ws, cs, len(rs), quant)
+        assert_bvh_bit_exact(scp)
+        assert_rgba_close(s.render(dst, W2, H2), oracle.render(scp, dst, W2, H2, "bvh"), "packed")
+        sp.splats_set_radius(0, 0.0)
