@@ -59,14 +59,16 @@ template <class Gather>
 __global__ void __launch_bounds__(LBVH_THREADS)
 emit_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src,
             const FrameState* __restrict__ st, float4* __restrict__ sphere, float4* __restrict__ rgba,
-            Node* __restrict__ nodes, int* __restrict__ leaf_parent) {
+            uint32_t* __restrict__ ids_out, Node* __restrict__ nodes, int* __restrict__ leaf_parent) {
   const int n = (int)st->n;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     // ---- (a) gather
     float4 sp, col;
-    src.get(__ldg(perm + i), sp, col);
+    const uint32_t id = __ldg(perm + i);
+    src.get(id, sp, col);
     sphere[i] = sp;
     rgba[i] = col;
+    ids_out[i] = id;   // the BVH keeps its own copy: the sort buffers belong to the next build
     if (n == 1) leaf_parent[0] = -1;
     if (i >= n - 1) continue;
 
@@ -165,7 +167,7 @@ __device__ __forceinline__ void box_of_sphere(const float4 sp, float lo[3], floa
 template <class Gather>
 __global__ void __launch_bounds__(PYR_THREADS)
 leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
-                    float4* __restrict__ sphere, float4* __restrict__ rgba, float4* pyr) {
+                    float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, float4* pyr) {
   pdl_wait();
   pdl_trigger();
   __shared__ float s_box[6][PYR_LEAVES];
@@ -185,9 +187,11 @@ leaf_pyramid_kernel(const uint32_t* __restrict__ perm, const Gather src, FrameSt
     float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
     if (i < n) {
       float4 sp, col;
-      src.get(__ldg(perm + i), sp, col);
+      const uint32_t id = __ldg(perm + i);
+      src.get(id, sp, col);
       sphere[i] = sp;
       rgba[i] = col;
+      ids_out[i] = id;   // the BVH keeps its own copy: the sort buffers belong to the next build
       box_of_sphere(sp, lo, hi);
     }
 #pragma unroll

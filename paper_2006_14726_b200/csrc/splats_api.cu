@@ -33,7 +33,7 @@ struct Context {
   int64_t cap = 0;
   int num_sms = 0;
   // device memory
-  FrameState* state = nullptr;      // [2], by frame parity
+  FrameState* state = nullptr;      // [3]: frame f uses state[f % 3] and re-arms state[(f + 1) % 3]
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
   unsigned* sched = nullptr;        // render tile ticket + done counter, one pair per render in flight
   // renders launched since the last fully serialising launch on the stream (see do_render)
@@ -44,9 +44,20 @@ struct Context {
   uint64_t* key[2] = {nullptr, nullptr};
   uint32_t* val[2] = {nullptr, nullptr};
   uint64_t* status = nullptr;       // [max sort tiles][256]
-  float4* sphere = nullptr;
-  float4* rgba = nullptr;
-  Node* nodes = nullptr;
+  // Two complete BVHs: build f writes set[f & 1] while the renders may still read the other one
+  // (splats_update_begin / splats_update_commit); splats, colours, ids, nodes in sorted order.
+  struct BvhSet {
+    float4* sphere = nullptr;
+    float4* rgba = nullptr;
+    uint32_t* ids = nullptr;
+    Node* nodes = nullptr;
+  } set[2];
+  int cur_set = 0, cur_state = 0;   // what splats_render* reads
+  // a build enqueued by splats_update_begin that splats_update_commit has not made current yet
+  bool pending = false;
+  int pending_set = 0, pending_state = 0;
+  cudaStream_t build_stream = nullptr;   // high priority; created on the first splats_update_begin
+  cudaEvent_t ev_begin = nullptr, ev_built = nullptr;
   uint64_t* zkey = nullptr;         // depth buffer of splats_render_points, all ones between calls
   int* leaf_parent = nullptr;
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
@@ -69,7 +80,6 @@ struct Context {
   unsigned n_uploads = 0, n_readbacks = 0;
   // frame bookkeeping
   unsigned frame = 0;               // number of updates enqueued
-  int parity = 0;                   // FrameState of the latest update
   uint32_t epoch = 0;
   bool has_bvh = false;
   int sort_grid = 0;
@@ -165,7 +175,11 @@ cudaError_t dmalloc(T** p, size_t count) {
 void free_all(Context* c) {
   cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
-  cudaFree(c->status); cudaFree(c->sphere); cudaFree(c->rgba); cudaFree(c->nodes);
+  cudaFree(c->status);
+  for (int i = 0; i < 2; ++i) { cudaFree(c->set[i].sphere); cudaFree(c->set[i].rgba); cudaFree(c->set[i].ids); cudaFree(c->set[i].nodes); }
+  if (c->build_stream) cudaStreamDestroy(c->build_stream);
+  if (c->ev_begin) cudaEventDestroy(c->ev_begin);
+  if (c->ev_built) cudaEventDestroy(c->ev_built);
   cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->zkey);
   for (int i = 0; i < Context::N_IN; ++i) {
     cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
@@ -236,13 +250,16 @@ RadiusParams make_radius(const Context* c, const wr_camera* cam, int H, float r_
 // Src yields the splat centres of elements [0, P) (build_kernels.cuh), Gather the sphere and
 // colour of a splat id (lbvh.cuh).
 template <class Src, class Gather>
-int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
-  const int parity = (int)(c->frame & 1u);
-  FrameState* st = c->state + parity;
-  FrameState* st_next = c->state + (parity ^ 1);
+int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool async = false) {
+  // build f goes to BVH set f & 1 and frame state f % 3 and re-arms state (f + 1) % 3; both were
+  // last used by build f - 2 whose renders are complete (stream order, or the begin/commit protocol)
+  const int tset = (int)(c->frame & 1u), tstate = (int)(c->frame % 3u);
+  FrameState* st = c->state + tstate;
+  FrameState* st_next = c->state + (tstate + 1) % 3;
+  const Context::BvhSet& bs = c->set[tset];
   const int tiles = P > 0 ? (int)((P + TILE_PX - 1) / TILE_PX) : 1;
-  cudaStream_t s = c->stream;
-  const bool prof = c->profiling;
+  cudaStream_t s = async ? c->build_stream : c->stream;
+  const bool prof = c->profiling && !async;   // per-stage events live on the caller's stream
 
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
@@ -281,24 +298,31 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P) {
   const int lgrid_max = P > 0 ? (int)((P + LBVH_THREADS - 1) / LBVH_THREADS) : 1;
   const int lgrid = lgrid_max < c->num_sms * 8 ? lgrid_max : c->num_sms * 8;
   if (c->refit_mode == SPLATS_REFIT_ATOMIC) {
-    emit_kernel<Gather><<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], gather, st, c->sphere, c->rgba, c->nodes,
+    emit_kernel<Gather><<<lgrid, LBVH_THREADS, 0, s>>>(c->key[0], c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, bs.nodes,
                                                        c->leaf_parent);
     if (prof) m[4] = c->mark();
-    refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(c->sphere, c->leaf_parent, c->nodes, st);
+    refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(bs.sphere, c->leaf_parent, bs.nodes, st);
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
-    launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, c->sphere, c->rgba, c->pyr);
+    launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
     if (prof) m[4] = c->mark();
-    launch(pdl, emit_boxes_kernel, lgrid, LBVH_THREADS, 0, s, c->key[0], c->sphere, c->pyr, st, c->nodes);
+    launch(pdl, emit_boxes_kernel, lgrid, LBVH_THREADS, 0, s, c->key[0], bs.sphere, c->pyr, st, bs.nodes);
   }
   if (prof) m[5] = c->mark();
   c->launches += 4 + sort_launches;
   if (prof)
     for (int i = 0; i < 5; ++i) c->spans.push_back({i, m[i], m[i + 1]});
   CU(cudaGetLastError());
-  c->parity = parity;
   c->frame += 1;
-  c->has_bvh = true;
+  if (async) {
+    c->pending = true;
+    c->pending_set = tset;
+    c->pending_state = tstate;
+  } else {
+    c->cur_set = tset;
+    c->cur_state = tstate;
+    c->has_bvh = true;
+  }
   return SPLATS_OK;
 }
 
@@ -317,11 +341,11 @@ int do_update_frame(Context* c, const float* color, const float* depth, const wr
 int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false, bool rgba8 = false) {
   RenderParams prm;
   prm.cam = make_camera(cam, W2, H2);
-  prm.nodes = c->nodes;
-  prm.sphere = c->sphere;
-  prm.rgba = c->rgba;
-  prm.ids = c->val[0];
-  prm.st = c->state + c->parity;
+  prm.nodes = c->set[c->cur_set].nodes;
+  prm.sphere = c->set[c->cur_set].sphere;
+  prm.rgba = c->set[c->cur_set].rgba;
+  prm.ids = c->set[c->cur_set].ids;
+  prm.st = c->state + c->cur_state;
   prm.out = reinterpret_cast<float4*>(out);
   prm.out8 = reinterpret_cast<uint32_t*>(out);
   const int tiles = ((W2 + 7) / 8) * ((H2 + 3) / 4);
@@ -394,7 +418,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   cudaError_t e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
   const size_t cap = (size_t)c->cap;
   const size_t max_sort_tiles = (cap + SORT_MIN_TILE - 1) / SORT_MIN_TILE;
-  if (e == cudaSuccess) e = dmalloc(&c->state, 2);
+  if (e == cudaSuccess) e = dmalloc(&c->state, 3);
   if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
   if (e == cudaSuccess) e = dmalloc(&c->sched, 2 * Context::MAX_OVERLAP);
   if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * Context::MAX_OVERLAP * sizeof(unsigned));
@@ -403,9 +427,12 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
   }
   if (e == cudaSuccess) e = dmalloc(&c->status, max_sort_tiles * RADIX);
-  if (e == cudaSuccess) e = dmalloc(&c->sphere, cap);
-  if (e == cudaSuccess) e = dmalloc(&c->rgba, cap);
-  if (e == cudaSuccess) e = dmalloc(&c->nodes, cap);
+  for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+    e = dmalloc(&c->set[i].sphere, cap);
+    if (e == cudaSuccess) e = dmalloc(&c->set[i].rgba, cap);
+    if (e == cudaSuccess) e = dmalloc(&c->set[i].ids, cap);
+    if (e == cudaSuccess) e = dmalloc(&c->set[i].nodes, cap);
+  }
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
   if (e == cudaSuccess) e = dmalloc(&c->zkey, cap);
   if (e == cudaSuccess) e = cudaMemset(c->zkey, 0xff, cap * sizeof(uint64_t));
@@ -424,7 +451,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     FrameState init;
     memset(&init, 0, sizeof(init));
     for (int a = 0; a < 3; ++a) init.lo[a] = 0xffffffffu;
-    for (int i = 0; i < 2 && e == cudaSuccess; ++i)
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i)
       e = cudaMemcpy(c->state + i, &init, sizeof(init), cudaMemcpyHostToDevice);
   }
   if (e == cudaSuccess) {
@@ -487,10 +514,10 @@ int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_
   if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_render_points before any update");
   PointParams p;
   p.cam = make_camera(dst_camera, W2, H2);
-  p.sphere = c->sphere;
-  p.rgba = c->rgba;
-  p.ids = c->val[0];
-  p.st = c->state + c->parity;
+  p.sphere = c->set[c->cur_set].sphere;
+  p.rgba = c->set[c->cur_set].rgba;
+  p.ids = c->set[c->cur_set].ids;
+  p.st = c->state + c->cur_state;
   p.zkey = c->zkey;
   p.out = reinterpret_cast<float4*>(out_rgba);
   p.point_px = point_px;
@@ -703,7 +730,7 @@ int splats_count(unsigned* n_host) {
   if (!n_host) return fail(SPLATS_EINVAL, "null pointer argument");
   Context* c = g_ctx;
   if (!c->has_bvh) { *n_host = 0; return SPLATS_OK; }
-  CU(cudaMemcpyAsync(n_host, &c->state[c->parity].n, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaMemcpyAsync(n_host, &c->state[c->cur_state].n, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
   return SPLATS_OK;
 }
@@ -717,11 +744,11 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   if (rc) return rc;
   if (n == 0) return SPLATS_OK;
   if (keys) CU(cudaMemcpyAsync(keys, c->key[0], (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream));
-  if (perm) CU(cudaMemcpyAsync(perm, c->val[0], (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
+  if (perm) CU(cudaMemcpyAsync(perm, c->set[c->cur_set].ids, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
   if (children || parents || node_aabbs) {
     if (parents) CU(cudaMemsetAsync(parents, 0xff, (size_t)(2 * n - 1) * sizeof(int), c->stream));
     const int grid = (int)((n + LBVH_THREADS - 1) / LBVH_THREADS);
-    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->nodes, c->sphere, c->state + c->parity, children, parents,
+    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->set[c->cur_set].nodes, c->set[c->cur_set].sphere, c->state + c->cur_state, children, parents,
                                                         node_aabbs);
     c->launches += 1;
     CU(cudaGetLastError());
@@ -737,11 +764,11 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi) {
   unsigned n = 0;
   int rc = splats_count(&n);
   if (rc) return rc;
-  if (sphere && n) CU(cudaMemcpyAsync(sphere, c->sphere, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
-  if (rgba && n) CU(cudaMemcpyAsync(rgba, c->rgba, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  if (sphere && n) CU(cudaMemcpyAsync(sphere, c->set[c->cur_set].sphere, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  if (rgba && n) CU(cudaMemcpyAsync(rgba, c->set[c->cur_set].rgba, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
   if (lo_hi) {
     FrameState hs;
-    CU(cudaMemcpyAsync(&hs, c->state + c->parity, sizeof(uint32_t) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(&hs, c->state + c->cur_state, sizeof(uint32_t) * 8, cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     float h[6];
     for (int a = 0; a < 3; ++a) {
