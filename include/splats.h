@@ -72,6 +72,23 @@ int splats_create(void* cuda_stream, int max_W, int max_H);
 int splats_update(const float* color, const float* depth, const wr_camera* src_camera,
                   int W, int H, float r_scale);
 
+/* Decoupled build.  The paper's client keeps displaying warped frames while the next server frame
+ * is on its way ("decoupled the rendering and display phases"; requests are "handled
+ * in threads separate from the main rendering thread").  splats_update_begin is
+ * splats_update on a stream of the library: the build starts after everything enqueued so far
+ * on the caller's stream, writes a second BVH, and does not hold up what the caller enqueues
+ * next -- splats_render* keep reading the current BVH and may run at the same time.
+ * splats_update_commit makes the new BVH the current one: everything enqueued afterwards waits
+ * for the build.  Results are those of splats_update.  Between begin and commit: the input
+ * buffers must stay valid and unchanged; splats_update*, a second begin and splats_export fail
+ * with SPLATS_ESTATE.  Arguments and other errors as splats_update.  (Measured on B200: the build
+ * does not get faster or slower this way and a step of the benchmark takes the same time, because
+ * the persistent render blocks leave no room for the sort's 128-register blocks on an SM; what
+ * the pair buys is that the renders of the current BVH are not delayed by an arriving frame.) */
+int splats_update_begin(const float* color, const float* depth, const wr_camera* src_camera,
+                        int W, int H, float r_scale);
+int splats_update_commit(void);
+
 /* Display frame ("the current pixel buffer is warped according to the new
  * transformation"; ray trace the spheres): one primary ray per destination
  * pixel through the BVH of the latest splats_update, every sphere entry hit ordered by

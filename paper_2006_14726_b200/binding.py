@@ -61,6 +61,7 @@ def lib() -> ctypes.CDLL:
         cam_p = ctypes.POINTER(wr_camera)
         L.splats_create.argtypes = [_vp, _ci, _ci]
         L.splats_update.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
+        L.splats_update_begin.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_first_hit.argtypes = [cam_p, _ci, _ci, _vp]
         L.splats_render_rgba8.argtypes = [cam_p, _ci, _ci, _vp]
@@ -129,6 +130,16 @@ def splats_update(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, 
     c = _cam(src_camera)
     _check(lib().splats_update(_dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H),
                                ctypes.byref(c), int(W), int(H), float(r_scale)))
+
+
+def splats_update_begin(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, H: int, r_scale: float) -> None:
+    c = _cam(src_camera)
+    _check(lib().splats_update_begin(_dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H),
+                                     ctypes.byref(c), int(W), int(H), float(r_scale)))
+
+
+def splats_update_commit() -> None:
+    _check(lib().splats_update_commit())
 
 
 def splats_render(dst_camera, W2: int, H2: int, out_rgba: torch.Tensor) -> None:

@@ -35,6 +35,7 @@ struct Context {
   // device memory
   FrameState* state = nullptr;      // [3]: frame f uses state[f % 3] and re-arms state[(f + 1) % 3]
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
+  uint32_t* pack_tile_count = nullptr;  // the same for splats_pack, which may run while a build is in flight
   unsigned* sched = nullptr;        // render tile ticket + done counter, one pair per render in flight
   // renders launched since the last fully serialising launch on the stream (see do_render)
   static constexpr int MAX_OVERLAP = 8;
@@ -173,7 +174,7 @@ cudaError_t dmalloc(T** p, size_t count) {
 }
 
 void free_all(Context* c) {
-  cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->sched);
+  cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->pack_tile_count); cudaFree(c->sched);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status);
   for (int i = 0; i < 2; ++i) { cudaFree(c->set[i].sphere); cudaFree(c->set[i].rgba); cudaFree(c->set[i].ids); cudaFree(c->set[i].nodes); }
@@ -251,6 +252,7 @@ RadiusParams make_radius(const Context* c, const wr_camera* cam, int H, float r_
 // colour of a splat id (lbvh.cuh).
 template <class Src, class Gather>
 int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool async = false) {
+  if (c->pending) return fail(SPLATS_ESTATE, "a build started by splats_update_begin is pending: call splats_update_commit first");
   // build f goes to BVH set f & 1 and frame state f % 3 and re-arms state (f + 1) % 3; both were
   // last used by build f - 2 whose renders are complete (stream order, or the begin/commit protocol)
   const int tset = (int)(c->frame & 1u), tstate = (int)(c->frame % 3u);
@@ -326,7 +328,8 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   return SPLATS_OK;
 }
 
-int do_update_frame(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale) {
+int do_update_frame(Context* c, const float* color, const float* depth, const wr_camera* cam, int W, int H, float r_scale,
+                    bool async = false) {
   FrameSource src;
   src.depth = depth;
   src.cam = make_camera(cam, W, H);
@@ -335,7 +338,7 @@ int do_update_frame(Context* c, const float* color, const float* depth, const wr
   g.color = reinterpret_cast<const float4*>(color);
   g.cam = src.cam;
   g.rp = make_radius(c, cam, H, r_scale);
-  return do_update(c, src, g, (int64_t)W * H);
+  return do_update(c, src, g, (int64_t)W * H, async);
 }
 
 int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false, bool rgba8 = false) {
@@ -420,6 +423,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   const size_t max_sort_tiles = (cap + SORT_MIN_TILE - 1) / SORT_MIN_TILE;
   if (e == cudaSuccess) e = dmalloc(&c->state, 3);
   if (e == cudaSuccess) e = dmalloc(&c->tile_count, cap / TILE_PX + 2);
+  if (e == cudaSuccess) e = dmalloc(&c->pack_tile_count, cap / TILE_PX + 2);
   if (e == cudaSuccess) e = dmalloc(&c->sched, 2 * Context::MAX_OVERLAP);
   if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * Context::MAX_OVERLAP * sizeof(unsigned));
   for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
@@ -487,6 +491,49 @@ int splats_update(const float* color, const float* depth, const wr_camera* src_c
   if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
     return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
   return do_update_frame(g_ctx, color, depth, src_camera, W, H, r_scale);
+}
+
+// Start of a decoupled build: everything enqueued so far on the caller's stream happens before
+// it, nothing enqueued later waits for it until splats_update_commit.
+int begin_build(Context* c) {
+  if (c->pending) return fail(SPLATS_ESTATE, "a build started by splats_update_begin is already pending");
+  if (!c->build_stream) {
+    int lo = 0, hi = 0;
+    CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // hi = numerically lowest = highest priority
+    CU(cudaStreamCreateWithPriority(&c->build_stream, cudaStreamNonBlocking, hi));
+    CU(cudaEventCreateWithFlags(&c->ev_begin, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->ev_built, cudaEventDisableTiming));
+  }
+  CU(cudaEventRecord(c->ev_begin, c->stream));
+  CU(cudaStreamWaitEvent(c->build_stream, c->ev_begin, 0));
+  return SPLATS_OK;
+}
+
+int splats_update_begin(const float* color, const float* depth, const wr_camera* src_camera, int W, int H, float r_scale) {
+  int rc = check_frame_args(g_ctx, color, depth, src_camera, W, H);
+  if (rc) return rc;
+  if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
+  if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
+    return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
+  rc = begin_build(g_ctx);
+  if (rc) return rc;
+  rc = do_update_frame(g_ctx, color, depth, src_camera, W, H, r_scale, true);
+  if (rc) return rc;
+  CU(cudaEventRecord(g_ctx->ev_built, g_ctx->build_stream));
+  return SPLATS_OK;
+}
+
+int splats_update_commit(void) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context: call splats_create first");
+  Context* c = g_ctx;
+  if (!c->pending) return fail(SPLATS_ESTATE, "splats_update_commit without splats_update_begin");
+  CU(cudaStreamWaitEvent(c->stream, c->ev_built, 0));
+  c->cur_set = c->pending_set;
+  c->cur_state = c->pending_state;
+  c->pending = false;
+  c->has_bvh = true;
+  c->render_streak = 0;
+  return SPLATS_OK;
 }
 
 int splats_render(const wr_camera* dst_camera, int W2, int H2, float* out_rgba) {
@@ -601,9 +648,9 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
   c->render_streak = 0;
-  pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count);
+  pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, c->stream>>>(a, c->pack_tile_count);
   const int grid2 = a.num_tiles < c->num_sms * 4 ? a.num_tiles : c->num_sms * 4;
-  pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
+  pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->pack_tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
   if (c->profiling) c->spans.push_back({6, m0, c->mark()});
   c->launches += 2;
   CU(cudaGetLastError());
@@ -739,6 +786,7 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   Context* c = g_ctx;
   if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export before any update");
+  if (c->pending) return fail(SPLATS_ESTATE, "splats_export while a build is pending (its sorted keys are scratch of the build)");
   unsigned n = 0;
   int rc = splats_count(&n);
   if (rc) return rc;
@@ -854,6 +902,7 @@ unsigned long long splats_launch_count(void) { return g_ctx ? g_ctx->launches : 
 int splats_synchronize(void) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   CU(cudaStreamSynchronize(g_ctx->stream));
+  if (g_ctx->build_stream) CU(cudaStreamSynchronize(g_ctx->build_stream));
   if (g_ctx->h2d_stream) {
     CU(cudaStreamSynchronize(g_ctx->h2d_stream));
     CU(cudaStreamSynchronize(g_ctx->d2h_stream));
@@ -879,6 +928,7 @@ const char* splats_last_error(void) { return g_err.c_str(); }
 void splats_destroy(void) {
   if (!g_ctx) return;
   cudaStreamSynchronize(g_ctx->stream);
+  if (g_ctx->build_stream) cudaStreamSynchronize(g_ctx->build_stream);
   if (g_ctx->h2d_stream) { cudaStreamSynchronize(g_ctx->h2d_stream); cudaStreamSynchronize(g_ctx->d2h_stream); }
   free_all(g_ctx);
   delete g_ctx;

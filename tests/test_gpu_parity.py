@@ -395,3 +395,46 @@ def test_seeded_fuzz_whole_path(seed):
         assert_bvh_bit_exact(scp)
         assert_rgba_close(s.render(dst, W2, H2), oracle.render(scp, dst, W2, H2, "bvh"), "packed")
         sp.splats_set_radius(0, 0.0)
+
+
+def test_decoupled_build_begin_commit():
+    # splats_update_begin / splats_update_commit: the next BVH is built on the library's stream
+    # while renders of the current one run; every image and every BVH equals the sequential result.
+    cfg = synth.make_config(1)
+    frames = [synth.source_frame(cfg, 0) + (cfg.src_cams[0], cfg.W, cfg.H, 1.0)]
+    for b, (W, H, rs) in enumerate(((300, 200, 2.0), (512, 512, 1.0), (64, 64, 1.0))):
+        c, d, cam = synth.random_frame(W, H, seed=60 + b, fill=0.6)
+        frames.append((c, d, cam, W, H, rs))
+    scenes = [oracle.build_scene(c, d, cam, W, H, rs) for (c, d, cam, W, H, rs) in frames]
+    dev = [(torch.from_numpy(c).cuda(), torch.from_numpy(d).cuda()) for (c, d, *_ ) in frames]
+    cams = [synth.orbit_camera(3.0 * i, 2.0 * i) for i in range(4)]
+    with Session(512, 512) as s:
+        sp.splats_set_option(sp.OPT_OVERLAP, 1)
+        with pytest.raises(sp.SplatsError):
+            sp.splats_update_commit()                                   # nothing pending
+        c0, d0, cam0, W0, H0, rs0 = frames[0]
+        sp.splats_update(dev[0][0], dev[0][1], cam0, W0, H0, rs0)
+        outs = []
+        for k in range(len(frames)):
+            nxt = (k + 1) % len(frames)
+            cn, dn, camn, Wn, Hn, rsn = frames[nxt]
+            sp.splats_update_begin(dev[nxt][0], dev[nxt][1], camn, Wn, Hn, rsn)     # builds BVH k+1 ...
+            with pytest.raises(sp.SplatsError):
+                sp.splats_update_begin(dev[nxt][0], dev[nxt][1], camn, Wn, Hn, rsn)
+            with pytest.raises(sp.SplatsError):
+                sp.splats_update(dev[nxt][0], dev[nxt][1], camn, Wn, Hn, rsn)
+            imgs = [torch.full((120, 160, 4), -7.0, dtype=torch.float32, device="cuda") for _ in cams]
+            for cam, img in zip(cams, imgs):                                           # ... while BVH k is rendered
+                sp.splats_render(cam, 160, 120, img)
+            outs.append(imgs)
+            sp.splats_update_commit()
+            if k == 1:
+                torch.cuda.synchronize()
+                assert_bvh_bit_exact(scenes[nxt])                                      # the committed BVH is the new one
+        sp.splats_synchronize()
+        torch.cuda.synchronize()
+        for k, imgs in enumerate(outs):
+            for cam, img in zip(cams, imgs):
+                assert_rgba_close(img.cpu().numpy(), oracle.render(scenes[k], cam, 160, 120, "bvh"), f"step {k}")
+        # after the loop the current BVH is frame 0 again
+        assert_bvh_bit_exact(scenes[0])
