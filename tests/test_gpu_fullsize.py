@@ -64,3 +64,27 @@ def test_config4_full_size():
         s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
         assert_bvh_bit_exact(sc)
         _check_renders(s, sc, cfg.dst_cams, cfg.W, cfg.H, False, 200_000, 192, 40)
+
+
+def test_config3_bench_step_in_bench_launch_configuration():
+    # exactly what bench.py times: SPLATS_OPT_OVERLAP on, one update and its four renders into four
+    # images enqueued back to back, no synchronisation in between; all four frames in full
+    import torch
+    from paper_2006_14726_b200 import binding as sp
+    cfg = synth.make_config(3)
+    build = 14
+    color, depth = synth.source_frame(cfg, build)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[build], cfg.W, cfg.H, cfg.r_scale)
+    with Session(cfg.W, cfg.H):
+        sp.splats_set_option(sp.OPT_OVERLAP, 1)
+        dc, dd = torch.from_numpy(color).cuda(), torch.from_numpy(depth).cuda()
+        outs = [torch.full((cfg.H, cfg.W, 4), -7.0, dtype=torch.float32, device="cuda") for _ in range(4)]
+        for rep in range(2):                      # the second step overwrites the images of the first
+            sp.splats_update(dc, dd, cfg.src_cams[build], cfg.W, cfg.H, cfg.r_scale)
+            for j in range(4):
+                sp.splats_render(cfg.dst_cams[4 * build + j], cfg.W, cfg.H, outs[j])
+        torch.cuda.synchronize()
+        assert_bvh_bit_exact(sc)
+        for j in range(4):
+            ref = oracle.render(sc, cfg.dst_cams[4 * build + j], cfg.W, cfg.H, "bvh")
+            assert_rgba_close(outs[j].cpu().numpy(), ref, f"display frame {4 * build + j}")
