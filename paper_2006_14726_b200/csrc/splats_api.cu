@@ -40,6 +40,7 @@ struct Context {
   // renders launched since the last fully serialising launch on the stream (see do_render)
   static constexpr int MAX_OVERLAP = 8;
   int render_streak = 0;
+  bool serialize_next_render = false;   // set when renders may be in flight that the bookkeeping below no longer knows
   const char* inflight_lo[MAX_OVERLAP] = {};
   const char* inflight_hi[MAX_OVERLAP] = {};
   uint64_t* key[2] = {nullptr, nullptr};
@@ -266,7 +267,7 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
   const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
-  c->render_streak = 0;
+  if (!async) c->render_streak = 0;   // (a decoupled build runs on its own stream: the renders in flight stay tracked)
   // an ordinary launch: everything before it in the stream, overlapping renders included, is complete
   launch(false, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
@@ -368,7 +369,11 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   const char* out_hi = out_lo + (size_t)W2 * H2 * (rgba8 ? 4 : 16);
   bool pdl = c->pdl && !c->profiling;
   int wait_prev = 1;
-  if (!(pdl && c->overlap)) {
+  if (c->serialize_next_render) {   // e.g. after splats_update_commit: earlier renders may still be running
+    pdl = false;
+    c->render_streak = 0;
+    c->serialize_next_render = false;
+  } else if (!(pdl && c->overlap)) {
     c->render_streak = 0;   // every render waits for its predecessor; one pair of ticket counters
   } else if (c->render_streak > 0) {
     bool independent = c->render_streak < Context::MAX_OVERLAP;
@@ -532,7 +537,7 @@ int splats_update_commit(void) {
   c->cur_state = c->pending_state;
   c->pending = false;
   c->has_bvh = true;
-  c->render_streak = 0;
+  c->serialize_next_render = true;   // the renders of the previous BVH may still be in flight
   return SPLATS_OK;
 }
 
@@ -848,7 +853,7 @@ int splats_set_option(int option, int value) {
     case SPLATS_OPT_OVERLAP:
       if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_OVERLAP takes 0 or 1");
       g_ctx->overlap = value != 0;
-      g_ctx->render_streak = 0;
+      g_ctx->serialize_next_render = true;
       return SPLATS_OK;
     case SPLATS_OPT_PDL:
       if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_PDL takes 0 or 1");

@@ -415,6 +415,7 @@ def test_decoupled_build_begin_commit():
         c0, d0, cam0, W0, H0, rs0 = frames[0]
         sp.splats_update(dev[0][0], dev[0][1], cam0, W0, H0, rs0)
         outs = []
+        reuse = torch.full((120, 160, 4), -7.0, dtype=torch.float32, device="cuda")
         for k in range(len(frames)):
             nxt = (k + 1) % len(frames)
             cn, dn, camn, Wn, Hn, rsn = frames[nxt]
@@ -428,6 +429,11 @@ def test_decoupled_build_begin_commit():
                 sp.splats_render(cam, 160, 120, img)
             outs.append(imgs)
             sp.splats_update_commit()
+            # the same image buffer is rendered into from the old BVH (possibly still in flight) and,
+            # right after the commit, from the new one: the second write must win
+            sp.splats_render(cams[0], 160, 120, reuse)
+            if k == 0:
+                first_reuse_scene = nxt
             if k == 1:
                 torch.cuda.synchronize()
                 assert_bvh_bit_exact(scenes[nxt])                                      # the committed BVH is the new one
@@ -438,3 +444,4 @@ def test_decoupled_build_begin_commit():
                 assert_rgba_close(img.cpu().numpy(), oracle.render(scenes[k], cam, 160, 120, "bvh"), f"step {k}")
         # after the loop the current BVH is frame 0 again
         assert_bvh_bit_exact(scenes[0])
+        assert_rgba_close(reuse.cpu().numpy(), oracle.render(scenes[0], cams[0], 160, 120, "bvh"), "reused image")
