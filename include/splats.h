@@ -256,7 +256,8 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *     use the same BVH and write disjoint images do not depend on each other, so up to eight of
  *     them are allowed to execute concurrently: the next render's blocks fill the SMs that the
  *     tail of the previous one leaves idle.  Results are unchanged.  Stream order is kept towards
- *     everything else (updates, other calls of this library, later work of the caller), and a
+ *     everything else (updates, other calls of this library, later work of the caller: a render
+ *     never completes before the render launched before it), and a
  *     render whose image overlaps one that may still be in flight is serialised.  The one thing
  *     given up: work that the CALLER enqueues between two such render calls is not guaranteed to
  *     be complete before the second render starts writing its image (the render reads nothing

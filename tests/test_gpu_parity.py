@@ -330,6 +330,13 @@ def test_overlapping_renders_option():
         outs = [torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda") for _ in range(11)]
         for i, cam in enumerate(cams):
             sp.splats_render(cam, W, H, outs[i])
+        # stream-ordered copies of EARLIER images right behind the last render, no device-wide
+        # synchronisation: completion must be in launch order for them to see finished images
+        early = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(3)]
+        for i in range(3):
+            early[i].copy_(outs[7 + i], non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        early = [e.clone() for e in early]
         shared = torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda")
         sp.splats_render(cams[0], W, H, shared)
         sp.splats_render(cams[5], W, H, shared)             # same image twice: the second one must win
@@ -348,6 +355,8 @@ def test_overlapping_renders_option():
         torch.cuda.synchronize()
         for i in (0, 3, 4, 7, 10):
             assert_rgba_close(outs[i].cpu().numpy(), oracle.render(sc, cams[i], W, H, "bvh"), f"render {i}")
+        for i in range(3):
+            assert torch.equal(early[i], outs[7 + i].cpu()), f"stream-ordered copy of render {7 + i} saw an unfinished image"
         ref5 = oracle.render(sc, cams[5], W, H, "bvh")
         assert_rgba_close(shared.cpu().numpy(), ref5, "aliased image")
         assert np.array_equal(fh.cpu().numpy(), oracle.render(sc, cams[3], W, H, "bvh", first_hit=True))
