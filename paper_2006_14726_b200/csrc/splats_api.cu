@@ -271,7 +271,7 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   // an ordinary launch: everything before it in the stream, overlapping renders included, is complete
   launch(false, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
-  const int grid2 = tiles < c->num_sms * 4 ? tiles : c->num_sms * 4;
+  const int grid2 = tiles < c->num_sms * 8 ? tiles : c->num_sms * 8;
   launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
          c->val[0], c->key[1], c->val[1], c->sort_mode);
   if (prof) m[2] = c->mark();
