@@ -3,8 +3,8 @@
 // using ray tracing"; "spheres that are represented as real quadrics",
 // PAPER.md:55; CUDA software ray tracing without RT cores).
 //
-// One thread per destination pixel, one warp per 8x4 pixel tile, four warps (16x8 pixels)
-// per block.  Traversal keeps the K nearest hits beyond a cursor (t, id) in a register
+// One thread per destination pixel, one warp per 8x4 pixel tile, one warp per block (32 resident
+// blocks per SM; four consecutive tickets are the four tiles of a 16x8 supertile).  Traversal keeps the K nearest hits beyond a cursor (t, id) in a register
 // k-buffer sorted by (t, id); after the walk they are composited in order, and if the ray is
 // not yet opaque (alpha < 0.99) and the k-buffer was full (hits may have been dropped), the ray is
 // re-launched from the last composited (t, id).  The result is exactly "sort all hits by
@@ -17,7 +17,7 @@
 
 namespace sw {
 
-constexpr int RENDER_THREADS = 128;
+constexpr int RENDER_THREADS = 32;   // one warp = one 8x4 tile per block: the finest unit for filling another render's tail
 #ifndef SPLATS_KBUF
 #define SPLATS_KBUF 4
 #endif
@@ -148,7 +148,7 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 // OUT8 = true writes the pixel as RGBA8 (round(255 c), the colour format of the wire, S10) instead
 // of four float32: a quarter of the bytes for a client that only displays the image.
 template <int KBUF, bool FIRST, bool OUT8 = false>
-__global__ void __launch_bounds__(RENDER_THREADS, 8)
+__global__ void __launch_bounds__(RENDER_THREADS, 1024 / RENDER_THREADS)
 render_kernel(RenderParams prm) {
   if (prm.wait_prev) pdl_wait();
   pdl_trigger();
