@@ -111,6 +111,10 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int shift = 8 * pass;
   const uint64_t ep = (uint64_t)epoch << 32;
+  const bool single_wave = num_tiles <= (int)gridDim.x;   // every tile has its own resident block
+  int gs_log = 3;
+  while ((1 << (2 * gs_log)) < num_tiles) ++gs_log;
+  uint64_t* gstatus = status + (size_t)num_tiles * RADIX;   // group totals live behind the tiles' words
 
   {  // bin bases of this digit: exclusive scan of the global histogram
     uint32_t h = __ldcg(&st->hist[pass][tid]);
@@ -165,7 +169,7 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
     }
     // ---- publish the aggregate, then scan the tile's counts while the status word travels
     uint64_t* my = status + (size_t)tile * RADIX + tid;
-    if (tile != 0) st_volatile_u64(my, ep | FLAG_AGG | count);
+    if (tile != 0 || single_wave) st_volatile_u64(my, ep | FLAG_AGG | count);
     const uint32_t toff = block_excl_scan_256(count, s.scan_tmp, nullptr);
     s.tile_off[tid] = toff;
     __syncthreads();
@@ -182,8 +186,53 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
       }
     }
 
-    // ---- decoupled look-back for bin `tid`
     uint32_t excl;
+    if (single_wave) {
+      // ---- one wave of tiles: every tile publishes its aggregate at about the same time, and a
+      // chained walk would be ~tiles / 16 dependent L2 round trips.  Two-level sum instead: tiles
+      // form groups of 2^gs_log (about sqrt(tiles)); the last tile of a group publishes the
+      // group total as soon as it has read its group's aggregates; a tile adds the totals of the
+      // earlier groups and the aggregates of the earlier tiles of its own group: three round
+      // trips however many tiles there are.
+      excl = s.digit_base[tid];
+      const int g = tile >> gs_log, first = g << gs_log;
+      uint32_t within = 0;
+      for (int base = first; base < tile; base += LOOKBACK) {
+        uint64_t w[LOOKBACK];
+        bool ok;
+        do {
+          ok = true;
+#pragma unroll
+          for (int k = 0; k < LOOKBACK; ++k)
+            w[k] = base + k < tile ? ld_volatile_u64(status + (size_t)(base + k) * RADIX + tid) : (ep | FLAG_AGG);
+#pragma unroll
+          for (int k = 0; k < LOOKBACK; ++k)
+            if ((w[k] >> 32) != epoch || (w[k] & (FLAG_AGG | FLAG_INC)) == 0) ok = false;
+        } while (!ok);
+#pragma unroll
+        for (int k = 0; k < LOOKBACK; ++k) within += (uint32_t)w[k] & VALUE_MASK;
+      }
+      if (tile == first + (1 << gs_log) - 1)
+        st_volatile_u64(gstatus + (size_t)g * RADIX + tid, ep | FLAG_AGG | (within + count));
+      excl += within;
+      for (int base = 0; base < g; base += LOOKBACK) {
+        uint64_t w[LOOKBACK];
+        bool ok;
+        do {
+          ok = true;
+#pragma unroll
+          for (int k = 0; k < LOOKBACK; ++k)
+            w[k] = base + k < g ? ld_volatile_u64(gstatus + (size_t)(base + k) * RADIX + tid) : (ep | FLAG_AGG);
+#pragma unroll
+          for (int k = 0; k < LOOKBACK; ++k)
+            if ((w[k] >> 32) != epoch || (w[k] & FLAG_AGG) == 0) ok = false;
+        } while (!ok);
+#pragma unroll
+        for (int k = 0; k < LOOKBACK; ++k) excl += (uint32_t)w[k] & VALUE_MASK;
+      }
+    } else
+    {
+    // ---- decoupled look-back for bin `tid`
     if (tile == 0) {
       excl = s.digit_base[tid];
     } else {
@@ -215,7 +264,8 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
         t -= used;
       }
     }
-    st_volatile_u64(my, ep | FLAG_INC | (excl + count));
+    }
+    if (!single_wave) st_volatile_u64(my, ep | FLAG_INC | (excl + count));
     s.bin_base[tid] = (int64_t)excl - (int64_t)toff;
     __syncthreads();
 

@@ -435,7 +435,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     e = dmalloc(&c->key[i], cap);
     if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
   }
-  if (e == cudaSuccess) e = dmalloc(&c->status, max_sort_tiles * RADIX);
+  const size_t status_rows = max_sort_tiles + max_sort_tiles / 8 + 4;   // tile words + group totals (onesweep.cuh)
+  if (e == cudaSuccess) e = dmalloc(&c->status, status_rows * RADIX);
   for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
     e = dmalloc(&c->set[i].sphere, cap);
     if (e == cudaSuccess) e = dmalloc(&c->set[i].rgba, cap);
@@ -455,7 +456,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     if (e == cudaSuccess) e = dmalloc(&c->pyr, 2 * off);
     if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_pyr, &c->pyr_layout, sizeof(PyramidLayout));
   }
-  if (e == cudaSuccess) e = cudaMemset(c->status, 0, max_sort_tiles * RADIX * sizeof(uint64_t));
+  if (e == cudaSuccess) e = cudaMemset(c->status, 0, status_rows * RADIX * sizeof(uint64_t));
   if (e == cudaSuccess) {
     FrameState init;
     memset(&init, 0, sizeof(init));
