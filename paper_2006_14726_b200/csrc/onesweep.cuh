@@ -8,8 +8,9 @@
 // blocks are resident and every block walks its tiles in ascending order, the lowest
 // unfinished tile can always make progress: no deadlock, no atomic ticket.  The look-back
 // status words carry an epoch (unique per pass and frame) so the status array never needs
-// clearing.  The digit histograms (hence the bin bases) come from unproject_kernel, which had
-// the keys in registers anyway.
+// clearing.  When every tile has its own resident block (one wave) the chain is replaced by a
+// two-level sum (tile aggregates + group totals), see onesweep_pass.  The digit histograms (hence
+// the bin bases) come from unproject_kernel, which had the keys in registers anyway.
 //
 // One launch runs several passes, separated by a grid barrier (the grid is co-resident
 // anyway), in one of three modes:
