@@ -44,8 +44,13 @@ FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
 # DRAM bytes per launch from the `ncu --set full` captures summarised under profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum); None until a capture exists for that kernel.
 NCU_TRAFFIC_BYTES = {
-    "render": 21.5e6,   # profiles/r01b_ncu_full_summary.txt (source frame 10, cold L2: BVH + splats read once)
-    "sort": 2.9e6,      # the 5 MB working set stays in L2 between the passes
+    # profiles/r01c_ncu_full_summary.txt and r01e_ncu_render_summary.txt, source frame 10 (N = 297 k), cold L2
+    "bounds": 8.32e6,
+    "unproject_morton_compact": 4.23e6,
+    "sort": 2.73e6,        # the keys and values stay in L2 between the passes
+    "tree_1": 5.39e6,
+    "tree_2": 12.2e6,
+    "render": 21.7e6,      # BVH + splats read once; the image stays in L2 under ncu's cache control
 }
 
 
@@ -366,7 +371,8 @@ def run_ours(args):
         gbs = bytes_sum[name] / (ms_sum * 1e-3) / 1e9 if ms_sum > 0 else 0.0
         kernels.append({"stage": name, "launches_per_call": 1, "calls": calls,
                         "ms_avg": ms_sum / calls, "share": ms_sum / ms_staged, "algorithmic_bytes_avg": bytes_sum[name] / calls,
-                        "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak})
+                        "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak,
+                        "traffic_ncu": NCU_TRAFFIC_BYTES.get(name)})
     dominant = max(kernels, key=lambda r: r["share"])
     build = [r for r in kernels if r["stage"] != "render"]
     build_ms = sum(r["ms_avg"] for r in build)
