@@ -15,13 +15,16 @@
  *   - "dev" pointers are CUDA device pointers on the device that was current at
  *     splats_create; "host" pointers are ordinary host memory (pinned memory makes the
  *     *_host copies asynchronous).  The caller owns every buffer it passes in; the library
- *     owns splats, keys, BVH and scratch, all allocated once in splats_create.
+ *     owns splats, keys, two BVH sets and scratch, all allocated once in splats_create (about
+ *     275 bytes per capacity pixel; the staging of the *_host calls, 88 bytes per pixel, and the
+ *     stream of splats_update_begin are created on first use).
  *   - splats_update / splats_render only ENQUEUE work on the stream given to splats_create and
  *     return; input/output buffers must stay valid until that work has run.  No allocation
  *     and no host<->device synchronisation happens on those two calls.
  *   - Return value: 0 = ok, SPLATS_EINVAL (-1) invalid argument, SPLATS_ENOBVH (-2) render
  *     before any update, SPLATS_ECUDA (-3) CUDA error, SPLATS_ESTATE (-4) no context /
- *     context already exists.  splats_last_error() gives the text.  Nothing aborts or throws.
+ *     context already exists / call not allowed while a splats_update_begin is pending.
+ *     splats_last_error() gives the text.  Nothing aborts or throws.
  *   - There is no CPU fallback: without a CUDA device splats_create fails with SPLATS_ECUDA.
  */
 #ifndef SPLATS_H_
