@@ -268,8 +268,9 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   if (prof) m[0] = c->mark();
   const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
   if (!async) c->render_streak = 0;   // (a decoupled build runs on its own stream: the renders in flight stay tracked)
-  // an ordinary launch: everything before it in the stream, overlapping renders included, is complete
-  launch(false, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
+  // bounds_kernel waits for its predecessor at its first instruction; overlapping renders
+  // complete in launch order (render.cuh), so everything before it in the stream is complete
+  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 8 ? tiles : c->num_sms * 8;
   launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
@@ -362,9 +363,10 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   // predecessor: the next render's blocks fill the SMs that the tail of the previous one leaves
   // idle.  The first render after anything else waits (the BVH must be complete; everything
   // before it in the stream is ordered), every MAX_OVERLAP-th one and any render whose image
-  // overlaps one that may still be in flight is an ordinary launch (full stream order), and so
-  // is the first kernel of whatever follows (bounds_kernel, pack, points, ...).  Each render in
-  // flight has its own pair of ticket counters.
+  // overlaps one that may still be in flight is an ordinary launch (full stream order).  A
+  // render that skips the wait at its start waits at its end (render.cuh), so renders complete
+  // in launch order and whatever follows is ordered after all of them.  Each render in flight
+  // has its own pair of ticket counters.
   const char* out_lo = reinterpret_cast<const char*>(out);
   const char* out_hi = out_lo + (size_t)W2 * H2 * (rgba8 ? 4 : 16);
   bool pdl = c->pdl && !c->profiling;
