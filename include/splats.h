@@ -296,12 +296,14 @@ int splats_set_radius(int mode, float param);
 
 /* Per-stage device times, measured with CUDA events recorded on the library's stream around
  * each stage of every update / render issued while profiling is on.  Off by default (the
- * event records cost about a microsecond each).  splats_stage_ms synchronises the stream,
+ * event records cost about a microsecond each, and while it is on the kernels are launched
+ * one after the other without programmatic dependent launches).  splats_stage_ms synchronises the stream,
  * returns for each stage the SUM of its durations in milliseconds and how many times it ran
  * since profiling was switched on or since the previous query, and clears the record.
- * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all 8 passes), 3 first tree kernel
- * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 second tree
- * kernel (pyramid mode: hierarchy + node boxes; atomic mode: refit), 5 render (either query),
+ * stage order: 0 bounds, 1 unproject+morton+compact, 2 sort (all passes), 3 first tree kernel
+ * (pyramid mode: gather + leaf boxes + pyramid; atomic mode: gather + hierarchy), 4 the rest of
+ * the tree (pyramid mode: hierarchy kernel + node-box kernel, which otherwise runs beside stage
+ * 3; atomic mode: refit), 5 render (either query),
  * 6 splats_pack (both launches), 7 splats_render_points (three launches), 8 splats_march.
  * calls may be NULL. */
 #define SPLATS_NUM_STAGES 9

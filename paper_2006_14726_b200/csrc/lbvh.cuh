@@ -144,8 +144,9 @@ refit_kernel(const float4* __restrict__ sphere, const int* __restrict__ leaf_par
 // per level (a dependent chain as long as the tree is deep), (1) leaf_pyramid_kernel gathers
 // the splats into sorted order and builds a binary min/max pyramid over the leaf boxes --
 // bottom-up, ten levels per block in shared memory, the remaining ones by the last block to
-// finish -- and (2) emit_boxes_kernel emits node i (Karras) and obtains both child boxes by a
-// range query on the pyramid (<= 2 log2(range) independent entry reads, no atomics, no fences).
+// finish --, (2) hierarchy_kernel finds the range and split of every node i (Karras) beside it,
+// and (3) boxes_kernel obtains both child boxes of a node by a range query on the pyramid
+// (<= 2 log2(range) independent entry reads, no atomics, no fences).
 // min/max are exact and associative, so the boxes are bit-identical to a bottom-up refit.
 constexpr int PYR_THREADS = 256;
 constexpr int PYR_LEAVES = 1024;     // leaves per block = 2^PYR_LOCAL
@@ -355,12 +356,71 @@ __device__ __forceinline__ int descend4(const uint64_t* __restrict__ keys, int n
   return base;
 }
 
-// Thread i emits internal node i of the binary radix tree (Karras: direction, range end by
-// galloping + search, split by search) and fills both child boxes from the pyramid; the
-// 64-byte record is written once, with four 16-byte stores.
+// Internal node i of the binary radix tree (Karras: direction, range end by galloping + search,
+// split by search): the sorted leaves it covers, [first, last], and its split gamma (left child
+// covers [first, gamma]).
+__device__ __forceinline__ void karras_node(const uint64_t* __restrict__ keys, int n, int i, int& first, int& gamma,
+                                            int& last) {
+  const uint64_t ki = __ldg(keys + i);
+  const int d = delta(keys, n, i, ki, i + 1) > delta(keys, n, i, ki, i - 1) ? 1 : -1;
+  const int dmin = delta(keys, n, i, ki, i - d);
+  // gallop: the range length l satisfies lb <= l < 2 lb (four probes per round)
+  int lb = 1;
+  while (true) {
+    const int c = (int)(delta(keys, n, i, ki, i + 2 * lb * d) > dmin) + (int)(delta(keys, n, i, ki, i + 4 * lb * d) > dmin) +
+                  (int)(delta(keys, n, i, ki, i + 8 * lb * d) > dmin) + (int)(delta(keys, n, i, ki, i + 16 * lb * d) > dmin);
+    lb <<= c;
+    if (c < 4) break;
+  }
+  const int l = descend4(keys, n, i, ki, d, dmin, lb, lb);
+  const int j = i + l * d;
+  const int dnode = delta(keys, n, i, ki, j);
+  // split: largest s in [0, l) whose key still shares more than dnode bits with key i
+  const int s = descend4(keys, n, i, ki, d, dnode, 0, l > 1 ? 1 << (32 - __clz(l - 1)) : 1);
+  gamma = i + s * d + min(d, 0);
+  first = min(i, j);
+  last = max(i, j);
+}
+
+// The 64-byte record of node i: both child boxes as range queries on the pyramid, child links.
+__device__ __forceinline__ void write_node(const float4* __restrict__ sphere, const float4* __restrict__ pyr, FrameState* st,
+                                           Node* __restrict__ nodes, int i, int first, int gamma, int last) {
+  const int cnt_l = gamma - first + 1, cnt_r = last - gamma;
+  BoxAcc L, R;
+  range_box2(sphere, pyr, (uint32_t)first, (uint32_t)gamma + 1u, (uint32_t)gamma + 1u, (uint32_t)last + 1u, L, R);
+  const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : gamma;
+  const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)gamma + 1u, (uint32_t)cnt_r) : gamma + 1;
+  float4* rec = reinterpret_cast<float4*>(nodes + i);
+  rec[0] = make_float4(L.lo[0], L.lo[1], L.lo[2], L.hi[0]);
+  rec[1] = make_float4(L.hi[1], L.hi[2], R.lo[0], R.lo[1]);
+  rec[2] = make_float4(R.lo[2], R.hi[0], R.hi[1], R.hi[2]);
+  rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
+  if (i == 0) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
+  }
+}
+
+// The hierarchy needs only the sorted keys, the pyramid only the sorted ids: hierarchy_kernel
+// runs beside leaf_pyramid_kernel (it is launched as a programmatic dependent that does not wait
+// for it at the start but at the end, so that the kernel after it is ordered after both), and
+// boxes_kernel then joins the two: ranges + pyramid -> node records.
 __global__ void __launch_bounds__(LBVH_THREADS)
-emit_boxes_kernel(const uint64_t* __restrict__ keys, const float4* __restrict__ sphere,
-                  const float4* __restrict__ pyr, FrameState* st, Node* __restrict__ nodes) {
+hierarchy_kernel(const uint64_t* __restrict__ keys, const FrameState* __restrict__ st, int4* __restrict__ ranges, int wait_at_start) {
+  if (wait_at_start) pdl_wait();
+  pdl_trigger();
+  const int n = (int)st->n;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n - 1; i += gridDim.x * blockDim.x) {
+    int first, gamma, last;
+    karras_node(keys, n, i, first, gamma, last);
+    ranges[i] = make_int4(first, gamma, last, 0);
+  }
+  if (!wait_at_start) pdl_wait();
+}
+
+__global__ void __launch_bounds__(LBVH_THREADS)
+boxes_kernel(const int4* __restrict__ ranges, const float4* __restrict__ sphere, const float4* __restrict__ pyr,
+             FrameState* st, Node* __restrict__ nodes) {
   pdl_wait();
   pdl_trigger();
   const int n = (int)st->n;
@@ -371,38 +431,8 @@ emit_boxes_kernel(const uint64_t* __restrict__ keys, const float4* __restrict__ 
     for (int a = 0; a < 3; ++a) { st->root_lo[a] = lo[a]; st->root_hi[a] = hi[a]; }
   }
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n - 1; i += gridDim.x * blockDim.x) {
-    const uint64_t ki = __ldg(keys + i);
-    const int d = delta(keys, n, i, ki, i + 1) > delta(keys, n, i, ki, i - 1) ? 1 : -1;
-    const int dmin = delta(keys, n, i, ki, i - d);
-    // gallop: the range length l satisfies lb <= l < 2 lb (four probes per round)
-    int lb = 1;
-    while (true) {
-      const int c = (int)(delta(keys, n, i, ki, i + 2 * lb * d) > dmin) + (int)(delta(keys, n, i, ki, i + 4 * lb * d) > dmin) +
-                    (int)(delta(keys, n, i, ki, i + 8 * lb * d) > dmin) + (int)(delta(keys, n, i, ki, i + 16 * lb * d) > dmin);
-      lb <<= c;
-      if (c < 4) break;
-    }
-    const int l = descend4(keys, n, i, ki, d, dmin, lb, lb);
-    const int j = i + l * d;
-    const int dnode = delta(keys, n, i, ki, j);
-    // split: largest s in [0, l) whose key still shares more than dnode bits with key i
-    const int s = descend4(keys, n, i, ki, d, dnode, 0, l > 1 ? 1 << (32 - __clz(l - 1)) : 1);
-    const int gamma = i + s * d + min(d, 0);
-    const int first = min(i, j), last = max(i, j);
-    const int cnt_l = gamma - first + 1, cnt_r = last - gamma;
-    BoxAcc L, R;
-    range_box2(sphere, pyr, (uint32_t)first, (uint32_t)gamma + 1u, (uint32_t)gamma + 1u, (uint32_t)last + 1u, L, R);
-    const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : gamma;
-    const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)gamma + 1u, (uint32_t)cnt_r) : gamma + 1;
-    float4* rec = reinterpret_cast<float4*>(nodes + i);
-    rec[0] = make_float4(L.lo[0], L.lo[1], L.lo[2], L.hi[0]);
-    rec[1] = make_float4(L.hi[1], L.hi[2], R.lo[0], R.lo[1]);
-    rec[2] = make_float4(R.lo[2], R.hi[0], R.hi[1], R.hi[2]);
-    rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
-    if (i == 0) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
-    }
+    const int4 r = __ldg(ranges + i);
+    write_node(sphere, pyr, st, nodes, i, r.x, r.y, r.z);
   }
 }
 

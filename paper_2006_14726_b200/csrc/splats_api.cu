@@ -63,6 +63,7 @@ struct Context {
   uint64_t* zkey = nullptr;         // depth buffer of splats_render_points, all ones between calls
   int* leaf_parent = nullptr;
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
+  int4* ranges = nullptr;           // (first, split, last) of every internal node, hierarchy_kernel -> boxes_kernel
   PyramidLayout pyr_layout;
   int refit_mode = SPLATS_REFIT_PYRAMID;
   int sort_mode = SPLATS_SORT_HYBRID;
@@ -182,7 +183,7 @@ void free_all(Context* c) {
   if (c->build_stream) cudaStreamDestroy(c->build_stream);
   if (c->ev_begin) cudaEventDestroy(c->ev_begin);
   if (c->ev_built) cudaEventDestroy(c->ev_built);
-  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->zkey);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->ranges); cudaFree(c->zkey);
   for (int i = 0; i < Context::N_IN; ++i) {
     cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
     if (c->in_uploaded[i]) cudaEventDestroy(c->in_uploaded[i]);
@@ -310,7 +311,10 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
     launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
     if (prof) m[4] = c->mark();
-    launch(pdl, emit_boxes_kernel, lgrid, LBVH_THREADS, 0, s, c->key[0], bs.sphere, c->pyr, st, bs.nodes);
+    // the hierarchy (keys only) runs beside the pyramid (ids only); boxes_kernel joins them
+    launch(pdl, hierarchy_kernel, lgrid, LBVH_THREADS, 0, s, (const uint64_t*)c->key[0], (const FrameState*)st, c->ranges, pdl ? 0 : 1);
+    launch(pdl, boxes_kernel, lgrid, LBVH_THREADS, 0, s, (const int4*)c->ranges, (const float4*)bs.sphere, (const float4*)c->pyr, st, bs.nodes);
+    c->launches += 1;
   }
   if (prof) m[5] = c->mark();
   c->launches += 4 + sort_launches;
@@ -446,6 +450,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     if (e == cudaSuccess) e = dmalloc(&c->set[i].nodes, cap);
   }
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->ranges, cap);
   if (e == cudaSuccess) e = dmalloc(&c->zkey, cap);
   if (e == cudaSuccess) e = cudaMemset(c->zkey, 0xff, cap * sizeof(uint64_t));
   {  // pyramid levels 1.. : ceil(cap / 2^k) entries each
