@@ -361,13 +361,16 @@ render_kernel(RenderParams prm) {
   __syncthreads();
   if (tid == 0) {
     __threadfence();
-    if (atomicInc(prm.sched + 1, gridDim.x - 1) == gridDim.x - 1) prm.sched[0] = 0u;
+    if (atomicInc(prm.sched + 1, gridDim.x - 1) == gridDim.x - 1) {
+      prm.sched[0] = 0u;
+      // A render that did not wait for its predecessor at the start must not COMPLETE before it:
+      // whatever comes next in the stream (a copy of an earlier image, an event, the next
+      // update) orders itself after the last kernel only, so completion has to stay in launch
+      // order.  One thread of the last block to finish holds the grid open; every other block
+      // exits and frees its slot at once.
+      if (!prm.wait_prev) pdl_wait();
+    }
   }
-  // A render that did not wait for its predecessor at the start must not COMPLETE before it:
-  // whatever comes next in the stream (a copy of an earlier image, an event, the next update)
-  // orders itself after the last kernel only, so completion has to stay in launch order.  The
-  // predecessor started earlier and is all but finished by now.
-  if (!prm.wait_prev) pdl_wait();
 }
 
 }  // namespace sw
