@@ -271,6 +271,7 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 #define SPLATS_OPT_REFIT       0
 #define SPLATS_REFIT_PYRAMID   0
 #define SPLATS_REFIT_ATOMIC    1
+#define SPLATS_REFIT_TILED     2
 #define SPLATS_OPT_SORT        1
 #define SPLATS_SORT_HYBRID         0
 #define SPLATS_SORT_LSD8           1

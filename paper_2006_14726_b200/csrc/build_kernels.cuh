@@ -197,6 +197,7 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
     if (tid == 4) st_next->pyr_done = 0u;
     if (tid == 5) st_next->sort_bar = 0u;
     if (tid == 6) st_next->sort_fallback = 0u;
+    if (tid == 7) st_next->spine_n = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
   }

@@ -145,6 +145,8 @@ struct FrameState {
   float root_hi[3];
   uint32_t sort_bar;       // grid barrier counter of the sort launch (init 0)
   uint32_t sort_fallback;  // set when the hybrid sort has to redo all 8 passes (init 0)
+  uint32_t spine_n;        // nodes queued by tree_tile_kernel for tree_spine_kernel (init 0)
+  uint32_t pad_[3];
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
 

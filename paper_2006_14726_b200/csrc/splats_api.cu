@@ -65,7 +65,7 @@ struct Context {
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
   int4* ranges = nullptr;           // (first, split, last) of every internal node, hierarchy_kernel -> boxes_kernel
   PyramidLayout pyr_layout;
-  int refit_mode = SPLATS_REFIT_PYRAMID;
+  int refit_mode = SPLATS_REFIT_TILED;
   int sort_mode = SPLATS_SORT_HYBRID;
   int radius_mode = SPLATS_RADIUS_FOOTPRINT;
   bool pdl = true;                  // programmatic dependent launches between the hot-path kernels
@@ -307,6 +307,16 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
                                                        c->leaf_parent);
     if (prof) m[4] = c->mark();
     refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(bs.sphere, c->leaf_parent, bs.nodes, st);
+  } else if (c->refit_mode == SPLATS_REFIT_TILED) {
+    // gather + leaf boxes + pyramid + every node whose range lies inside one tile of sorted leaves;
+    // then the few nodes that span tiles (lbvh.cuh)
+    const int tgrid = P > 0 ? (int)((P + TT_LEAVES - 1) / TT_LEAVES) : 1;
+    launch(pdl, tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
+           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.nodes, c->ranges);
+    if (prof) m[4] = c->mark();
+    const int sgrid2 = c->num_sms * 4;
+    launch(pdl, tree_spine_kernel, sgrid2, LBVH_THREADS, 0, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
+           (const float4*)bs.sphere, (const float4*)c->pyr, bs.nodes);
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
     launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
@@ -471,6 +481,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     for (int i = 0; i < 3 && e == cudaSuccess; ++i)
       e = cudaMemcpy(c->state + i, &init, sizeof(init), cudaMemcpyHostToDevice);
   }
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tree_tile_kernel<FrameGather>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tree_tile_kernel<PackedGather>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
   if (e == cudaSuccess) {
     c->sort_smem = sizeof(SortSmem);
     e = cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem);
@@ -850,7 +862,7 @@ int splats_set_option(int option, int value) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   switch (option) {
     case SPLATS_OPT_REFIT:
-      if (value != SPLATS_REFIT_PYRAMID && value != SPLATS_REFIT_ATOMIC) return fail(SPLATS_EINVAL, "unknown refit mode");
+      if (value != SPLATS_REFIT_PYRAMID && value != SPLATS_REFIT_ATOMIC && value != SPLATS_REFIT_TILED) return fail(SPLATS_EINVAL, "unknown refit mode");
       g_ctx->refit_mode = value;
       return SPLATS_OK;
     case SPLATS_OPT_SORT:

@@ -131,7 +131,8 @@ def test_pyramid_block_boundaries(W, H):
 
 
 def test_atomic_refit_mode_gives_the_same_tree():
-    # SPLATS_OPT_REFIT: the classic atomic-counter refit must give the bit-identical BVH
+    # SPLATS_OPT_REFIT: the classic atomic-counter refit and the pyramid + per-node searches must give the
+    # bit-identical BVH (the default is the tiled tree, which every other test exercises)
     cfg = synth.make_config(1)
     color, depth = synth.source_frame(cfg, 0)
     with Session(cfg.W, cfg.H) as s:
@@ -140,6 +141,9 @@ def test_atomic_refit_mode_gives_the_same_tree():
         c2, d2, cam2 = synth.random_frame(127, 65, seed=3, fill=0.4)
         check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
         sp.splats_set_option(sp.OPT_REFIT, sp.REFIT_PYRAMID)
+        check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
+        check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams[:1], mode="bvh")
+        sp.splats_set_option(sp.OPT_REFIT, sp.REFIT_TILED)   # the default
         check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
         with pytest.raises(sp.SplatsError):
             sp.splats_set_option(sp.OPT_REFIT, 7)
