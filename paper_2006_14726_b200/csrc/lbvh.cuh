@@ -436,357 +436,6 @@ boxes_kernel(const int4* __restrict__ ranges, const float4* __restrict__ sphere,
   }
 }
 
-// ===================================================================== tiled tree (default)
-// splats_set_option(SPLATS_OPT_REFIT, SPLATS_REFIT_TILED): a4 and a5 in one pass over the sorted
-// leaves, two launches.
-//
-// The radix tree over the sorted (key, position) pairs is the Cartesian tree of the adjacent
-// common-prefix lengths d[g] = delta(g, g + 1): the internal node that splits between g and g + 1
-// covers the leaves (p, q] where p (q) is the nearest position to the left (right) of g with a
-// smaller d -- inside a node's range every other adjacent delta is larger than the one at its
-// split, and the deltas just outside are smaller.  In Karras' numbering that node is `q` when it
-// is a left child (d[q] > d[p]: the parent splits at q) and `p + 1` when it is a right child.
-//
-// tree_tile_kernel: one block per TT_LEAVES consecutive sorted leaves.  It gathers the splats
-// into sorted order (as leaf_pyramid_kernel), keeps *all* levels of the tile's box pyramid and
-// a min pyramid over the tile's deltas (one byte each: delta + 1 <= 96, 0 = "beyond the array")
-// in shared memory, finds p and q of every split of the tile by a nearest-smaller-value search
-// on the byte pyramid, and -- when both lie inside the tile, which is the case for all but the
-// strict prefix / suffix minima of the tile's deltas (<= 2 x 97 nodes) -- takes both child boxes
-// as range queries on the shared-memory box pyramid and writes the finished 64-byte node record.
-// The other nodes go to a queue with what is known about them.
-// tree_spine_kernel: finishes the queued nodes: missing range ends by galloping + 4-ary search
-// on the sorted keys, boxes by range queries on the global pyramid (levels >= 1, written by the
-// tile kernel; its top levels by the last block to finish).
-// Same tree, same numbering, same boxes as the other two modes, bit for bit.
-constexpr int TT_LOG = 10;
-constexpr int TT_LEAVES = 1 << TT_LOG;
-constexpr int TT_THREADS = 256;
-constexpr int TT_PER = TT_LEAVES / TT_THREADS;
-constexpr int TT_QMAX = 200;   // >= 2 x 97: strict prefix + suffix minima of byte-sized deltas
-static_assert(TT_LOG == PYR_LOCAL, "the tile kernel writes the same global pyramid levels as leaf_pyramid_kernel");
-
-__host__ __device__ __forceinline__ constexpr int tt_off(int k) { return 2 * TT_LEAVES - ((2 * TT_LEAVES) >> k); }
-
-struct TileSmem {
-  float box[6][2 * TT_LEAVES];   // level k (entries of 2^k leaves) at tt_off(k)
-  uint8_t d[2 * TT_LEAVES];      // delta + 1 of the pair (l, l + 1), min pyramid at the same offsets
-  int4 q[TT_QMAX];               // queued nodes: (split, first or -1, last or -1, 0)
-  uint32_t qn, qbase;
-  uint32_t dleft;                // delta + 1 of the pair (base - 1, base); 0 at the start of the array
-  int last;
-};
-
-// first position q in [s, TT_LEAVES) with d[q] < v (level-0 positions), TT_LEAVES if there is none
-__device__ __forceinline__ int nsv_right(const uint8_t* __restrict__ d, int s, uint32_t v) {
-  int i = s, k = 0;
-  while (true) {
-    if ((i << k) >= TT_LEAVES) return TT_LEAVES;
-    if (d[tt_off(k) + i] < v) break;
-    ++i;                                        // everything in [s, i << k) is >= v
-    const int up = min(__ffs(i) - 1, TT_LOG - k);   // the same position seen from a coarser level
-    i >>= up;
-    k += up;
-  }
-  while (k > 0) {
-    --k;
-    i <<= 1;
-    if (d[tt_off(k) + i] >= v) ++i;
-  }
-  return i;
-}
-// last position p in [0, s] with d[p] < v, -1 if there is none
-__device__ __forceinline__ int nsv_left(const uint8_t* __restrict__ d, int s, uint32_t v) {
-  int i = s, k = 0;
-  while (true) {
-    if (i < 0) return -1;
-    if (d[tt_off(k) + i] < v) break;
-    --i;                                        // everything in ((i + 1) << k, s] is >= v
-    if (i < 0) return -1;
-    const int up = min(__ffs(i + 1) - 1, TT_LOG - k);   // trailing ones: blocks that end at the same position
-    i >>= up;
-    k += up;
-  }
-  while (k > 0) {
-    --k;
-    i = 2 * i + 1;
-    if (d[tt_off(k) + i] >= v) --i;
-  }
-  return i;
-}
-
-// box of the tile-local leaves [l, r), l < r, from the shared-memory pyramid
-__device__ __forceinline__ void range_box_tile(const float (*__restrict__ box)[2 * TT_LEAVES], int l, int r, float lo[3], float hi[3]) {
-  const float INF = __int_as_float(0x7f800000);
-#pragma unroll
-  for (int a = 0; a < 3; ++a) { lo[a] = INF; hi[a] = -INF; }
-  int off = 0, width = TT_LEAVES;
-  while (l < r) {
-    if (l & 1) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], box[a][off + l]); hi[a] = fmaxf(hi[a], box[3 + a][off + l]); }
-      ++l;
-    }
-    if (r & 1) {
-      --r;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], box[a][off + r]); hi[a] = fmaxf(hi[a], box[3 + a][off + r]); }
-    }
-    l >>= 1;
-    r >>= 1;
-    off += width;
-    width >>= 1;
-  }
-}
-
-__device__ __forceinline__ void store_node(Node* __restrict__ nodes, int idx, const float llo[3], const float lhi[3],
-                                           const float rlo[3], const float rhi[3], int first, int gamma, int last) {
-  const int cnt_l = gamma - first + 1, cnt_r = last - gamma;
-  const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : gamma;
-  const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)gamma + 1u, (uint32_t)cnt_r) : gamma + 1;
-  float4* rec = reinterpret_cast<float4*>(nodes + idx);
-  rec[0] = make_float4(llo[0], llo[1], llo[2], lhi[0]);
-  rec[1] = make_float4(lhi[1], lhi[2], rlo[0], rlo[1]);
-  rec[2] = make_float4(rlo[2], rhi[0], rhi[1], rhi[2]);
-  rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
-}
-
-struct Box6 { float v[6]; };
-__device__ __forceinline__ Box6 box_merge(const Box6& a, const Box6& b) {
-  Box6 r;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) { r.v[k] = fminf(a.v[k], b.v[k]); r.v[3 + k] = fmaxf(a.v[3 + k], b.v[3 + k]); }
-  return r;
-}
-
-// Levels above TT_LOG of the global pyramid, by the last block of tree_tile_kernel to finish:
-// five levels per round trip (a warp loads 32 consecutive entries and merges them with shuffles).
-__device__ __forceinline__ void pyramid_top(float4* pyr, uint32_t cnt_prev, int k_prev) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  constexpr int NWARPS = TT_THREADS / 32;
-  const float INF = __int_as_float(0x7f800000);
-  while (cnt_prev > 1) {
-    const float4* src = pyr + 2 * (size_t)c_pyr.off[k_prev];
-    const uint32_t chunks = (cnt_prev + 31) >> 5;
-    for (uint32_t c = warp; c < chunks; c += NWARPS) {
-      const uint32_t j = c * 32 + lane;
-      Box6 b;
-      if (j < cnt_prev) {
-        const float4 lo = __ldcg(src + 2 * (size_t)j), hi = __ldcg(src + 2 * (size_t)j + 1);
-        b.v[0] = lo.x; b.v[1] = lo.y; b.v[2] = lo.z; b.v[3] = hi.x; b.v[4] = hi.y; b.v[5] = hi.z;
-      } else {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { b.v[a] = INF; b.v[3 + a] = -INF; }
-      }
-#pragma unroll
-      for (int s = 1; s <= 5; ++s) {
-        Box6 o;
-#pragma unroll
-        for (int a = 0; a < 6; ++a) o.v[a] = __shfl_down_sync(0xffffffffu, b.v[a], 1 << (s - 1));
-        b = box_merge(b, o);
-        const uint32_t cnt = (cnt_prev + (1u << s) - 1) >> s;
-        if ((lane & ((1 << s) - 1)) == 0 && (j >> s) < cnt && k_prev + s <= PYR_MAX_LEVELS) {
-          float4* e = pyr + 2 * ((size_t)c_pyr.off[k_prev + s] + (j >> s));
-          __stcg(e, make_float4(b.v[0], b.v[1], b.v[2], 0.0f));
-          __stcg(e + 1, make_float4(b.v[3], b.v[4], b.v[5], 0.0f));
-        }
-      }
-    }
-    __syncthreads();
-    cnt_prev = (cnt_prev + 31) >> 5;
-    k_prev += 5;
-  }
-}
-
-template <class Gather>
-__global__ void __launch_bounds__(TT_THREADS)
-tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
-                 float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, float4* pyr,
-                 Node* __restrict__ nodes, int4* __restrict__ queue) {
-  pdl_wait();
-  pdl_trigger();
-  extern __shared__ __align__(16) unsigned char tt_smem_raw[];
-  TileSmem& s = *reinterpret_cast<TileSmem*>(tt_smem_raw);
-  const int n = (int)st->n;
-  const int nblocks = (n + TT_LEAVES - 1) / TT_LEAVES;
-  if ((int)blockIdx.x >= nblocks) return;
-  const int tid = threadIdx.x;
-  const int base = blockIdx.x * TT_LEAVES;
-  const float INF = __int_as_float(0x7f800000);
-
-  // ---- deltas of the adjacent pairs (l, l + 1) of the tile, + 1; 0 beyond the array
-  if (tid == 0) {
-    s.qn = 0;
-    uint32_t dl = 0;
-    if (base > 0) {
-      const uint64_t x = __ldg(keys + base - 1) ^ __ldg(keys + base);
-      dl = 1u + (x ? (uint32_t)__clzll((long long)x) : 64u + (uint32_t)__clz((base - 1) ^ base));
-    }
-    s.dleft = dl;
-  }
-  uint32_t id[TT_PER];
-#pragma unroll
-  for (int j = 0; j < TT_PER; ++j) {
-    const int i = base + tid + j * TT_THREADS;
-    id[j] = i < n ? __ldg(perm + i) : 0u;
-  }
-#pragma unroll
-  for (int j = 0; j < TT_PER; ++j) {
-    const int l = tid + j * TT_THREADS, i = base + l;
-    uint32_t dv = 0;
-    if (i + 1 < n) {
-      const uint64_t x = __ldg(keys + i) ^ __ldg(keys + i + 1);
-      dv = 1u + (x ? (uint32_t)__clzll((long long)x) : 64u + (uint32_t)__clz(i ^ (i + 1)));
-    }
-    s.d[l] = (uint8_t)dv;
-  }
-  // ---- gather the splats of the tile into sorted order; leaf boxes -> level 0
-#pragma unroll
-  for (int j = 0; j < TT_PER; ++j) {
-    const int l = tid + j * TT_THREADS, i = base + l;
-    float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
-    if (i < n) {
-      float4 sp, col;
-      src.get(id[j], sp, col);
-      sphere[i] = sp;
-      rgba[i] = col;
-      ids_out[i] = id[j];   // the BVH keeps its own copy: the sort buffers belong to the next build
-      box_of_sphere(sp, lo, hi);
-    }
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { s.box[a][l] = lo[a]; s.box[3 + a][l] = hi[a]; }
-  }
-  if (n == 1 && tid == 0) {   // the single leaf is the root
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { st->root_lo[a] = s.box[a][0]; st->root_hi[a] = s.box[3 + a][0]; }
-  }
-  __syncthreads();
-
-  // ---- levels 1..TT_LOG of both pyramids (all levels stay in shared memory); the box levels
-  // also go to the global pyramid for the queued nodes
-#pragma unroll
-  for (int k = 1; k <= TT_LOG; ++k) {
-    const int cnt = TT_LEAVES >> k, o0 = tt_off(k - 1), o1 = tt_off(k);
-    for (int j = tid; j < cnt; j += TT_THREADS) {
-      float v[6];
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        v[a] = fminf(s.box[a][o0 + 2 * j], s.box[a][o0 + 2 * j + 1]);
-        v[3 + a] = fmaxf(s.box[3 + a][o0 + 2 * j], s.box[3 + a][o0 + 2 * j + 1]);
-      }
-#pragma unroll
-      for (int a = 0; a < 6; ++a) s.box[a][o1 + j] = v[a];
-      s.d[o1 + j] = min(s.d[o0 + 2 * j], s.d[o0 + 2 * j + 1]);
-      if (base + (j << k) < n) {
-        float4* e = pyr + 2 * ((size_t)c_pyr.off[k] + (base >> k) + j);
-        __stcg(e, make_float4(v[0], v[1], v[2], 0.0f));
-        __stcg(e + 1, make_float4(v[3], v[4], v[5], 0.0f));
-      }
-    }
-    __syncthreads();
-  }
-
-  // ---- the nodes whose split lies in this tile
-  const uint32_t dleft = s.dleft;
-#pragma unroll 1
-  for (int j = 0; j < TT_PER; ++j) {
-    const int l = tid + j * TT_THREADS, g = base + l;
-    if (g + 1 >= n) continue;
-    const uint32_t v = s.d[l];
-    const int q = nsv_right(s.d, l + 1, v);
-    int p = l > 0 ? nsv_left(s.d, l - 1, v) : -1;
-    bool open_l = false;
-    if (p < 0) {                       // nothing smaller inside the tile: the pair (base - 1, base)?
-      if (dleft < v) p = -1; else open_l = true;
-    }
-    const bool open_r = q >= TT_LEAVES;
-    if (open_l || open_r) {
-      const uint32_t slot = atomicAdd(&s.qn, 1u);
-      s.q[slot] = make_int4(g, open_l ? -1 : base + p + 1, open_r ? -1 : base + q, 0);
-      continue;
-    }
-    const int first = base + p + 1, last = base + q;
-    const uint32_t dl = p < 0 ? dleft : s.d[p], dr = s.d[q];
-    const int idx = dr > dl ? last : first;
-    float llo[3], lhi[3], rlo[3], rhi[3];
-    range_box_tile(s.box, p + 1, l + 1, llo, lhi);
-    range_box_tile(s.box, l + 1, q + 1, rlo, rhi);
-    store_node(nodes, idx, llo, lhi, rlo, rhi, first, g, last);
-    if (idx == 0) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(llo[a], rlo[a]); st->root_hi[a] = fmaxf(lhi[a], rhi[a]); }
-    }
-  }
-  __syncthreads();
-  const uint32_t qn = s.qn;
-  if (qn) {
-    if (tid == 0) s.qbase = atomicAdd(&st->spine_n, qn);
-    __syncthreads();
-    for (uint32_t e = tid; e < qn; e += TT_THREADS) queue[s.qbase + e] = s.q[e];
-  }
-  if (nblocks == 1) return;
-
-  // ---- the last block to finish builds the levels above TT_LOG
-  __threadfence();
-  if (tid == 0) s.last = atomicAdd(&st->pyr_done, 1u) == (uint32_t)nblocks - 1u;
-  __syncthreads();
-  if (!s.last) return;
-  __threadfence();
-  pyramid_top(pyr, (uint32_t)nblocks, TT_LOG);
-}
-
-// Largest distance x >= x0 (in direction dir from g) with delta(g, g + x dir) >= dref, given that
-// it holds at x0: gallop (x16 per round, four probes) then 4-ary descent.
-__device__ __forceinline__ int spine_extend(const uint64_t* __restrict__ keys, int n, int g, uint64_t kg, int dir, int dref, int x0) {
-  int lb = x0 > 0 ? x0 : 1, base = x0;
-  // invariant: holds at `base`; find a power-of-two step that fails
-  int step = 1;
-  while (step < lb) step <<= 1;
-  while (true) {
-    const int c = (int)(delta(keys, n, g, kg, g + (base + step) * dir) >= dref) + (int)(delta(keys, n, g, kg, g + (base + 2 * step) * dir) >= dref) +
-                  (int)(delta(keys, n, g, kg, g + (base + 4 * step) * dir) >= dref) + (int)(delta(keys, n, g, kg, g + (base + 8 * step) * dir) >= dref);
-    // the predicate is monotone in the distance: c probes hold, the next one fails
-    if (c == 0) break;
-    base += step << (c - 1);
-    if (c < 4) { step <<= (c - 1); break; }
-    step <<= 4;
-  }
-  // holds at base, fails at base + step
-  int width = step;
-  while (width >= 4) {
-    const int qd = width >> 2;
-    const int c = (int)(delta(keys, n, g, kg, g + (base + qd) * dir) >= dref) + (int)(delta(keys, n, g, kg, g + (base + 2 * qd) * dir) >= dref) +
-                  (int)(delta(keys, n, g, kg, g + (base + 3 * qd) * dir) >= dref);
-    base += c * qd;
-    width = qd;
-  }
-  if (width == 2 && delta(keys, n, g, kg, g + (base + 1) * dir) >= dref) base += 1;
-  return base;
-}
-
-__global__ void __launch_bounds__(LBVH_THREADS)
-tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4* __restrict__ queue,
-                  const float4* __restrict__ sphere, const float4* __restrict__ pyr, Node* __restrict__ nodes) {
-  pdl_wait();
-  pdl_trigger();
-  const int n = (int)st->n;
-  const int qn = (int)st->spine_n;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < qn; e += gridDim.x * blockDim.x) {
-    const int4 ent = __ldg(queue + e);
-    const int g = ent.x;
-    const uint64_t kg = __ldg(keys + g);
-    const int dnode = delta(keys, n, g, kg, g + 1);
-    const int tile_lo = g & ~(TT_LEAVES - 1), tile_hi = min(tile_lo + TT_LEAVES - 1, n - 1);
-    // an open end lies beyond the tile: start the search at the tile's edge
-    const int first = ent.y >= 0 ? ent.y : g - spine_extend(keys, n, g, kg, -1, dnode, g - tile_lo);
-    const int last = ent.z >= 0 ? ent.z : g + spine_extend(keys, n, g, kg, +1, dnode, tile_hi - g);
-    const int dl = first > 0 ? delta(keys, n, first - 1, __ldg(keys + first - 1), first) : -1;
-    const int dr = last < n - 1 ? delta(keys, n, last, __ldg(keys + last), last + 1) : -1;
-    const int idx = dr > dl ? last : first;
-    write_node(sphere, pyr, st, nodes, idx, first, g, last);
-  }
-}
-
 // Canonical export for the bit-exact acceptance checks (include/splats.h, splats_export).
 // Parent links are not part of the traversal structure: they are derived here from the
 // child links (parents[] must be pre-filled with -1 by the caller; the root keeps it).

@@ -18,6 +18,7 @@
 #include "pack.cuh"
 #include "points.cuh"
 #include "render.cuh"
+#include "tree_tile.cuh"
 
 namespace {
 
@@ -63,7 +64,9 @@ struct Context {
   uint64_t* zkey = nullptr;         // depth buffer of splats_render_points, all ones between calls
   int* leaf_parent = nullptr;
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
-  int4* ranges = nullptr;           // (first, split, last) of every internal node, hierarchy_kernel -> boxes_kernel
+  int4* ranges = nullptr;           // (first, split, last) of every internal node, hierarchy_kernel -> boxes_kernel; tiled mode: the queue of tree_spine_kernel
+  uint8_t* tile_min = nullptr;      // tiled tree: smallest delta + 1 of every tile of sorted leaves
+  uint16_t* tile_fb = nullptr;      // tiled tree: first / last split below every threshold, per tile
   PyramidLayout pyr_layout;
   int refit_mode = SPLATS_REFIT_TILED;
   int sort_mode = SPLATS_SORT_HYBRID;
@@ -183,7 +186,7 @@ void free_all(Context* c) {
   if (c->build_stream) cudaStreamDestroy(c->build_stream);
   if (c->ev_begin) cudaEventDestroy(c->ev_begin);
   if (c->ev_built) cudaEventDestroy(c->ev_built);
-  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->ranges); cudaFree(c->zkey);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->ranges); cudaFree(c->zkey); cudaFree(c->tile_min); cudaFree(c->tile_fb);
   for (int i = 0; i < Context::N_IN; ++i) {
     cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
     if (c->in_uploaded[i]) cudaEventDestroy(c->in_uploaded[i]);
@@ -312,11 +315,13 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     // then the few nodes that span tiles (lbvh.cuh)
     const int tgrid = P > 0 ? (int)((P + TT_LEAVES - 1) / TT_LEAVES) : 1;
     launch(pdl, tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
-           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.nodes, c->ranges);
+           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.nodes, c->ranges, c->tile_min, c->tile_fb);
     if (prof) m[4] = c->mark();
-    const int sgrid2 = c->num_sms * 4;
-    launch(pdl, tree_spine_kernel, sgrid2, LBVH_THREADS, 0, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
-           (const float4*)bs.sphere, (const float4*)c->pyr, bs.nodes);
+    int nt_log = 0;
+    while ((1 << nt_log) < tgrid) ++nt_log;
+    const int sgrid2 = (tgrid * TT_QMAX + SPINE_THREADS - 1) / SPINE_THREADS;   // enough for a full queue; idle blocks exit at once
+    launch(pdl, tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
+           (const float4*)bs.sphere, (const float4*)c->pyr, bs.nodes, (const uint8_t*)c->tile_min, (const uint16_t*)c->tile_fb, nt_log);
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
     launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
@@ -461,6 +466,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   }
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
   if (e == cudaSuccess) e = dmalloc(&c->ranges, cap);
+  if (e == cudaSuccess) e = dmalloc(&c->tile_min, cap / TT_LEAVES + 2);
+  if (e == cudaSuccess) e = dmalloc(&c->tile_fb, (cap / TT_LEAVES + 2) * 2 * TT_VPAD);
   if (e == cudaSuccess) e = dmalloc(&c->zkey, cap);
   if (e == cudaSuccess) e = cudaMemset(c->zkey, 0xff, cap * sizeof(uint64_t));
   {  // pyramid levels 1.. : ceil(cap / 2^k) entries each
@@ -481,6 +488,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     for (int i = 0; i < 3 && e == cudaSuccess; ++i)
       e = cudaMemcpy(c->state + i, &init, sizeof(init), cudaMemcpyHostToDevice);
   }
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(tree_spine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(tree_tile_kernel<FrameGather>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(tree_tile_kernel<PackedGather>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
   if (e == cudaSuccess) {
