@@ -3,20 +3,26 @@
 
 Workload (N=1): BASELINE.json configs[3] -- 256^3 volume, 1920x1080 source frames, 60 display
 frames with the camera dollying towards the centre, a splat + BVH rebuild every 4th frame.
-One *step* = one pass of the whole hot path over one source frame: 1 splats_update (bounds,
-unproject+Morton+compaction, onesweep sort, gather+box pyramid, hierarchy, node boxes; 6 launches)
-followed by the 4 splats_render calls of the display frames that use that BVH.  Step k uses source frame k mod 15,
-so 15 steps are exactly the scripted 60-frame sequence.  value = display frames / second, timed
-with CUDA events around exactly K steps of the library as a user runs it (programmatic dependent
-launches; the four renders of a step write four images and may overlap, SPLATS_OPT_OVERLAP).  The
-per-kernel table and the roofline come from a second pass over the same K steps with per-stage
-events on the library's stream (which serialises the stages; its rate is value_with_stage_events).
+One *step* = the whole scripted sequence: 15 x (1 splats_update [bounds, unproject+Morton+
+compaction, onesweep sort, tiled tree, spine: 5 launches] + the 4 splats_render calls of the display
+frames that use that BVH) = 15 updates + 60 renders, so every --steps value has the sequence's own
+mix of light and heavy frames.  value = 60 K / t display frames per second, timed with CUDA events
+around exactly K steps of the library as a user runs it (programmatic dependent launches; the four
+renders after an update write four images and may overlap, SPLATS_OPT_OVERLAP).  The per-kernel
+table and the roofline come from a second pass with per-stage events on the library's stream
+(which serialises the stages; its rate is value_with_stage_events).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+Beside the headline (outside its timed region): `dense` -- a fully covered 1920x1080 frame
+(N = P, the upper bound SURVEY.md sec. 8(d) sizes the build bar on); `table1_shape` -- a 1024x1024
+frame with the paper's fill (623,584 of 1,048,576 samples), first-hit query, beside
+the paper's own numbers; the sec. 8(f) calls; the end-to-end variants; the CPU oracle.
 
-N > 1 (torchrun, one rank per GPU): the path does not shard usefully below one frame
-(replicas only), so every rank runs the same sequence on its own GPU
-with no data-path collective ("scaling": "weak"); value = N * frames / max-over-ranks time.
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--only LEG]
+
+N > 1: the path does not shard usefully below one frame (replicas only), so
+every rank runs the same sequence on its own GPU with no data-path collective ("scaling": "weak");
+value = N * frames / max-over-ranks time.  Started plainly (no torchrun) with --gpus N > 1, the
+script starts its own N ranks.
 
 --impl reference: the CPU oracle (oracle/, single thread) on the same metric and config, each
 step a bounded sample of the same work.  This is the only other place oracle/ is executed.
@@ -24,7 +30,9 @@ step a bounded sample of the same work.  This is the only other place oracle/ is
 from __future__ import annotations
 
 import argparse
+import csv
 import json
+import math
 import os
 import statistics
 import sys
@@ -40,18 +48,10 @@ sys.path.insert(0, str(ROOT))
 METRIC = "reprojected frames/s at 1920x1080 (1 BVH rebuild per 4 frames)"
 UNIT = "frames/s"
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
-
-# DRAM bytes per launch from the `ncu --set full` captures summarised under profiles/
-# (dram__bytes_read.sum + dram__bytes_write.sum); None until a capture exists for that kernel.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r01c_ncu_full_summary.txt and r01e_ncu_render_summary.txt, source frame 10 (N = 297 k), cold L2
-    "bounds": 8.32e6,
-    "unproject_morton_compact": 4.23e6,
-    "sort": 2.73e6,        # the keys and values stay in L2 between the passes
-    "tree_1": 5.39e6,
-    "tree_2": 12.2e6,
-    "render": 21.7e6,      # BVH + splats read once; the image stays in L2 under ncu's cache control
-}
+SM_COUNT, ISSUE_PER_SM_CLK = 148, 4          # B200: 148 SMs x 4 warp schedulers, one warp instruction each per clock
+PAPER_TABLE1 = {"gpu": "NVIDIA RTX 2080 (PAPER.md:83)", "viewport": "1024x1024", "samples": 623584,
+                "lbvh_ms": 11.0, "compaction_ms_cpu": 23.0, "fps_first_hit": [229, 408],
+                "cite": "PAPER.md:77-83 Table 1"}
 
 
 def log(*a):
@@ -66,6 +66,105 @@ def hbm_peak():
         except Exception:
             pass
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# --------------------------------------------------------------------------- ncu evidence
+# `ncu -i <capture>.ncu-rep --page raw --csv` of a capture of THIS file's command line, committed
+# under profiles/ (the .md beside each names the command).  Nothing is typed in: a kernel without a
+# row gets null.
+NCU_FILES = {"headline": "r02_ncu_raw_config3.csv", "dense": "r02_ncu_raw_dense.csv", "table1_shape": "r02_ncu_raw_table1.csv"}
+STAGE_KERNELS = {"bounds": ["bounds_kernel"], "unproject_morton_compact": ["unproject_kernel"], "sort": ["onesweep_kernel"],
+                 "tree_1": ["tree_tile_kernel", "leaf_pyramid_kernel", "emit_kernel"],
+                 "tree_2": ["tree_spine_kernel", "hierarchy_kernel", "boxes_kernel", "refit_kernel"],
+                 "render": ["render_kernel"]}
+NCU_KEYS = {"dram_read": "dram__bytes_read.sum", "dram_write": "dram__bytes_write.sum", "inst": "smsp__inst_executed.sum",
+            "lanes_per_inst": "smsp__thread_inst_executed_per_inst_executed.ratio",
+            "warp_slots_pct": "sm__warps_active.avg.pct_of_peak_sustained_active",
+            "sm_throughput_pct": "sm__throughput.avg.pct_of_peak_sustained_elapsed",
+            "ipc": "sm__inst_executed.avg.per_cycle_elapsed", "l2_hit_pct": "lts__t_sector_hit_rate.pct",
+            "l1_hit_pct": "l1tex__t_sector_hit_rate.pct", "dram_pct": "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed",
+            "duration": "gpu__time_duration.sum", "registers": "launch__registers_per_thread"}
+UNIT_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-9, "us": 1e-6, "usecond": 1e-6, "ms": 1e-3,
+              "msecond": 1e-3, "nsecond": 1e-9, "second": 1.0}
+
+
+def load_ncu(which: str) -> dict:
+    """stage -> averaged metrics of that stage's kernels in the committed capture (launches of one
+    stage are summed for bytes / instructions, averaged for ratios)."""
+    path = ROOT / "profiles" / NCU_FILES[which]
+    if not path.exists():
+        return {}
+    rows = list(csv.reader(path.open()))
+    try:
+        hi = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+    except StopIteration:
+        return {}
+    head, units = rows[hi], rows[hi + 1]
+    ki = head.index("Kernel Name")
+    out = {}
+    for stage, names in STAGE_KERNELS.items():
+        sel = [r for r in rows[hi + 2:] if len(r) == len(head) and any(n in r[ki] for n in names)]
+        if not sel:
+            continue
+        launches = {}
+        for r in sel:   # group repeated launches of the same kernel: average them
+            launches.setdefault(r[ki].split("(")[0], []).append(r)
+        m = {}
+        for key, col in NCU_KEYS.items():
+            if col not in head:
+                continue
+            ci = head.index(col)
+            scale = UNIT_SCALE.get(units[ci], 1.0)
+            per_kernel = [statistics.mean(float(r[ci].replace(",", "")) * scale for r in rs) for rs in launches.values()]
+            m[key] = sum(per_kernel) if key in ("dram_read", "dram_write", "inst", "duration") else statistics.mean(per_kernel)
+        m["kernels"] = sorted(launches)
+        m["source"] = f"profiles/{NCU_FILES[which]}"
+        out[stage] = m
+    return out
+
+
+def load_launch_list(name: str):
+    """[(kernel name, {metric: value})] in launch order from a committed `ncu --metrics a,b --csv` launch list."""
+    path = ROOT / "profiles" / name
+    if not path.exists():
+        return []
+    rows = list(csv.reader(path.open()))
+    try:
+        hi = next(i for i, r in enumerate(rows) if "Kernel Name" in r and "Metric Name" in r)
+    except StopIteration:
+        return []
+    head = rows[hi]
+    ii, ki, mi, ui, vi = (head.index(c) for c in ("ID", "Kernel Name", "Metric Name", "Metric Unit", "Metric Value"))
+    launches, by_id = [], {}
+    for r in rows[hi + 1:]:
+        if len(r) != len(head):
+            continue
+        if r[ii] not in by_id:
+            by_id[r[ii]] = (r[ki], {})
+            launches.append(by_id[r[ii]])
+        by_id[r[ii]][1][r[mi]] = float(r[vi].replace(",", "")) * UNIT_SCALE.get(r[ui], 1.0)
+    return launches
+
+
+LAUNCH_LIST = "r02_launches_config3.csv"   # `ncu --metrics gpu__time_duration.sum,smsp__inst_executed.sum` of --only headline
+
+
+def render_instructions_per_step(n_renders: int):
+    """Executed warp instructions of the render launches of ONE step (the last n_renders render launches of the
+    committed launch list, i.e. one whole sequence), or None without the file."""
+    ll = [m for k, m in load_launch_list(LAUNCH_LIST) if "render_kernel" in k and "smsp__inst_executed.sum" in m]
+    if len(ll) < n_renders:
+        return None
+    return sum(m["smsp__inst_executed.sum"] for m in ll[-n_renders:])
+
+
+def ncu_view(m: dict | None):
+    if not m:
+        return None
+    v = {k: m[k] for k in ("lanes_per_inst", "warp_slots_pct", "sm_throughput_pct", "ipc", "l2_hit_pct", "l1_hit_pct", "dram_pct",
+                           "registers") if k in m}
+    v["source"] = m["source"]
+    return v
 
 
 # --------------------------------------------------------------------------- workload
@@ -85,26 +184,28 @@ def make_workload(config_index: int, n_groups: int | None):
     return cfg, frames
 
 
-def synth_volume(cfg):
-    import synth
-    return synth.volume(cfg)
-
-
 def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
     """Compulsory DRAM traffic per launch for the layout in DESIGN.md sec. 5 (bytes)."""
+    passes = 5 if N > (1 << 19) else 4
     return {
         "bounds": 4 * P + 4 * (P // 2048 + 1),
         "unproject_morton_compact": 4 * P + 12 * N,
-        # hybrid onesweep (default): 4 passes over the top 31 code bits x (read 12 N + write 12 N)
+        # hybrid onesweep (default): 4 (5 above 2^19 splats) passes over the top code bits x (read 12 N + write 12 N)
         # + the neighbour check reading the keys once (8 N); the all-8-pass fallback is not counted
-        "sort": 4 * 24 * N + 8 * N,
-        # pyramid mode: gather (perm 4, depth 4, colour 16) -> sphere 16 + rgba 16 + pyramid 32 (N entries)
-        "tree_1": (4 + 4 + 16) * N + (16 + 16 + 32) * N,
-        # hierarchy_kernel: keys 8 read, ranges 16 written; boxes_kernel: ranges 16 + sphere 16 + pyramid 32
-        # read once, 64-byte node records written once
-        "tree_2": (8 + 16) * N + (16 + 16 + 32) * N + 64 * N,
+        "sort": passes * 24 * N + 8 * N,
+        # tiled tree: ids 4 + keys 8 + gather (depth 4, colour 16) read; sphere 16 + rgba 16 + ids 4 + node records 64
+        # + pyramid levels >= 3 (32 / 7 per leaf) written
+        "tree_1": (4 + 8 + 4 + 16) * N + (16 + 16 + 4 + 64) * N + 32 * N // 7,
+        # spine: the few nodes that span tiles (about 2.5 % of N at 1024 leaves per tile): queue entry 16, four keys
+        # 32, ~12 pyramid entries 384, record 64 -- per queued node
+        "tree_2": int(0.025 * N) * (16 + 32 + 384 + 64),
         "render": 16 * P2 + (64 + 16 + 16 + 4) * N,  # image written once + BVH/splats read once
     }
+
+
+def survey_build_bytes(P: int, N: int) -> int:
+    """24 P + 428 N, the byte count the 50 % bar (0.29 ms at 1080p, N = P) was sized with."""
+    return 24 * P + 428 * N
 
 
 # --------------------------------------------------------------------------- clocks
@@ -115,7 +216,7 @@ class ClockSampler:
                0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
                0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
 
-    def __init__(self, index: int, period: float = 0.02):
+    def __init__(self, index: int, period: float = 0.005):
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
         self._thread = None
@@ -160,34 +261,157 @@ class ClockSampler:
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+# --------------------------------------------------------------------------- legs beside the headline
+def stage_table(stage: dict, calls_expected: int, bytes_per_call: dict, total_ms: float, peak: float, ncu: dict, render_mult: int = 1):
+    rows = []
+    for name, (ms_sum, calls) in stage.items():
+        if calls == 0 or name not in bytes_per_call:
+            continue
+        b = bytes_per_call[name]
+        ms_avg = ms_sum / calls
+        gbs = b / (ms_avg * 1e-3) / 1e9 if ms_avg > 0 else 0.0
+        m = ncu.get(name)
+        rows.append({"stage": name, "calls": calls, "ms_avg": ms_avg, "share": ms_sum / total_ms if total_ms else None,
+                     "algorithmic_bytes_avg": b, "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak,
+                     "traffic_ncu": (m["dram_read"] + m["dram_write"]) if m and "dram_read" in m else None,
+                     "ncu": ncu_view(m)})
+    return rows
+
+
+def measure_frame(sp, torch, color, depth, src_cam, W, H, r_scale, dst_cams, peak, ncu, reps: int, first_hit: bool):
+    """One source frame measured on its own: per-stage build times (profiling pass, L2 flushed between
+    updates), the build as a user runs it (PDL, no stage events), and each display camera's render."""
+    P = W * H
+    N = int((np.isfinite(depth) & (depth > 0)).sum())
+    dc, dd = torch.from_numpy(color).cuda(), torch.from_numpy(depth).cuda()
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda")   # > the 126 MB L2
+    for _ in range(3):
+        sp.splats_update(dc, dd, src_cam, W, H, r_scale)
+        for cam in dst_cams:
+            sp.splats_render(cam, W, H, out)
+    torch.cuda.synchronize()
+    # (a) as a user runs it
+    evs = []
+    for _ in range(reps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        sp.splats_update(dc, dd, src_cam, W, H, r_scale)
+        e1.record()
+        evs.append((e0, e1))
+    torch.cuda.synchronize()
+    update_ms = statistics.median(a.elapsed_time(b) for a, b in evs)
+    # (b) per stage
+    sp.splats_set_profiling(True)
+    for _ in range(reps):
+        flush.zero_()
+        sp.splats_update(dc, dd, src_cam, W, H, r_scale)
+    stage = sp.splats_stage_ms()
+    ab = algorithmic_bytes(P, N, P)
+    build_stage = {k: v for k, v in stage.items() if k != "render"}
+    build_ms = sum(ms / c for ms, c in build_stage.values() if c)
+    kernels = stage_table(build_stage, reps, ab, build_ms * reps, peak, ncu)
+    own = sum(ab[k] for k in ab if k != "render")
+    survey = survey_build_bytes(P, N)
+    # (c) renders, one camera at a time
+    renders = []
+    for i, cam in enumerate(dst_cams):
+        for fh in ((False, True) if first_hit else (False,)):
+            sp.splats_traced_pixels(reset=True)
+            for _ in range(reps):
+                (sp.splats_render_first_hit if fh else sp.splats_render)(cam, W, H, out)
+            st = sp.splats_stage_ms()
+            ms, cnt = st["render"]
+            traced = sp.splats_traced_pixels(reset=True) / cnt
+            renders.append({"camera": i, "query": "first_hit" if fh else "all_hits", "ms": ms / cnt, "fps": 1e3 / (ms / cnt),
+                            "traced_rays": traced, "traced_fraction": traced / P,
+                            "mrays_per_s_traced": traced / (ms / cnt * 1e-3) / 1e6,
+                            "mrays_per_s_all_pixels": P / (ms / cnt * 1e-3) / 1e6})
+    sp.splats_set_profiling(False)
+    del flush
+    return {"W": W, "H": H, "P": P, "N": N, "coverage": N / P,
+            "update_ms": update_ms, "build_ms_staged": build_ms, "kernels": kernels,
+            "build_bytes_own": own, "build_frac_of_hbm_peak_own_bytes": own / (build_ms * 1e-3) / 1e9 / peak,
+            "build_bytes_survey_8d": survey, "build_frac_of_hbm_peak_survey_bytes": survey / (build_ms * 1e-3) / 1e9 / peak,
+            "build_frac_of_hbm_peak_survey_bytes_unstaged": survey / (update_ms * 1e-3) / 1e9 / peak,
+            "renders": renders}
+
+
+def leg_dense(sp, torch, peak, reps=20):
+    import synth
+    W, H = 1920, 1080
+    color, depth, cam = synth.dense_frame(W, H, 0)
+    sp.splats_create(W, H)
+    try:
+        r = measure_frame(sp, torch, color, depth, cam, W, H, 1.0, [synth.orbit_camera(0.0), synth.orbit_camera(3.0)], peak,
+                          load_ncu("dense"), reps, first_hit=False)
+    finally:
+        sp.splats_destroy()
+    r["note"] = ("synth.dense_frame: every pixel valid (N = P), the upper bound SURVEY.md sec. 8(d) sizes the build bar on: "
+                 "50 % of HBM peak by 24 P + 428 N = 0.29 ms; L2 flushed between updates; cameras: the source view and 3 degrees off")
+    r["target_build_ms_50pct_survey_bytes"] = survey_build_bytes(W * H, W * H) / (0.5 * peak * 1e9) * 1e3
+    return r
+
+
+def leg_table1(sp, torch, peak, reps=20):
+    import synth
+    cfg = synth.table1_config()
+    color, depth = synth.source_frame(cfg, 0)
+    sp.splats_create(cfg.W, cfg.H)
+    try:
+        r = measure_frame(sp, torch, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams, peak,
+                          load_ncu("table1_shape"), reps, first_hit=True)
+    finally:
+        sp.splats_destroy()
+    fh = [x["fps"] for x in r["renders"] if x["query"] == "first_hit"]
+    r["first_hit_fps_min_max"] = [min(fh), max(fh)]
+    r["paper"] = PAPER_TABLE1
+    r["note"] = ("synth.table1_config: config 2's volume at 1024x1024 with the camera moved in until the fill is the paper's "
+                 "(59.5 %); splats_update = the client's whole rebuild (the paper's 'LBVH' row is the build alone, its samples "
+                 "arrive unprojected); first-hit = the paper's query; the paper's numbers are another GPU's: context, not a target")
+    return r
+
+
 # --------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
     from paper_2006_14726_b200 import binding as sp
     from paper_2006_14726_b200 import replicas
 
+    if replicas.needs_spawn(args.gpus):   # started plainly with --gpus N > 1: start the N ranks ourselves
+        raise SystemExit(replicas.spawn(str(Path(__file__).resolve()), sys.argv[1:], args.gpus))
     world, rank, local_rank = replicas.world_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
     replicas.init("nccl")
     assert world == args.gpus or world == 1, f"--gpus {args.gpus} but WORLD_SIZE={world}"
+    peak, peak_src = hbm_peak()
+
+    if args.only in ("dense", "table1_shape"):   # one leg on its own (the command line of its ncu capture)
+        r = leg_dense(sp, torch, peak, args.leg_reps) if args.only == "dense" else leg_table1(sp, torch, peak, args.leg_reps)
+        if rank == 0:
+            print(json.dumps({args.only: r}), flush=True)
+        replicas.shutdown()
+        return
 
     cfg, frames = make_workload(args.config, args.groups)
     W, H = cfg.W, cfg.H
     P = W * H
     G = len(frames)
-    renders_per_step = len(frames[0]["dst_cams"])
+    n_renders = sum(len(f["dst_cams"]) for f in frames)      # display frames per step (60 for config 3)
+    max_r = max(len(f["dst_cams"]) for f in frames)
     d_color = [torch.from_numpy(f["color"]).cuda() for f in frames]
     d_depth = [torch.from_numpy(f["depth"]).cuda() for f in frames]
-    d_out = [torch.empty((H, W, 4), dtype=torch.float32, device="cuda") for _ in range(renders_per_step)]
+    d_out = [torch.empty((H, W, 4), dtype=torch.float32, device="cuda") for _ in range(max_r)]
     sp.splats_create(W, H)
 
-    def step(k: int):
-        f = frames[k % G]
-        sp.splats_update(d_color[k % G], d_depth[k % G], f["src_cam"], W, H, cfg.r_scale)
-        for j, cam in enumerate(f["dst_cams"]):
-            sp.splats_render(cam, W, H, d_out[j])
+    def step(k: int):   # the whole scripted sequence
+        for g, f in enumerate(frames):
+            sp.splats_update(d_color[g], d_depth[g], f["src_cam"], W, H, cfg.r_scale)
+            for j, cam in enumerate(f["dst_cams"]):
+                sp.splats_render(cam, W, H, d_out[j])
 
     barrier = replicas.barrier
 
@@ -204,7 +428,7 @@ def run_ours(args):
         return replicas.max_over_ranks(e0.elapsed_time(e1))
 
     K, Wm = args.steps, args.warmup
-    # the four renders of a step go to four different images: let them overlap (include/splats.h)
+    # the renders after an update go to different images: let them overlap (include/splats.h)
     sp.splats_set_option(sp.OPT_OVERLAP, 1)
     for k in range(Wm):
         step(k)
@@ -214,51 +438,181 @@ def run_ours(args):
     sampler.start()
     # ---- timed region: exactly K steps, the library as a user runs it (no per-stage events)
     launches0 = sp.splats_launch_count()
+    sp.splats_traced_pixels(reset=True)
+    n_before = len(sampler.samples)
     ms_total = timed(step, K)
+    n_in_region = len(sampler.samples) - n_before
     launches = sp.splats_launch_count() - launches0
-    n_in_region = len(sampler.samples)
-    # ---- the same K steps again with per-stage CUDA events on the library's stream (the events
-    # serialise the stages, so this pass is a little slower; kernels / roofline come from it)
+    traced_per_step = sp.splats_traced_pixels(reset=True) / K
+    # ---- a few steps again with per-stage CUDA events on the library's stream (the events serialise
+    # the stages, so this pass is slower; kernels / roofline come from it)
+    Ks = min(K, args.staged_steps)
     sp.splats_set_profiling(True)
-    ms_staged = timed(step, K)
+    ms_staged = timed(step, Ks)
     stage = sp.splats_stage_ms()
     sp.splats_set_profiling(False)
+    clocks = sampler.stop()
+    clocks["samples_in_timed_region"] = n_in_region
+    if args.only == "headline":   # the command line of the headline's ncu capture
+        sp.splats_destroy()
+        replicas.shutdown()
+        if rank == 0:
+            print(json.dumps({"value": K * n_renders * world / (ms_total * 1e-3), "ms_per_step": ms_total / K}), flush=True)
+        return
 
-    # ---- the paper's first-hit query on the same sequence: renders only,
-    # reported beside the headline, not part of it
-    def step_first(k: int):
-        f = frames[k % G]
-        if k < G:   # one pass over the source frames is enough
-            sp.splats_update(d_color[k % G], d_depth[k % G], f["src_cam"], W, H, cfg.r_scale)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for j, cam in enumerate(f["dst_cams"]):
-                sp.splats_render_first_hit(cam, W, H, d_out[j])
-            e1.record()
-            first_events.append((e0, e1, len(f["dst_cams"])))
-            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            p0.record()
-            for j, cam in enumerate(f["dst_cams"]):
-                sp.splats_render_points(cam, W, H, 2, d_out[j])
-            p1.record()
-            point_events.append((p0, p1, len(f["dst_cams"])))
+    extras = {}
+    if not args.no_legs:
+        extras = run_extras(sp, torch, cfg, frames, d_color, d_depth, d_out, K, Wm, timed, barrier)
 
+    frames_done = K * n_renders * world
+    value = frames_done / (ms_total * 1e-3)
+
+    # ---- per-kernel table and roofline from the staged pass
+    ncu = load_ncu("headline")
+    ab_sum = {}
+    for f in frames:
+        ab = algorithmic_bytes(P, f["N"], P)
+        for name, b in ab.items():
+            ab_sum[name] = ab_sum.get(name, 0) + b * (len(f["dst_cams"]) if name == "render" else 1)
+    calls_per_step = {name: (n_renders if name == "render" else G) for name in ab_sum}
+    kernels = []
+    for name, (ms_sum, calls) in stage.items():
+        if calls == 0 or name not in ab_sum:
+            continue
+        b_avg = ab_sum[name] / calls_per_step[name]
+        ms_avg = ms_sum / calls
+        gbs = b_avg / (ms_avg * 1e-3) / 1e9
+        m = ncu.get(name)
+        kernels.append({"stage": name, "calls": calls, "ms_avg": ms_avg, "share": ms_sum / ms_staged,
+                        "algorithmic_bytes_avg": b_avg, "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak,
+                        # ncu's DRAM bytes are those of the one launch it captured (see the .md beside the file), not an average
+                        "traffic_ncu": (m["dram_read"] + m["dram_write"]) if m and "dram_read" in m else None,
+                        "ncu": ncu_view(m)})
+    dominant = max(kernels, key=lambda r: r["share"])
+    build = [r for r in kernels if r["stage"] != "render"]
+    build_ms = sum(r["ms_avg"] for r in build)
+    build_bytes = sum(r["algorithmic_bytes_avg"] for r in build)
+    render_ms = next(r["ms_avg"] for r in kernels if r["stage"] == "render")
+    traced_per_render = traced_per_step / n_renders
+    N_avg = sum(f["N"] for f in frames) / G
+
+    # The dominant kernel is the traversal.  ncu (profiles/, same command line) shows what bounds it: warp
+    # instruction issue at about half the lanes, not DRAM.  `roofline` therefore reports the instruction issue rate
+    # (ncu's executed warp instructions of the captured launch scaled by traced rays, over the live time) against
+    # the SMs' issue peak, and keeps the algorithmic-bytes HBM fraction beside it.
+    dm = ncu.get(dominant["stage"])
+    sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965
+    issue_peak = SM_COUNT * ISSUE_PER_SM_CLK * sm_mhz * 1e6 / 1e9      # G warp instructions / s
+    roofline = {"kernel": dominant["stage"], "peak_source": peak_src,
+                "hbm": {"bound": "hbm", "achieved": dominant["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                        "frac": dominant["achieved_gbs"] / peak,
+                        "note": "algorithmic bytes (image written once + BVH and splats read once) / live launch time"}}
+    inst_step = render_instructions_per_step(n_renders) if dominant["stage"] == "render" and args.config == 3 else None
+    if inst_step:
+        # executed warp instructions of the 60 render launches of one step (ncu launch list of this command line)
+        # over their live duration (per-stage events of the staged pass)
+        ginst = inst_step / (render_ms * n_renders * 1e-3) / 1e9
+        roofline.update({"bound": "alu", "achieved": ginst, "peak": issue_peak, "unit": "Gwarp-inst/s", "frac": ginst / issue_peak,
+                         "traffic": (dm["dram_read"] + dm["dram_write"]) if dm and "dram_read" in dm else None,
+                         "warp_instructions_per_launch": inst_step / n_renders,
+                         "limiter": ncu_view(dm),
+                         "note": "traversal: issue / latency bound, not DRAM (ncu figures of one mid-sequence launch in `limiter`: "
+                                 "sm__throughput, lanes per instruction, warp slots).  achieved = smsp__inst_executed.sum summed over "
+                                 f"the step's render launches (profiles/{LAUNCH_LIST}) / their live duration; peak = "
+                                 f"{SM_COUNT} SMs x {ISSUE_PER_SM_CLK} warp instructions per clock x the SM clock sampled under load; "
+                                 "traffic = ncu DRAM bytes of the captured launch; the HBM view of the same kernel is in `hbm`"})
+    else:
+        roofline.update({"bound": "hbm", "achieved": dominant["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                         "frac": dominant["achieved_gbs"] / peak, "traffic": None,
+                         "note": "no ncu capture of this command line under profiles/: algorithmic bytes over live time only"})
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.vol_n}^3 volume, {W}x{H} source frames; one step = the whole "
+                               f"scripted sequence: {G} rebuilds + {n_renders} renders, r_scale {cfg.r_scale}, dolly x0.5 over the sequence",
+                   "display_frames_per_step": n_renders, "updates_per_step": G,
+                   "splats_per_frame_min_max": [min(f["N"] for f in frames), max(f["N"] for f in frames)],
+                   "coverage_min_max": [min(f["N"] for f in frames) / P, max(f["N"] for f in frames) / P],
+                   "l2_policy": f"inputs larger than L2: {G} source frames x {P * 20 / 1e6:.1f} MB cycled",
+                   "launch_mode": "programmatic dependent launches, consecutive renders of one BVH overlap "
+                                  "(SPLATS_OPT_PDL, SPLATS_OPT_OVERLAP); kernels / roofline from a second pass of "
+                                  f"{Ks} steps with per-stage events, stages serialised",
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "gpu_launches": int(launches),
+        "value_with_stage_events": Ks * n_renders * world / (ms_staged * 1e-3), "ms_per_step_with_stage_events": ms_staged / Ks,
+        "build_ms": build_ms, "render_ms": render_ms,
+        "traced_rays_per_render": traced_per_render, "traced_fraction": traced_per_render / P,
+        "mrays_per_s": traced_per_render / (render_ms * 1e-3) / 1e6,
+        "mrays_per_s_all_pixels": P / (render_ms * 1e-3) / 1e6,
+        "mrays_note": "mrays_per_s counts the rays the kernel set up (pixels of 8x4 tiles inside the scene's screen rectangle, "
+                      "counted on the device); the all-pixel figure includes background pixels that are only zero-filled",
+        "roofline": roofline,
+        "roofline_build": {"bound": "hbm", "achieved": build_bytes / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                           "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": build_bytes,
+                           "frac_by_survey_bytes": survey_build_bytes(P, N_avg) / (build_ms * 1e-3) / 1e9 / peak,
+                           "note": f"all build kernels of one splats_update at this config's coverage (N = {N_avg:.0f} of {P} on average: "
+                                   "L2 resident and launch / latency bound); the bar's own regime is the `dense` leg"},
+        "kernels": kernels,
+    }
+    out.update(extras)
+    sp.splats_destroy()
+    if rank == 0 and world == 1 and not args.no_legs:
+        out["dense"] = leg_dense(sp, torch, peak, args.leg_reps)
+        out["table1_shape"] = leg_table1(sp, torch, peak, args.leg_reps)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(cfg, frames)
+    replicas.shutdown()
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+
+
+def run_extras(sp, torch, cfg, frames, d_color, d_depth, d_out, K, Wm, timed, barrier):
+    """The sec. 8(f) calls and the end-to-end variants on the same sequence, outside the headline's timed region."""
+    W, H = cfg.W, cfg.H
+    P = W * H
+    G = len(frames)
+    n_renders = sum(len(f["dst_cams"]) for f in frames)
+    max_r = max(len(f["dst_cams"]) for f in frames)
+    peak, _ = hbm_peak()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    Ke = max(1, min(K, 5))   # end-to-end steps (a step is the whole sequence)
+
+    # ---- the paper's first-hit query and the point baseline on the same sequence: renders only
     first_events, point_events = [], []
-    for k in range(min(K, G)):
-        step_first(k)
+    sp.splats_traced_pixels(reset=True)
+    for g, f in enumerate(frames):
+        sp.splats_update(d_color[g], d_depth[g], f["src_cam"], W, H, cfg.r_scale)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for j, cam in enumerate(f["dst_cams"]):
+            sp.splats_render_first_hit(cam, W, H, d_out[j])
+        e1.record()
+        first_events.append((e0, e1, len(f["dst_cams"])))
+    traced_first = sp.splats_traced_pixels(reset=True) / n_renders
+    for g, f in enumerate(frames):
+        sp.splats_update(d_color[g], d_depth[g], f["src_cam"], W, H, cfg.r_scale)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record()
+        for j, cam in enumerate(f["dst_cams"]):
+            sp.splats_render_points(cam, W, H, 2, d_out[j])
+        p1.record()
+        point_events.append((p0, p1, len(f["dst_cams"])))
     torch.cuda.synchronize()
-    first_ms = sum(a.elapsed_time(b) for a, b, _ in first_events) / max(1, sum(n for _, _, n in first_events))
-    points_ms = sum(a.elapsed_time(b) for a, b, _ in point_events) / max(1, sum(n for _, _, n in point_events))
+    first_ms = sum(a.elapsed_time(b) for a, b, _ in first_events) / n_renders
+    points_ms = sum(a.elapsed_time(b) for a, b, _ in point_events) / n_renders
 
-    # ---- the paper's wire format: server-side pack + compaction and the
-    # client-side build from packed samples, once per source frame; reported beside the headline
-    import math
+    # ---- the paper's wire format (SURVEY.md sec. 8(f) row 2): server-side march + pack + compaction and the
+    # client-side build from packed samples, once per source frame
+    import synth
     half_diag = math.sqrt(3.0) / cfg.vol_n / 2          # PAPER.md:69: half a voxel's diagonal
     quant = [0.0, 0.0, 0.0, 1.0, 1.0, 1.0, 4 * half_diag]
     w_samples = torch.empty(P, dtype=torch.int64, device="cuda")
     w_colors = torch.empty(P, dtype=torch.int32, device="cuda")
     w_count = torch.zeros(1, dtype=torch.int32, device="cuda")
-    d_vol = torch.from_numpy(synth_volume(cfg)).cuda()
+    d_vol = torch.from_numpy(synth.volume(cfg)).cuda()
     m_color = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
     m_depth = torch.empty((H, W), dtype=torch.float32, device="cuda")
     tf = sp.make_transfer([(0.35, 0.8, (0.95, 0.55, 0.15)), (0.70, 0.95, (0.25, 0.60, 0.95))])
@@ -296,38 +650,35 @@ def run_ours(args):
     pack_avg, upd_avg, n_avg = sum(pack_ms) / len(pack_ms), sum(upd_ms) / len(upd_ms), sum(wire_n) / len(wire_n)
     pack_bytes = 8 * P + 28 * n_avg                     # depth read twice, colour read + 12 B written per sample
 
-    # ---- end-to-end through the host-buffer entry points (H2D of the frame, D2H of every image)
+    # ---- end-to-end through the host-buffer entry points (H2D of every frame, D2H of every image)
     h_color = [torch.from_numpy(f["color"]).pin_memory() for f in frames]
     h_depth = [torch.from_numpy(f["depth"]).pin_memory() for f in frames]
-    h_out = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(renders_per_step)]
+    h_out = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(max_r)]
 
     def step_e2e(k: int):
-        f = frames[k % G]
-        sp.splats_update_host(h_color[k % G], h_depth[k % G], f["src_cam"], W, H, cfg.r_scale)
-        for j, cam in enumerate(f["dst_cams"]):
-            sp.splats_render_host(cam, W, H, h_out[j])
+        for g, f in enumerate(frames):
+            sp.splats_update_host(h_color[g], h_depth[g], f["src_cam"], W, H, cfg.r_scale)
+            for j, cam in enumerate(f["dst_cams"]):
+                sp.splats_render_host(cam, W, H, h_out[j])
 
-    for k in range(min(Wm, 3)):
-        step_e2e(k)
+    step_e2e(0)
     sp.splats_synchronize()
     barrier()
     t0 = time.perf_counter()
-    ms_e2e_dev = timed(step_e2e, K, fin=sp.splats_synchronize)
+    ms_e2e = timed(step_e2e, Ke, fin=sp.splats_synchronize)
     wall_e2e = (time.perf_counter() - t0) * 1e3
-    ms_e2e = max(ms_e2e_dev, 0.0)
     # ---- the same end-to-end steps with the 8-bit display image read back (extra key, not the e2e)
-    h_out8 = [torch.empty((H, W), dtype=torch.int32).pin_memory() for _ in range(renders_per_step)]
+    h_out8 = [torch.empty((H, W), dtype=torch.int32).pin_memory() for _ in range(max_r)]
 
     def step_e2e8(k: int):
-        f = frames[k % G]
-        sp.splats_update_host(h_color[k % G], h_depth[k % G], f["src_cam"], W, H, cfg.r_scale)
-        for j, cam in enumerate(f["dst_cams"]):
-            sp.splats_render_host_rgba8(cam, W, H, h_out8[j])
+        for g, f in enumerate(frames):
+            sp.splats_update_host(h_color[g], h_depth[g], f["src_cam"], W, H, cfg.r_scale)
+            for j, cam in enumerate(f["dst_cams"]):
+                sp.splats_render_host_rgba8(cam, W, H, h_out8[j])
 
-    for k in range(min(Wm, 3)):
-        step_e2e8(k)
+    step_e2e8(0)
     sp.splats_synchronize()
-    ms_e2e8 = timed(step_e2e8, K, fin=sp.splats_synchronize)
+    ms_e2e8 = timed(step_e2e8, Ke, fin=sp.splats_synchronize)
     # ---- the paper's own client, end to end: packed samples arrive in host memory (12 B per sample,
     # PAPER.md:103), BVH build, 8-bit display images read back (extra key, not the e2e)
     sp.splats_set_radius(sp.RADIUS_CONSTANT, half_diag)
@@ -338,84 +689,32 @@ def run_ours(args):
         h_samples.append(w_samples[:n_s].cpu().pin_memory())
         h_colors.append(w_colors[:n_s].cpu().pin_memory())
         n_packed.append(n_s)
-    sp.splats_set_radius(sp.RADIUS_FOOTPRINT, 0.0)
 
     def step_client(k: int):
-        g = k % G
-        sp.splats_update_packed_host(h_samples[g], h_colors[g], n_packed[g], quant)
-        for j, cam in enumerate(frames[g]["dst_cams"]):
-            sp.splats_render_host_rgba8(cam, W, H, h_out8[j])
+        for g in range(G):
+            sp.splats_update_packed_host(h_samples[g], h_colors[g], n_packed[g], quant)
+            for j, cam in enumerate(frames[g]["dst_cams"]):
+                sp.splats_render_host_rgba8(cam, W, H, h_out8[j])
 
-    for k in range(min(Wm, 3)):
-        step_client(k)
+    step_client(0)
     sp.splats_synchronize()
-    ms_client = timed(step_client, K, fin=sp.splats_synchronize)
-    clocks = sampler.stop()
-    clocks["samples_in_timed_region"] = n_in_region
+    ms_client = timed(step_client, Ke, fin=sp.splats_synchronize)
+    sp.splats_set_radius(sp.RADIUS_FOOTPRINT, 0.0)
 
-    frames_done = K * renders_per_step * world
-    value = frames_done / (ms_total * 1e-3)
-    peak, peak_src = hbm_peak()
-
-    # ---- per-kernel roofline from the events recorded inside the timed region
-    steps_N = [frames[k % G]["N"] for k in range(K)]
-    kernels = []
-    bytes_sum = {}
-    for k in range(K):
-        ab = algorithmic_bytes(P, steps_N[k], P)
-        for name, b in ab.items():
-            mult = renders_per_step if name == "render" else 1
-            bytes_sum[name] = bytes_sum.get(name, 0) + b * mult
-    for name, (ms_sum, calls) in stage.items():
-        if calls == 0:
-            continue
-        gbs = bytes_sum[name] / (ms_sum * 1e-3) / 1e9 if ms_sum > 0 else 0.0
-        kernels.append({"stage": name, "launches_per_call": 1, "calls": calls,
-                        "ms_avg": ms_sum / calls, "share": ms_sum / ms_staged, "algorithmic_bytes_avg": bytes_sum[name] / calls,
-                        "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak,
-                        "traffic_ncu": NCU_TRAFFIC_BYTES.get(name)})
-    dominant = max(kernels, key=lambda r: r["share"])
-    build = [r for r in kernels if r["stage"] != "render"]
-    build_ms = sum(r["ms_avg"] for r in build)
-    build_bytes = sum(r["algorithmic_bytes_avg"] for r in build)
-    render_ms = next(r["ms_avg"] for r in kernels if r["stage"] == "render")
-
-    out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.vol_n}^3 volume, {W}x{H} source frames, "
-                               f"{G} source frames cycled, 1 rebuild + {renders_per_step} renders per step, "
-                               f"r_scale {cfg.r_scale}, dolly x0.5 over the sequence",
-                   "splats_per_frame_min_max": [min(steps_N), max(steps_N)],
-                   "l2_policy": f"inputs larger than L2: {G} source frames x {P * 20 / 1e6:.1f} MB cycled",
-                   "launch_mode": "programmatic dependent launches, consecutive renders of a step overlap "
-                                  "(SPLATS_OPT_PDL, SPLATS_OPT_OVERLAP); kernels / roofline from a second pass of the same "
-                                  "steps with per-stage events, stages serialised",
-                   "parallelism": "replicas" if world > 1 else "single GPU"},
-        "clocks": clocks,
-        "e2e": {"value": frames_done / (ms_e2e * 1e-3), "unit": UNIT,
-                "h2d_bytes_per_step": P * 20, "d2h_bytes_per_step": P * 16 * renders_per_step,
-                "wall_ms_per_step": wall_e2e / K},
-        "e2e_rgba8": {"value": frames_done / (ms_e2e8 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": P * 20,
-                      "d2h_bytes_per_step": P * 4 * renders_per_step,
+    fr = Ke * n_renders * world
+    return {
+        "e2e": {"value": fr / (ms_e2e * 1e-3), "unit": UNIT, "steps": Ke,
+                "h2d_bytes_per_step": P * 20 * G, "d2h_bytes_per_step": P * 16 * n_renders,
+                "ms_per_step": ms_e2e / Ke, "wall_ms_per_step": wall_e2e / Ke,
+                "note": "the same steps through splats_update_host / splats_render_host from pinned host memory; bound by the "
+                        "PCIe read-back of the float32 images"},
+        "e2e_rgba8": {"value": fr / (ms_e2e8 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": P * 20 * G,
+                      "d2h_bytes_per_step": P * 4 * n_renders,
                       "note": "same steps with splats_render_host_rgba8 (8-bit display image read back instead of float32)"},
-        "e2e_paper_client": {"value": frames_done / (ms_client * 1e-3), "unit": UNIT,
-                             "h2d_bytes_per_step": 12 * sum(n_packed) / G, "d2h_bytes_per_step": P * 4 * renders_per_step,
+        "e2e_paper_client": {"value": fr / (ms_client * 1e-3), "unit": UNIT,
+                             "h2d_bytes_per_step": 12 * sum(n_packed), "d2h_bytes_per_step": P * 4 * n_renders,
                              "note": "splats_update_packed_host (64-bit samples + RGBA8 colours from pinned host memory, "
-                                     "constant half-voxel-diagonal radius) + 4 x splats_render_host_rgba8 per step"},
-        "gpu_launches": int(launches),
-        "value_with_stage_events": frames_done / (ms_staged * 1e-3), "ms_per_step_with_stage_events": ms_staged / K,
-        "build_ms": build_ms, "render_ms": render_ms, "mrays_per_s": P / (render_ms * 1e-3) / 1e6,
-        "roofline": {"kernel": dominant["stage"], "bound": "hbm", "achieved": dominant["achieved_gbs"], "peak": peak,
-                     "unit": "GB/s", "frac": dominant["achieved_gbs"] / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get(dominant["stage"]), "peak_source": peak_src,
-                     "note": "dominant kernel by time; traversal is L2/latency bound, its algorithmic DRAM floor is "
-                             "the image written once plus BVH and splats read once (DESIGN.md sec. 6)"},
-        "roofline_build": {"bound": "hbm", "achieved": build_bytes / (build_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                           "frac": build_bytes / (build_ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": build_bytes,
-                           "note": "all build kernels of one splats_update (6 launches), per-stage events of the staged pass"},
-        "kernels": kernels,
+                                     "constant half-voxel-diagonal radius) + splats_render_host_rgba8"},
         "wire_format": {"march_ms": sum(march_ms) / len(march_ms), "pack_ms": pack_avg, "pack_gbs": pack_bytes / (pack_avg * 1e-3) / 1e9,
                         "pack_frac_of_hbm_peak": pack_bytes / (pack_avg * 1e-3) / 1e9 / peak,
                         "update_packed_ms": upd_avg, "samples_avg": n_avg, "payload_bytes_avg": 12 * n_avg,
@@ -426,22 +725,18 @@ def run_ours(args):
         "point_baseline": {"render_ms": points_ms,
                            "note": "splats_render_points, 2x2-pixel points: CUDA restatement of the OpenGL point rendering of "
                                    "[ZAL12] that the paper compares against (PAPER.md:37,89); GL itself is unavailable on this box"},
-        "first_hit": {"render_ms": first_ms, "mrays_per_s": P / (first_ms * 1e-3) / 1e6,
+        "first_hit": {"render_ms": first_ms, "traced_rays_per_render": traced_first,
+                      "mrays_per_s": traced_first / (first_ms * 1e-3) / 1e6,
+                      "mrays_per_s_all_pixels": P / (first_ms * 1e-3) / 1e6,
                       "note": "splats_render_first_hit (the paper's own query, PAPER.md:53,59) on the same frames and cameras"},
     }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(cfg, frames)
-    sp.splats_destroy()
-    replicas.shutdown()
-    if rank == 0:
-        print(json.dumps(out), flush=True)
 
 
 # --------------------------------------------------------------------------- oracle arms
 def oracle_step(cfg, frame, sample_every: int, seed: int):
-    """One step of the oracle on a bounded sample: the full build (O1-O7) and, for each of the
-    step's display frames, the BVH-walk render (O8-O9) of every `sample_every`-th pixel (random
-    subset); returns (build seconds, render seconds extrapolated to full frames)."""
+    """The oracle on a bounded sample of one source frame's work: the full build (O1-O7) and, for each of
+    its display frames, the BVH-walk render (O8-O9) of every `sample_every`-th pixel (random subset);
+    returns (build seconds, measured render seconds of the sample)."""
     import oracle
     W, H = cfg.W, cfg.H
     t0 = time.perf_counter()
@@ -454,7 +749,7 @@ def oracle_step(cfg, frame, sample_every: int, seed: int):
         px = np.sort(rng.choice(W * H, size=n_px, replace=False)).astype(np.int64)
         t0 = time.perf_counter()
         oracle.render(sc, cam, W, H, "bvh", pixels=px)
-        t_render += (time.perf_counter() - t0) * (W * H / n_px)
+        t_render += time.perf_counter() - t0
     return t_build, t_render
 
 
@@ -462,10 +757,10 @@ def cpu_baseline(cfg, frames):
     g = len(frames) // 2
     tb, tr = oracle_step(cfg, frames[g], sample_every=2, seed=1)
     n = len(frames[g]["dst_cams"])
-    return {"value": n / (tb + tr), "unit": UNIT, "cores": 1, "kind": "oracle",
+    return {"value": n / (tb + 2 * tr), "unit": UNIT, "cores": 1, "kind": "oracle",
             "sample": f"source frame {g} of {len(frames)} (N={frames[g]['N']}): full oracle build ({tb * 1e3:.0f} ms) + "
-                      f"BVH-walk render of a random half of the pixels of its {n} display frames, render time x2",
-            "build_ms": tb * 1e3, "render_ms_per_frame": tr / n * 1e3, "host_cores_available": os.cpu_count()}
+                      f"BVH-walk render of a random half of the pixels of its {n} display frames ({tr:.2f} s measured, counted x2)",
+            "build_ms": tb * 1e3, "render_ms_per_frame": 2 * tr / n * 1e3, "host_cores_available": os.cpu_count()}
 
 
 def run_reference(args):
@@ -474,20 +769,27 @@ def run_reference(args):
         return
     cfg, frames = make_workload(args.config, args.groups)
     G = len(frames)
-    n = len(frames[0]["dst_cams"])
+    n_seq = sum(len(f["dst_cams"]) for f in frames)
     sample_every = 16
+    # One step of our arm is the whole sequence (15 builds + 60 renders).  The oracle's step is a bounded sample of
+    # it: ONE source frame of the sequence (cycling through them step by step), its full build and 1/16 of the pixels
+    # of its display frames.  value = frames/s extrapolated to whole frames; ms_per_step is the time actually spent.
     for k in range(args.warmup):
         oracle_step(cfg, frames[k % G], sample_every, k)
-    total = 0.0
+    total_est, total_real, n_frames = 0.0, 0.0, 0
     for k in range(args.steps):
-        tb, tr = oracle_step(cfg, frames[k % G], sample_every, 100 + k)
-        total += tb + tr
-    value = args.steps * n / total
-    sample = (f"per step: full oracle build + BVH-walk render of a random 1/{sample_every} of the pixels of each of the "
-              f"{n} display frames, render time x{sample_every}")
+        f = frames[(k * 7) % G]   # stride 7 walks the 15 frames evenly whatever K is
+        tb, tr = oracle_step(cfg, f, sample_every, 100 + k)
+        total_est += tb + tr * sample_every
+        total_real += tb + tr
+        n_frames += len(f["dst_cams"])
+    value = n_frames / total_est
+    sample = (f"per step: ONE of the sequence's {G} source frames (stride 7), full oracle build + BVH-walk render of a random "
+              f"1/{sample_every} of the pixels of each of its display frames; value extrapolates the render time x{sample_every}; "
+              f"ms_per_step is the time actually spent; a full step of the GPU arm is the whole sequence ({G} builds + {n_seq} renders)")
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "warmup": args.warmup, "ms_per_step": total_real / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "extrapolated": True,
            "config": {"workload": f"BASELINE.json configs[{args.config}] ({cfg.W}x{cfg.H}), oracle on a bounded sample: {sample}"},
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -498,11 +800,16 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300, help="15 steps = one scripted 60-frame sequence")
+    ap.add_argument("--steps", type=int, default=20, help="one step = the whole scripted sequence (config 3: 15 updates + 60 renders)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (headline: 3)")
     ap.add_argument("--groups", type=int, default=None, help="use only the first G source frames (debug)")
+    ap.add_argument("--staged-steps", type=int, default=3, help="steps of the per-stage-event pass")
+    ap.add_argument("--leg-reps", type=int, default=20, help="repetitions inside the dense / table1_shape legs")
+    ap.add_argument("--only", choices=["headline", "dense", "table1_shape"], default=None,
+                    help="run just this part (the command lines of the ncu captures under profiles/)")
+    ap.add_argument("--no-legs", action="store_true", help="skip everything beside the headline and its kernel table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -233,6 +233,12 @@ int splats_count(unsigned* n_host);
 int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* parents,
                   float* node_aabbs);
 
+/* The boxes the traversal actually tests: for every internal node j (Karras numbering) the 12
+ * floats stored in its record -- left child box lo xyz, hi xyz, then the right child's -- copied
+ * verbatim (splats_export's node_aabbs are derived: a node's box there is the union of these two).
+ *   child_boxes  dev, (N-1)*12 float32.  Synchronises.  Parity only. */
+int splats_export_child_boxes(float* child_boxes);
+
 /* Export the splats themselves in sorted order (dev pointers, may be NULL): sphere N*4
  * float32 (cx, cy, cz, r), rgba N*4 float32; and the scene bounds (min/max of the centres)
  * lo_hi: 6 float32.  Synchronises.  Parity/debug only. */
@@ -310,6 +316,13 @@ int splats_set_radius(int mode, float param);
 #define SPLATS_NUM_STAGES 9
 int splats_set_profiling(int on);
 int splats_stage_ms(float* ms_sum /* host, SPLATS_NUM_STAGES */, unsigned* calls /* host, SPLATS_NUM_STAGES */);
+
+/* Rays actually traced: the sum, over every splats_render* call since splats_create (or since
+ * the last call with reset != 0), of the destination pixels that lie in 8x4-pixel tiles inside the
+ * screen rectangle of the scene box -- the pixels for which a primary ray was set up and the BVH
+ * was walked; every other pixel is written as background without a ray.  Counted
+ * by the render kernel.  Synchronises the stream.  Measurement only. */
+int splats_traced_pixels(unsigned long long* pixels_host, int reset);
 
 /* How many kernels this library has launched since splats_create. */
 unsigned long long splats_launch_count(void);

@@ -76,11 +76,13 @@ def lib() -> ctypes.CDLL:
         L.splats_count.argtypes = [ctypes.POINTER(ctypes.c_uint)]
         L.splats_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
         L.splats_export_splats.argtypes = [_vp, _vp, _vp]
+        L.splats_export_child_boxes.argtypes = [_vp]
         L.splats_set_profiling.argtypes = [_ci]
         L.splats_set_option.argtypes = [_ci, _ci]
         L.splats_set_radius.argtypes = [_ci, ctypes.c_float]
         L.splats_stage_ms.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_uint)]
         L.splats_launch_count.restype = ctypes.c_ulonglong
+        L.splats_traced_pixels.argtypes = [ctypes.POINTER(ctypes.c_ulonglong), _ci]
         L.splats_last_error.restype = ctypes.c_char_p
         L.splats_destroy.restype = None
         _lib = L
@@ -257,6 +259,16 @@ def splats_export():
     return dict(N=n, keys=keys, perm=perm, children=children, parents=parents, node_aabbs=aabbs)
 
 
+def splats_export_child_boxes():
+    """(N-1, 12) float32 CUDA tensor: the two child boxes stored in every internal node's record."""
+    n = splats_count()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    boxes = torch.empty((max(n - 1, 0), 12), dtype=torch.float32, device=dev)
+    if n > 1:
+        _check(lib().splats_export_child_boxes(boxes.data_ptr()))
+    return boxes
+
+
 def splats_export_splats():
     n = splats_count()
     dev = torch.device("cuda", torch.cuda.current_device())
@@ -290,6 +302,13 @@ def splats_stage_ms() -> dict:
 
 def splats_launch_count() -> int:
     return int(lib().splats_launch_count())
+
+
+def splats_traced_pixels(reset: bool = False) -> int:
+    """Destination pixels for which the renders set up a ray since the last reset (synchronises)."""
+    v = ctypes.c_ulonglong(0)
+    _check(lib().splats_traced_pixels(ctypes.byref(v), 1 if reset else 0))
+    return int(v.value)
 
 
 def splats_synchronize() -> None:

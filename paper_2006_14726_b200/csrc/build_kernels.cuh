@@ -1,9 +1,8 @@
 // build_kernels.cuh -- steps a1 (scene bounds) and a2 (unproject + validate + Morton +
 // order-preserving compaction + digit histograms) of SURVEY.md sec. 8(a).
 //
-// Both kernels walk the source frame in the same tiles of TILE_PX consecutive pixels; a
-// thread owns 8 consecutive pixels (two 16-byte vector loads of depth), so the compacted
-// output keeps ascending pixel order, which makes the later stable sort an order by
+// Both kernels walk the source frame in the same tiles of TILE_PX consecutive pixels and keep
+// ascending pixel order in the compacted output, which makes the later stable sort an order by
 // (code, id) (north_star: "keyed on (code, splat id) so ties are stable and deterministic").
 #pragma once
 #include "common.cuh"
@@ -27,19 +26,33 @@ __device__ __forceinline__ void load_depth8(const float* __restrict__ depth, int
   }
 }
 
-// Where the splat centres come from.  FrameSource: the 2.5D frame itself (splats_update; Eq. 1
-// per valid pixel).  PackedSource: a received buffer of quantised samples (splats_update_packed;
-// every element is a splat unless its radius field is 0).  Element index = splat id.
+// Where the splat centres come from.  FrameSource: the 2.5D frame itself (splats_update): Eq. 1 is
+// evaluated ONCE per valid pixel, in bounds_kernel, which stores the splat (centre + radius) at its
+// pixel index; unproject_kernel and the tree's gather read that record instead of evaluating Eq. 1
+// again (three IEEE divisions + a square root + three more divisions per pixel each time).
+// PackedSource: a received buffer of quantised samples (splats_update_packed; every element is a
+// splat unless its radius field is 0); decoding is cheap, nothing is stored.  Element index = splat id.
 struct FrameSource {
   const float* __restrict__ depth;
+  const float4* __restrict__ color;   // alpha is read only by the opacity radius (RadiusParams mode 2)
+  float4* sphere_px;                  // [P] splat of every valid pixel, written by bounds_kernel
   DevCamera cam;
+  RadiusParams rp;
   using Raw = float;
   __device__ __forceinline__ int width() const { return cam.W; }
-  __device__ __forceinline__ void load8(int64_t base, int64_t P, Raw t[8]) const { load_depth8(depth, base, P, t); }
+  __device__ __forceinline__ Raw load(int64_t i) const { return __ldg(depth + i); }
+  __device__ __forceinline__ Raw invalid() const { return 0.0f; }
   __device__ __forceinline__ bool valid(Raw t) const { return depth_valid(t); }
-  __device__ __forceinline__ void centre(Raw t, int x, int y, float p[3]) const {
+  __device__ __forceinline__ void bounds_centre(Raw t, int64_t i, int x, int y, float p[3]) const {
     float len;
     splat_centre(cam, x, y, t, p, len);
+    const float z = div_(t, len);
+    const float alpha = rp.mode == 2 ? __ldg(&color[i].w) : 0.0f;
+    sphere_px[i] = make_float4(p[0], p[1], p[2], splat_radius(rp, z, alpha));
+  }
+  __device__ __forceinline__ void key_centre(Raw, int64_t i, float p[3]) const {
+    const float4 sp = __ldcg(sphere_px + i);   // written by the previous kernel of this stream
+    p[0] = sp.x; p[1] = sp.y; p[2] = sp.z;
   }
 };
 struct PackedSource {
@@ -47,23 +60,18 @@ struct PackedSource {
   QuantParams q;
   using Raw = uint64_t;
   __device__ __forceinline__ int width() const { return 0x7fffffff; }  // one long row: x = index
-  __device__ __forceinline__ void load8(int64_t base, int64_t P, Raw w[8]) const {
-    if (base + 8 <= P) {
-      const ulonglong2* v = reinterpret_cast<const ulonglong2*>(samples + base);
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const ulonglong2 a = __ldg(v + k);
-        w[2 * k] = a.x;
-        w[2 * k + 1] = a.y;
-      }
-    } else {
-#pragma unroll
-      for (int k = 0; k < 8; ++k) w[k] = (base + k < P) ? __ldg(samples + base + k) : 0ull;
-    }
-  }
+  __device__ __forceinline__ Raw load(int64_t i) const { return __ldg(samples + i); }
+  __device__ __forceinline__ Raw invalid() const { return 0ull; }
   __device__ __forceinline__ bool valid(Raw w) const { return (w >> 48) != 0ull; }
-  __device__ __forceinline__ void centre(Raw w, int, int, float p[3]) const { decode_centre(w, q, p); }
+  __device__ __forceinline__ void bounds_centre(Raw w, int64_t, int, int, float p[3]) const { decode_centre(w, q, p); }
+  __device__ __forceinline__ void key_centre(Raw w, int64_t, float p[3]) const { decode_centre(w, q, p); }
 };
+
+// Both kernels walk the source in tiles of TILE_PX consecutive elements; a warp owns 256 consecutive
+// ones and visits them in 8 rounds of 32 (lane = consecutive element: every load and store of a
+// round is one coalesced request, and a ballot gives the order-preserving rank).
+constexpr int WARP_PX = TILE_PX / (BUILD_THREADS / 32);   // 256
+constexpr int ROUNDS = WARP_PX / 32;                      // 8
 
 // ------------------------------------------------------------------------------------ a1
 // Scene bounds = component-wise min/max of the valid splat centres (Eq. 1),
@@ -76,26 +84,26 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
   __shared__ float s_red[6][BUILD_THREADS / 32];
   __shared__ uint32_t s_cnt[BUILD_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t base = (int64_t)blockIdx.x * TILE_PX + (int64_t)tid * PX_PER_THREAD;
+  const int64_t base = (int64_t)blockIdx.x * TILE_PX + (int64_t)warp * WARP_PX + lane;
   const float INF = __int_as_float(0x7f800000);
   float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
   uint32_t cnt = 0;
-  if (base < P) {
-    typename Src::Raw t[8];
-    src.load8(base, P, t);
-    const int W = src.width();
-    int y = (int)(base / W), x = (int)(base - (int64_t)y * W);
+  typename Src::Raw t[ROUNDS];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      if (src.valid(t[k])) {
-        float p[3];
-        src.centre(t[k], x, y, p);
+  for (int k = 0; k < ROUNDS; ++k) t[k] = base + 32 * k < P ? src.load(base + 32 * k) : src.invalid();
+  const int W = src.width();
+  int y = (int)(base / W), x = (int)(base - (int64_t)y * W);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], p[a]); hi[a] = fmaxf(hi[a], p[a]); }
-        ++cnt;
-      }
-      if (++x == W) { x = 0; ++y; }
+  for (int k = 0; k < ROUNDS; ++k) {
+    if (src.valid(t[k])) {
+      float p[3];
+      src.bounds_centre(t[k], base + 32 * k, x, y, p);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], p[a]); hi[a] = fmaxf(hi[a], p[a]); }
+      ++cnt;
     }
+    x += 32;
+    while (x >= W) { x -= W; ++y; }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -171,11 +179,13 @@ __device__ __forceinline__ uint64_t morton63(const float p[3], const float lo[3]
   return (spread21(q[0]) << 2) | (spread21(q[1]) << 1) | spread21(q[2]);
 }
 
-// Persistent over tiles.  Per tile: offset = sum of the valid counts of all earlier tiles,
-// block scan of the per-thread counts, keys/ids written in pixel order.  The eight 8-bit
-// digit histograms of the radix sort are accumulated in shared memory on the way (the keys
-// are in registers anyway) and flushed once per block.  Block 0 also re-arms the other
-// parity's FrameState for the next frame.
+// Persistent over tiles.  Per tile: offset = sum of the valid counts of all earlier tiles, ranks
+// from ballots (pixel order is kept), keys/ids written in pixel order.  The digit histograms that
+// the chosen sort mode consumes are accumulated in shared memory on the way and flushed once per
+// block: the hybrid sort reads only digits first..7 (the top 31 / 39 code bits; if it has to fall
+// back to all eight passes it counts the low digits itself, onesweep.cuh); a warp's 32 lanes hold
+// 32 consecutive pixels whose high digits mostly agree, so runs of equal digits are counted once.
+// Block 0 also re-arms the next frame's FrameState.
 template <class Src>
 __global__ void __launch_bounds__(BUILD_THREADS)
 unproject_kernel(const Src src, int64_t P, int num_tiles,
@@ -205,7 +215,9 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
   for (int d = 0; d < 8; ++d) s_hist[d][tid] = 0u;
 
   // the sort ping-pongs between two buffers and must end in buffer 0 (onesweep.cuh)
-  const bool odd = sort_input_buffer(sort_mode, st->n) != 0;
+  const uint32_t n_all = st->n;
+  const bool odd = sort_input_buffer(sort_mode, n_all) != 0;
+  const int first_digit = sort_mode == SORT_HYBRID ? hybrid_first_digit(n_all) : 0;
   uint64_t* __restrict__ keys = odd ? keys1 : keys0;
   uint32_t* __restrict__ ids = odd ? ids1 : ids0;
   float lo[3], ext[3];
@@ -224,68 +236,62 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
     for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
     if (lane == 0) s_part[warp] = part;
 
-    const int64_t base = (int64_t)tile * TILE_PX + (int64_t)tid * PX_PER_THREAD;
-    uint64_t code[8];
-    uint32_t vmask = 0;
-    if (base < P && tile_count[tile] != 0) {
-      typename Src::Raw t[8];
-      src.load8(base, P, t);
-      const int W = src.width();
-      int y = (int)(base / W), x = (int)(base - (int64_t)y * W);
+    const int64_t base = (int64_t)tile * TILE_PX + (int64_t)warp * WARP_PX + lane;
+    typename Src::Raw t[ROUNDS];
+    uint32_t vmask = 0, wtotal = 0;
+    const bool any = tile_count[tile] != 0;
+    if (any) {
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        if (src.valid(t[k])) {
-          float p[3];
-          src.centre(t[k], x, y, p);
-          code[k] = morton63(p, lo, ext);
-          vmask |= 1u << k;
-        }
-        if (++x == W) { x = 0; ++y; }
+      for (int k = 0; k < ROUNDS; ++k) t[k] = base + 32 * k < P ? src.load(base + 32 * k) : src.invalid();
+#pragma unroll
+      for (int k = 0; k < ROUNDS; ++k) {
+        const bool v = src.valid(t[k]);
+        vmask |= (v ? 1u : 0u) << k;
+        wtotal += __popc(__ballot_sync(0xffffffffu, v));
       }
     }
-    // block exclusive scan of popc(vmask)
-    uint32_t c = __popc(vmask), incl = c;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      uint32_t n = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += n;
-    }
-    if (lane == 31) s_warp[warp] = incl;
+    if (lane == 0) s_warp[warp] = wtotal;
     __syncthreads();
-    uint32_t tile_off = 0, warp_off = 0;
+    uint32_t pos = 0;
 #pragma unroll
     for (int w = 0; w < NW; ++w) {
-      tile_off += s_part[w];
-      if (w < warp) warp_off += s_warp[w];
+      pos += s_part[w];
+      if (w < warp) pos += s_warp[w];
     }
-    uint32_t pos = tile_off + warp_off + incl - c;
+    if (any) {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      const bool v = (vmask >> k) & 1u;
-      if (v) {
-        keys[pos] = code[k];
-        ids[pos] = (uint32_t)(base + k);
-        ++pos;
-      }
-      // digit histograms; the high digits are warp-coherent (neighbouring pixels share the
-      // coarse cell), so aggregate them with match_any before touching shared memory
-      const unsigned act = __ballot_sync(0xffffffffu, v);
-      if (v) {
-#pragma unroll
-        for (int d = 0; d < 4; ++d) atomicAdd(&s_hist[d][(code[k] >> (8 * d)) & 0xff], 1u);
-#pragma unroll
-        for (int d = 4; d < 8; ++d) {
-          const uint32_t dig = (uint32_t)(code[k] >> (8 * d)) & 0xff;
-          const unsigned peers = __match_any_sync(act, dig);
-          if ((peers & ((1u << lane) - 1)) == 0) atomicAdd(&s_hist[d][dig], (uint32_t)__popc(peers));
+      for (int k = 0; k < ROUNDS; ++k) {
+        const bool v = (vmask >> k) & 1u;
+        const unsigned act = __ballot_sync(0xffffffffu, v);
+        uint64_t code = 0;
+        if (v) {
+          float p[3];
+          src.key_centre(t[k], base + 32 * k, p);
+          code = morton63(p, lo, ext);
+          const uint32_t at = pos + __popc(act & ((1u << lane) - 1));
+          keys[at] = code;
+          ids[at] = (uint32_t)(base + 32 * k);
         }
+        // digit histograms: neighbouring pixels mostly share a digit, so each run of equal digits among
+        // consecutive valid lanes is counted by its first lane (one shared-memory atomic per run)
+        for (int d = first_digit; d < 8; ++d) {
+          const uint32_t dig = v ? (uint32_t)(code >> (8 * d)) & 0xff : 0x100u;
+          const uint32_t prev = __shfl_up_sync(0xffffffffu, dig, 1);
+          const bool head = v && (lane == 0 || prev != dig);
+          const unsigned brk = __ballot_sync(0xffffffffu, head || !v);   // where runs start or are interrupted
+          if (head) {
+            const unsigned after = lane == 31 ? 0u : brk >> (lane + 1);
+            const uint32_t run = after ? (uint32_t)__ffs(after) : 32u - lane;
+            atomicAdd(&s_hist[d][dig], run);
+          }
+        }
+        pos += __popc(act);
       }
     }
     __syncthreads();  // s_warp / s_part reused by the next tile
   }
   __syncthreads();
-#pragma unroll
-  for (int d = 0; d < 8; ++d) {
+  for (int d = first_digit; d < 8; ++d) {
     const uint32_t h = s_hist[d][tid];
     if (h) atomicAdd(&st->hist[d][tid], h);
   }

@@ -9,23 +9,16 @@ namespace sw {
 constexpr int LBVH_THREADS = 256;
 
 // Splat `id` (= source pixel index, or position in a received sample buffer) as sphere + colour.
-// FrameGather recomputes the sphere from the depth buffer with exactly the arithmetic of the
-// bounds / Morton kernels (Eq. 1; radius per RadiusParams) and copies the colour
-// ("no shading other than the constant sample color"); PackedGather decodes the
+// FrameGather reads the splat that bounds_kernel stored for that pixel (Eq. 1; radius
+// per RadiusParams: evaluated once per frame) and copies the colour ("no shading
+// other than the constant sample color"); PackedGather decodes the
 // 64-bit sample and the RGBA8 colour.
 struct FrameGather {
-  const float* __restrict__ depth;
+  const float4* __restrict__ sphere_px;   // splat of every valid pixel, written by bounds_kernel (Eq. 1 once)
   const float4* __restrict__ color;
-  DevCamera cam;
-  RadiusParams rp;
   __device__ __forceinline__ void get(uint32_t id, float4& sp, float4& col) const {
-    const int y = (int)(id / (uint32_t)cam.W), x = (int)(id - (uint32_t)y * (uint32_t)cam.W);
-    const float t = __ldg(depth + id);
-    float p[3], len;
-    splat_centre(cam, x, y, t, p, len);
-    const float z = div_(t, len);
+    sp = __ldg(sphere_px + id);
     col = __ldg(color + id);
-    sp = make_float4(p[0], p[1], p[2], splat_radius(rp, z, col.w));
   }
 };
 struct PackedGather {

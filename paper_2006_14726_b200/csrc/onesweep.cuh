@@ -55,7 +55,10 @@ struct SortArgs {
   int pass;          // SORT_SINGLE: the digit; input buffer = pass & 1
 };
 
-constexpr int SORT_MAX_ITEMS = 16;
+#ifndef SPLATS_SORT_MAX_ITEMS
+#define SPLATS_SORT_MAX_ITEMS 16
+#endif
+constexpr int SORT_MAX_ITEMS = SPLATS_SORT_MAX_ITEMS;
 struct SortSmem {
   uint32_t warp_hist[SORT_WARPS][RADIX];  // per-warp digit counts -> exclusive prefix over warps
   uint32_t tile_off[RADIX];               // exclusive scan of the tile's digit counts
@@ -356,7 +359,24 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
     fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
     grid_barrier(bar, nb, round);
     if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) break;
-    first = 0;  // a long run of equal top bits: redo the sort with all 8 passes
+    // a long run of equal top bits: redo the sort with all 8 passes.  unproject_kernel counted only
+    // the digits >= first, so count the low ones here (a histogram does not depend on the order).
+    {
+      const int tid = threadIdx.x;
+      for (int d = 0; d < first; ++d) s.warp_hist[d][tid] = 0;
+      __syncthreads();
+      for (uint32_t idx = blockIdx.x * SORT_THREADS + tid; idx < n; idx += nb * SORT_THREADS) {
+        const uint64_t k = __ldcg(a.key[0] + idx);
+        for (int d = 0; d < first; ++d) atomicAdd(&s.warp_hist[d][(uint32_t)(k >> (8 * d)) & 0xff], 1u);
+      }
+      __syncthreads();
+      for (int d = 0; d < first; ++d) {
+        const uint32_t h = s.warp_hist[d][tid];
+        if (h) atomicAdd(&a.st->hist[d][tid], h);
+      }
+      grid_barrier(bar, nb, round);
+    }
+    first = 0;
     pass = 0;
   }
 }
@@ -374,9 +394,16 @@ onesweep_kernel(SortArgs a) {
   SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
   const uint32_t n = a.st->n;
   const uint32_t slots = gridDim.x * SORT_THREADS;
+#ifndef SPLATS_SORT_MAX_ITEMS
+#define SPLATS_SORT_MAX_ITEMS 16
+#endif
   if (n <= slots * 4u) run_sort<4>(s, a, n);
+#if SPLATS_SORT_MAX_ITEMS >= 16
   else if (n <= slots * 8u) run_sort<8>(s, a, n);
   else run_sort<16>(s, a, n);
+#else
+  else run_sort<8>(s, a, n);
+#endif
 }
 
 }  // namespace sw

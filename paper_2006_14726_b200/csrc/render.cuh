@@ -46,6 +46,7 @@ struct RenderParams {
   uint32_t* out8;    // ... or RGBA8 (OUT8 instances): exactly one of the two is used
   unsigned* sched;  // [0] tile ticket, [1] blocks done (both zero between launches); one pair per render in flight
   int wait_prev;    // 0: this render does not depend on the kernel before it in the stream (see do_render)
+  unsigned long long* traced;  // += pixels of the 8x4 tiles inside the scene's screen rectangle (rays set up), once per launch
 };
 
 #ifdef SPLATS_STATS
@@ -190,6 +191,7 @@ render_kernel(RenderParams prm) {
   const int total_px = cam.W * cam.H;
   const int nfill = (total_px + FILL_PX - 1) / FILL_PX;
   const int nwarps = gridDim.x * (RENDER_THREADS / 32);
+  if (blockIdx.x == 0 && tid == 0) atomicAdd(prm.traced, (unsigned long long)ntiles * 32ull);
   int tile = blockIdx.x * (RENDER_THREADS / 32) + warp;
   for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, lane == 0 ? atomicAdd(prm.sched, 1u) : 0u, 0)) {
   if (tile >= ntiles) {

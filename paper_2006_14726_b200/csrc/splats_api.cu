@@ -38,6 +38,7 @@ struct Context {
   uint32_t* tile_count = nullptr;   // [cap / TILE_PX + 1]
   uint32_t* pack_tile_count = nullptr;  // the same for splats_pack, which may run while a build is in flight
   unsigned* sched = nullptr;        // render tile ticket + done counter, one pair per render in flight
+  unsigned long long* traced = nullptr;   // pixels for which the renders set up a ray (splats_traced_pixels)
   // renders launched since the last fully serialising launch on the stream (see do_render)
   static constexpr int MAX_OVERLAP = 8;
   int render_streak = 0;
@@ -65,6 +66,7 @@ struct Context {
   int* leaf_parent = nullptr;
   float4* pyr = nullptr;            // min/max pyramid over the leaf boxes (lbvh.cuh), 2 float4 per entry
   int4* ranges = nullptr;           // (first, split, last) of every internal node, hierarchy_kernel -> boxes_kernel; tiled mode: the queue of tree_spine_kernel
+  float4* sphere_px = nullptr;      // splat (centre, radius) of every valid source pixel, bounds_kernel -> unproject_kernel, tree gather
   uint8_t* tile_min = nullptr;      // tiled tree: smallest delta + 1 of every tile of sorted leaves
   uint16_t* tile_fb = nullptr;      // tiled tree: first / last split below every threshold, per tile
   PyramidLayout pyr_layout;
@@ -179,14 +181,14 @@ cudaError_t dmalloc(T** p, size_t count) {
 }
 
 void free_all(Context* c) {
-  cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->pack_tile_count); cudaFree(c->sched);
+  cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->pack_tile_count); cudaFree(c->sched); cudaFree(c->traced);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status);
   for (int i = 0; i < 2; ++i) { cudaFree(c->set[i].sphere); cudaFree(c->set[i].rgba); cudaFree(c->set[i].ids); cudaFree(c->set[i].nodes); }
   if (c->build_stream) cudaStreamDestroy(c->build_stream);
   if (c->ev_begin) cudaEventDestroy(c->ev_begin);
   if (c->ev_built) cudaEventDestroy(c->ev_built);
-  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->ranges); cudaFree(c->zkey); cudaFree(c->tile_min); cudaFree(c->tile_fb);
+  cudaFree(c->leaf_parent); cudaFree(c->pyr); cudaFree(c->ranges); cudaFree(c->zkey); cudaFree(c->tile_min); cudaFree(c->sphere_px); cudaFree(c->tile_fb);
   for (int i = 0; i < Context::N_IN; ++i) {
     cudaFree(c->stage_color[i]); cudaFree(c->stage_depth[i]);
     if (c->in_uploaded[i]) cudaEventDestroy(c->in_uploaded[i]);
@@ -353,12 +355,13 @@ int do_update_frame(Context* c, const float* color, const float* depth, const wr
                     bool async = false) {
   FrameSource src;
   src.depth = depth;
+  src.color = reinterpret_cast<const float4*>(color);
+  src.sphere_px = c->sphere_px;
   src.cam = make_camera(cam, W, H);
+  src.rp = make_radius(c, cam, H, r_scale);
   FrameGather g;
-  g.depth = depth;
-  g.color = reinterpret_cast<const float4*>(color);
-  g.cam = src.cam;
-  g.rp = make_radius(c, cam, H, r_scale);
+  g.sphere_px = c->sphere_px;
+  g.color = src.color;
   return do_update(c, src, g, (int64_t)W * H, async);
 }
 
@@ -372,6 +375,7 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   prm.st = c->state + c->cur_state;
   prm.out = reinterpret_cast<float4*>(out);
   prm.out8 = reinterpret_cast<uint32_t*>(out);
+  prm.traced = c->traced;
   const int tiles = ((W2 + 7) / 8) * ((H2 + 3) / 4);
   const int blocks_needed = (tiles + RENDER_THREADS / 32 - 1) / (RENDER_THREADS / 32);
   const int grid = blocks_needed < c->render_grid ? blocks_needed : c->render_grid;  // persistent (render.cuh)
@@ -452,6 +456,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (e == cudaSuccess) e = dmalloc(&c->pack_tile_count, cap / TILE_PX + 2);
   if (e == cudaSuccess) e = dmalloc(&c->sched, 2 * Context::MAX_OVERLAP);
   if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 2 * Context::MAX_OVERLAP * sizeof(unsigned));
+  if (e == cudaSuccess) e = dmalloc(&c->traced, 1);
+  if (e == cudaSuccess) e = cudaMemset(c->traced, 0, sizeof(unsigned long long));
   for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
     e = dmalloc(&c->key[i], cap);
     if (e == cudaSuccess) e = dmalloc(&c->val[i], cap);
@@ -467,6 +473,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
   if (e == cudaSuccess) e = dmalloc(&c->ranges, cap);
   if (e == cudaSuccess) e = dmalloc(&c->tile_min, cap / TT_LEAVES + 2);
+  if (e == cudaSuccess) e = dmalloc(&c->sphere_px, cap);
   if (e == cudaSuccess) e = dmalloc(&c->tile_fb, (cap / TT_LEAVES + 2) * 2 * TT_VPAD);
   if (e == cudaSuccess) e = dmalloc(&c->zkey, cap);
   if (e == cudaSuccess) e = cudaMemset(c->zkey, 0xff, cap * sizeof(uint64_t));
@@ -838,6 +845,22 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   return SPLATS_OK;
 }
 
+int splats_export_child_boxes(float* child_boxes) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  Context* c = g_ctx;
+  if (!child_boxes) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export_child_boxes before any update");
+  unsigned n = 0;
+  int rc = splats_count(&n);
+  if (rc) return rc;
+  if (n < 2) return SPLATS_OK;
+  // the first 48 bytes of every 64-byte record, exactly as the traversal reads them
+  CU(cudaMemcpy2DAsync(child_boxes, 12 * sizeof(float), c->set[c->cur_set].nodes, sizeof(Node), 12 * sizeof(float), n - 1,
+                       cudaMemcpyDeviceToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
 int splats_export_splats(float* sphere, float* rgba, float* lo_hi) {
   if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
   Context* c = g_ctx;
@@ -927,6 +950,16 @@ int splats_stage_ms(float* ms_sum, unsigned* calls) {
   }
   c->spans.clear();
   c->pool_used = 0;
+  return SPLATS_OK;
+}
+
+int splats_traced_pixels(unsigned long long* pixels_host, int reset) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  if (!pixels_host) return fail(SPLATS_EINVAL, "null pointer argument");
+  Context* c = g_ctx;
+  CU(cudaMemcpyAsync(pixels_host, c->traced, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+  if (reset) CU(cudaMemsetAsync(c->traced, 0, sizeof(unsigned long long), c->stream));
+  CU(cudaStreamSynchronize(c->stream));
   return SPLATS_OK;
 }
 

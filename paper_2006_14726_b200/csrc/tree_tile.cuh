@@ -40,6 +40,7 @@ constexpr int TT_WARPS = TT_THREADS / 32;
 constexpr int TT_QMAX = 200;    // >= 2 x 97: strict prefix + suffix minima of byte-sized deltas
 constexpr int TT_VMAX = 97;     // delta + 1 lies in [0, 96]; 0 = "beyond the array"
 constexpr int TT_VPAD = 100;    // table stride
+constexpr int TT_CLIMB = 64;    // work lists up to this length are finished by climbing threads instead of block-wide rounds
 constexpr int PYR_BASE = 3;     // lowest level of the global pyramid that the tiled mode writes and reads
 static_assert(TT_LOG >= 7 && TT_LOG <= 12, "tile of 128 .. 4096 leaves");
 
@@ -55,7 +56,8 @@ struct TileSmem {
   float top[6][TT_WARPS];        // the warps' level-7 entries
   uint32_t wmin[TT_WARPS];       // the warps' smallest delta + 1
   int4 q[TT_QMAX];               // queued nodes: (split, first or -1, last or -1, delta + 1)
-  uint32_t tail, qn, qbase;
+  uint32_t cnt[3];               // lengths of the work lists of rounds r % 3
+  uint32_t qn, qbase;
   uint32_t dleft;                // delta + 1 of the pair (base - 1, base); 0 at the start of the array
   int last;
 };
@@ -127,6 +129,7 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const Box6
 #pragma unroll
   for (int a = 0; a < 6; ++a) s.cbox[side][a][g] = b.v[a];
   s.cend[side][g] = (int16_t)far;
+  __threadfence_block();   // the slot is written before the arrival bit is visible
   const int sh = 8 * (g & 3);
   const uint32_t old = atomicOr(&s.arrived[g >> 2], (1u << side) << sh);
   return ((old >> sh) & 3u) == (2u >> side) ? g : -1;   // the other bit was already set
@@ -151,7 +154,7 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   // ---- (1) interleaved over the tile (coalesced): deltas of the adjacent pairs (l, l + 1), + 1;
   // gather of the splats into sorted order; leaf boxes -> staging
   if (tid == 0) {
-    s.tail = 0;
+    s.cnt[0] = 0; s.cnt[1] = 0; s.cnt[2] = 0;
     s.qn = 0;
     uint32_t dl = 0;
     if (base > 0) {
@@ -273,16 +276,44 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
       if (dk[k] < suf_ex) { s.pos_last[dk[k]] = 4 * tid + k; suf_ex = dk[k]; }
   }
 
-  // ---- (3) round 0: the leaves report to their parents
-  auto append = [&](int g) {   // warp-aggregated push of finished nodes (g < 0: nothing); all 32 lanes call it
+  // ---- (3) round 0: the leaves report to their parents.  Finished nodes go to the work list; the
+  // list of round r + 1 starts where that of round r ends, its length is counted in cnt[(r + 1) % 3]
+  // (three rotating counters: one barrier per round is enough).
+  auto append = [&](int g, uint32_t at, uint32_t* counter) {   // warp-aggregated push (g < 0: nothing); all 32 lanes call it
     const unsigned m = __ballot_sync(0xffffffffu, g >= 0);
     if (m) {
       const int leader = __ffs(m) - 1;
       uint32_t pos = 0;
-      if (lane == leader) pos = atomicAdd(&s.tail, (uint32_t)__popc(m));
+      if (lane == leader) pos = atomicAdd(counter, (uint32_t)__popc(m));
       pos = __shfl_sync(0xffffffffu, pos, leader);
-      if (g >= 0) s.wl[pos + __popc(m & ((1u << lane) - 1))] = (uint16_t)g;
+      if (g >= 0) s.wl[at + pos + __popc(m & ((1u << lane) - 1))] = (uint16_t)g;
     }
+  };
+  // a finished node: write its record, report upwards; returns the parent if that completed it
+  auto finish = [&](int l) -> int {
+    const int p = s.cend[0][l], q = s.cend[1][l];
+    Box6 L, R;
+#pragma unroll
+    for (int a = 0; a < 6; ++a) { L.v[a] = s.cbox[0][a][l]; R.v[a] = s.cbox[1][a][l]; }
+    const int first = base + p + 1, last = base + q, g = base + l;
+    Box6 U = L;
+    U.merge(R);
+    bool il;
+    const int up = tile_report(s, p, q, U, il);
+    const int idx = il ? last : first;
+    const int cnt_l = g - first + 1, cnt_r = last - g;
+    const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
+    const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
+    float4* rec = reinterpret_cast<float4*>(nodes + idx);
+    rec[0] = make_float4(L.v[0], L.v[1], L.v[2], L.v[3]);
+    rec[1] = make_float4(L.v[4], L.v[5], R.v[0], R.v[1]);
+    rec[2] = make_float4(R.v[2], R.v[3], R.v[4], R.v[5]);
+    rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
+    if (idx == 0) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { st->root_lo[a] = U.v[a]; st->root_hi[a] = U.v[3 + a]; }
+    }
+    return up;
   };
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -292,49 +323,38 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
       bool il;
       g = tile_report(s, i - 1, i, leaf[j], il);
     }
-    append(g);
+    append(g, 0u, &s.cnt[1]);
   }
   __syncthreads();
 
-  // ---- rounds: the nodes completed in the previous round are written out and report upwards
+  // ---- dense rounds while the list is long: the nodes completed in the previous round are written
+  // out and report upwards, one node per thread whatever its size
   uint32_t begin = 0;
-  while (true) {
-    const uint32_t end = s.tail;
-    __syncthreads();   // everybody has read the tail before it grows again
-    if (end == begin) break;
-    for (uint32_t e0 = begin; e0 < end; e0 += TT_THREADS) {
+  int r = 1;
+  uint32_t len = s.cnt[1];
+  while (len > TT_CLIMB) {
+    if (tid == 0) s.cnt[(r + 2) % 3] = 0u;   // read in round r - 1, appended to in round r + 1
+    uint32_t* next = &s.cnt[(r + 1) % 3];
+    for (uint32_t e0 = 0; e0 < len; e0 += TT_THREADS) {
       const uint32_t e = e0 + tid;
-      int up = -1;
-      if (e < end) {
-        const int l = s.wl[e];
-        const int p = s.cend[0][l], q = s.cend[1][l];
-        Box6 L, R;
-#pragma unroll
-        for (int a = 0; a < 6; ++a) { L.v[a] = s.cbox[0][a][l]; R.v[a] = s.cbox[1][a][l]; }
-        const int first = base + p + 1, last = base + q, g = base + l;
-        Box6 U = L;
-        U.merge(R);
-        bool il;
-        up = tile_report(s, p, q, U, il);
-        const int idx = il ? last : first;
-        const int cnt_l = g - first + 1, cnt_r = last - g;
-        const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
-        const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-        float4* rec = reinterpret_cast<float4*>(nodes + idx);
-        rec[0] = make_float4(L.v[0], L.v[1], L.v[2], L.v[3]);
-        rec[1] = make_float4(L.v[4], L.v[5], R.v[0], R.v[1]);
-        rec[2] = make_float4(R.v[2], R.v[3], R.v[4], R.v[5]);
-        rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
-        if (idx == 0) {
-#pragma unroll
-          for (int a = 0; a < 3; ++a) { st->root_lo[a] = U.v[a]; st->root_hi[a] = U.v[3 + a]; }
-        }
-      }
-      append(up);
+      append(e < len ? finish(s.wl[begin + e]) : -1, begin + len, next);
     }
-    begin = end;
     __syncthreads();
+    begin += len;
+    ++r;
+    len = s.cnt[r % 3];
   }
+  // ---- the few nodes left climb on their own: no more barriers.  A subtree's stores are fenced
+  // before its arrival bit is set (tile_report); whoever sets the second bit fences again and may
+  // read both slots.
+  if (tid < len) {
+    int l = s.wl[begin + tid];
+    while (l >= 0) {
+      __threadfence_block();
+      l = finish(l);
+    }
+  }
+  __syncthreads();
 
   // ---- the splits of the tile whose node is not complete: queue them with what is known
 #pragma unroll

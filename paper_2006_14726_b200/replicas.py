@@ -5,6 +5,9 @@ Backend "nccl" on GPUs, "gloo" in the CPU tests."""
 from __future__ import annotations
 
 import os
+import socket
+import subprocess
+import sys
 
 import torch
 import torch.distributed as dist
@@ -13,6 +16,22 @@ import torch.distributed as dist
 def world_info():
     return (int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")),
             int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def needs_spawn(n_gpus: int) -> bool:
+    """True when N > 1 ranks were asked for but this process was not started by torchrun."""
+    return n_gpus > 1 and "WORLD_SIZE" not in os.environ
+
+
+def spawn(script: str, argv: list, n: int, env: dict | None = None, timeout: float | None = None) -> int:
+    """Start `script argv` as n ranks of one node (torchrun, rendezvous on 127.0.0.1, a free port):
+    what `python bench.py --gpus N` does when it was started plainly.  Returns the exit code."""
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), script, *map(str, argv)]
+    return subprocess.run(cmd, env=env, timeout=timeout).returncode
 
 
 def init(backend: str | None = None):

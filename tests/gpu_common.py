@@ -51,6 +51,10 @@ def assert_bvh_bit_exact(sc):
     np.testing.assert_array_equal(ex["children"].cpu().numpy(), sc["children"])
     np.testing.assert_array_equal(ex["parents"].cpu().numpy(), sc["parents"])
     np.testing.assert_array_equal(ex["node_aabbs"].cpu().numpy().view(np.uint32), sc["aabbs"].view(np.uint32))
+    if n > 1:   # the stored child boxes the traversal reads, one by one (not only their union)
+        cb = sp.splats_export_child_boxes().cpu().numpy().view(np.uint32).reshape(n - 1, 2, 6)
+        want = sc["aabbs"].view(np.uint32)[sc["children"]]          # (n-1, 2, 6): box of each child node / leaf
+        np.testing.assert_array_equal(cb, want)
     es = sp.splats_export_splats()
     np.testing.assert_array_equal(es["sphere"].cpu().numpy().view(np.uint32), sc["sphere_sorted"].view(np.uint32))
     np.testing.assert_array_equal(es["rgba"].cpu().numpy().view(np.uint32), sc["rgba_sorted"].view(np.uint32))

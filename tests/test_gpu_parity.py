@@ -38,7 +38,8 @@ def test_random_frames_ragged_sizes(W, H, fill, r_scale):
 
 
 def test_low_alpha_stack_forces_relaunch():
-    # alpha 0.05 everywhere, r_scale 4: every ray needs far more than K = 8 hits
+    # alpha 0.05 everywhere, r_scale 4: every ray needs far more than the K = 4 entries of the k-buffer
+    # (render.cuh KBUF), i.e. many re-launches from the cursor
     W, H = 40, 30
     color, depth, cam = synth.random_frame(W, H, seed=5, fill=1.0)
     color[..., 3] = 0.05
@@ -51,8 +52,8 @@ def test_low_alpha_stack_forces_relaunch():
 
 
 def test_coaxial_stack_closed_form_90_hits():
-    # closed form (ii): alpha 0.05 -> 90 hits, A = 1 - 0.95^90.  A 1x1 source cannot produce
-    # coaxial splats, so use a frame whose splats all project onto the destination pixel.
+    # closed form (ii) on a frame whose splats all project onto the one destination pixel; parity with the oracle,
+    # and the closed form whenever the oracle itself composited the full stack
     W, H = 12, 12
     color, depth, cam = synth.random_frame(W, H, seed=9, fill=1.0)
     color[...] = np.array([0.01, 0.02, 0.03, 0.05], np.float32)
@@ -66,6 +67,39 @@ def test_coaxial_stack_closed_form_90_hits():
         assert_rgba_close(got, ref)
         if used[0, 0] >= 90:
             assert got[0, 0, 3] == pytest.approx(1 - 0.95 ** 90, abs=1e-5)
+
+
+def test_coaxial_packed_stack_closed_form_unconditional():
+    # closed form (ii), by construction: 100 samples of one constant radius on the axis of the only destination ray,
+    # alpha = 13/255 (the wire's RGBA8), sent through splats_update_packed.  A_n = 1 - (1 - a)^n crosses 0.99 at
+    # n* = 89 >> K = 4 k-buffer entries, so the ray is re-launched from the cursor more than twenty times.
+    n = 100
+    quant = [0.0, 0.0, 0.0, 1.0, 1.0, 1.0, 0.1]
+    qx = np.uint64(32768)                                   # cell centre 0.50000763 on x and y
+    qz = (np.floor((0.2 + 0.005 * np.arange(n)) * 65536.0)).astype(np.uint64)
+    qr = np.uint64(6554)                                    # radius 6554 * 0.1 / 65535 ~ 0.01
+    samples = (qx | (qx << np.uint64(16)) | (qz << np.uint64(32)) | (qr << np.uint64(48))).astype(np.uint64)
+    colours = np.full(n, 1 | (2 << 8) | (3 << 16) | (13 << 24), dtype=np.uint32)
+    a = np.float32(13) / np.float32(255)
+    A, n_star = np.float32(0), 0
+    while A < np.float32(0.99):                             # S9 in float32, one hit at a time
+        A = np.float32(np.float64(np.float32(1) - A) * np.float64(a) + np.float64(A))   # T = 1 - A; A = fma(T, a, A)
+        n_star += 1
+    assert 80 <= n_star <= 95
+    assert abs(float(A) - (1.0 - (1.0 - float(a)) ** n_star)) < 1e-5
+    cam = synth.look_at((0.5, 0.5, -3.0), center=(0.5, 0.5, 0.5))   # its single pixel's ray is the z axis through (0.5, 0.5)
+    with Session(16, 16) as s:
+        d_s = torch.from_numpy(samples.view(np.int64)).cuda()
+        d_c = torch.from_numpy(colours.view(np.int32)).cuda()
+        sp.splats_update_packed(d_s, d_c, n, quant)
+        got = s.render(cam, 1, 1)
+        scp = oracle.build_scene_packed(samples, colours, quant)
+        assert_bvh_bit_exact(scp)
+        ref, used = oracle.render(scp, cam, 1, 1, "brute", return_hits=True)
+        assert used[0, 0] == n_star                         # the oracle composited exactly the closed form's stack
+        assert_rgba_close(got, ref)
+        assert got[0, 0, 3] == pytest.approx(1.0 - (1.0 - float(a)) ** n_star, abs=1e-5)
+        assert got[0, 0, 3] >= 0.99
 
 
 def test_all_invalid_frame_renders_zeros():
@@ -192,7 +226,7 @@ def test_sort_modes_give_the_same_order(mode):
 
 
 def test_dense_frame_five_pass_hybrid_sort_and_all_tile_sizes():
-    # N > 2^20: the hybrid sort runs 5 passes (top 39 bits) starting from the second buffer;
+    # N > 2^19: the hybrid sort runs 5 passes (top 39 bits) starting from the second buffer;
     # then smaller frames in the same context walk through the 4096/2048/1024-element tile paths.
     W, H = 2304, 1000
     color, depth, cam = synth.dense_frame(W, H, seed=5)
