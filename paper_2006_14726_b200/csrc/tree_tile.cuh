@@ -62,6 +62,10 @@ struct TileSmem {
   int last;
 };
 
+// Slot of split l in cbox / cend during the rounds: XOR swizzle, so that the power-of-two strides
+// the work lists start with (4 leaves per thread, every other split finished) hit 32 different banks.
+__device__ __forceinline__ int tt_slot(int l) { return l ^ ((l >> 5) & 31); }
+
 struct Box6 {
   float v[6];
   __device__ __forceinline__ void init() {
@@ -126,9 +130,10 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const Box6
   int g, side, far;
   if (is_last) { g = q; side = 0; far = p; }
   else { if (p < 0) return -1; g = p; side = 1; far = q; }
+  const int gs = tt_slot(g);
 #pragma unroll
-  for (int a = 0; a < 6; ++a) s.cbox[side][a][g] = b.v[a];
-  s.cend[side][g] = (int16_t)far;
+  for (int a = 0; a < 6; ++a) s.cbox[side][a][gs] = b.v[a];
+  s.cend[side][gs] = (int16_t)far;
   __threadfence_block();   // the slot is written before the arrival bit is visible
   const int sh = 8 * (g & 3);
   const uint32_t old = atomicOr(&s.arrived[g >> 2], (1u << side) << sh);
@@ -291,10 +296,11 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   };
   // a finished node: write its record, report upwards; returns the parent if that completed it
   auto finish = [&](int l) -> int {
-    const int p = s.cend[0][l], q = s.cend[1][l];
+    const int ls = tt_slot(l);
+    const int p = s.cend[0][ls], q = s.cend[1][ls];
     Box6 L, R;
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { L.v[a] = s.cbox[0][a][l]; R.v[a] = s.cbox[1][a][l]; }
+    for (int a = 0; a < 6; ++a) { L.v[a] = s.cbox[0][a][ls]; R.v[a] = s.cbox[1][a][ls]; }
     const int first = base + p + 1, last = base + q, g = base + l;
     Box6 U = L;
     U.merge(R);
@@ -364,7 +370,7 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
     const uint32_t arr = (s.arrived[l >> 2] >> (8 * (l & 3))) & 3u;
     if (arr == 3u) continue;
     const uint32_t slot = atomicAdd(&s.qn, 1u);
-    s.q[slot] = make_int4(g, (arr & 1u) ? base + s.cend[0][l] + 1 : -1, (arr & 2u) ? base + s.cend[1][l] : -1, (int)s.d[l]);
+    s.q[slot] = make_int4(g, (arr & 1u) ? base + s.cend[0][tt_slot(l)] + 1 : -1, (arr & 2u) ? base + s.cend[1][tt_slot(l)] : -1, (int)s.d[l]);
   }
   __syncthreads();
   const uint32_t qn = s.qn;
