@@ -201,6 +201,20 @@ __device__ __forceinline__ void st_volatile_u64(uint64_t* p, uint64_t v) {
   asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// 256-bit global accesses (sm_100): one request per 32 bytes instead of two, which halves the L1
+// wavefronts of divergent 64-byte node fetches and scattered node writes.  32-byte aligned.
+struct f8 { float v[8]; };
+__device__ __forceinline__ f8 ldg_f8(const void* p) {   // read-only path (LDG.E.256.CONSTANT)
+  f8 r;
+  asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+      : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]), "=f"(r.v[4]), "=f"(r.v[5]), "=f"(r.v[6]), "=f"(r.v[7]) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg_f8(void* p, const f8& r) {
+  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "l"(p), "f"(r.v[0]), "f"(r.v[1]), "f"(r.v[2]), "f"(r.v[3]), "f"(r.v[4]), "f"(r.v[5]), "f"(r.v[6]), "f"(r.v[7]) : "memory");
+}
+
 __device__ __forceinline__ float4 ldg_stream_f4(const float4* p) {  // read-once data: do not keep in L1
   float4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"

@@ -257,10 +257,11 @@ render_kernel(RenderParams prm) {
 
       uint32_t node = n == 1 ? leaf_range_code(0u, 1u) : 0u;
       while (true) {
-        // ---- internal nodes: both child boxes come with the node (4 x 16-byte loads)
+        // ---- internal nodes: both child boxes come with the node (2 x 32-byte loads)
         while ((int)node >= 0) {
-          const float4* np = reinterpret_cast<const float4*>(prm.nodes + node);
-          const float4 n0 = __ldg(np), n1 = __ldg(np + 1), n2 = __ldg(np + 2), n3 = __ldg(np + 3);
+          const f8 ra = ldg_f8(prm.nodes + node), rb = ldg_f8(reinterpret_cast<const char*>(prm.nodes + node) + 32);
+          const float4 n0 = make_float4(ra.v[0], ra.v[1], ra.v[2], ra.v[3]), n1 = make_float4(ra.v[4], ra.v[5], ra.v[6], ra.v[7]);
+          const float4 n2 = make_float4(rb.v[0], rb.v[1], rb.v[2], rb.v[3]), n3 = make_float4(rb.v[4], rb.v[5], rb.v[6], rb.v[7]);
           STAT_ADD(0, 1);
           STAT_MAX(5, sp);
           // left box: lo (n0.x n0.y n0.z) hi (n0.w n1.x n1.y); right box: lo (n1.z n1.w n2.x) hi (n2.y n2.z n2.w)

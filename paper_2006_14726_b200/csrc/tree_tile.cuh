@@ -310,11 +310,12 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
     const int cnt_l = g - first + 1, cnt_r = last - g;
     const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
     const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-    float4* rec = reinterpret_cast<float4*>(nodes + idx);
-    rec[0] = make_float4(L.v[0], L.v[1], L.v[2], L.v[3]);
-    rec[1] = make_float4(L.v[4], L.v[5], R.v[0], R.v[1]);
-    rec[2] = make_float4(R.v[2], R.v[3], R.v[4], R.v[5]);
-    rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
+    f8 ra, rb;
+    ra.v[0] = L.v[0]; ra.v[1] = L.v[1]; ra.v[2] = L.v[2]; ra.v[3] = L.v[3]; ra.v[4] = L.v[4]; ra.v[5] = L.v[5]; ra.v[6] = R.v[0]; ra.v[7] = R.v[1];
+    rb.v[0] = R.v[2]; rb.v[1] = R.v[3]; rb.v[2] = R.v[4]; rb.v[3] = R.v[5];
+    rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
+    stg_f8(nodes + idx, ra);
+    stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
     if (idx == 0) {
 #pragma unroll
       for (int a = 0; a < 3; ++a) { st->root_lo[a] = U.v[a]; st->root_hi[a] = U.v[3 + a]; }
