@@ -87,7 +87,10 @@ int splats_update(const float* color, const float* depth, const wr_camera* src_c
  * with SPLATS_ESTATE.  Arguments and other errors as splats_update.  (Measured on B200: the build
  * does not get faster or slower this way and a step of the benchmark takes the same time, because
  * the persistent render blocks leave no room for the sort's 128-register blocks on an SM; what
- * the pair buys is that the renders of the current BVH are not delayed by an arriving frame.) */
+ * the pair buys is that the renders of the current BVH are not delayed by an arriving frame.)
+ * Progress: the sort of the build is a co-resident grid that spins on a grid barrier; beside a
+ * persistent render grid it is scheduled as render blocks retire, so it advances because renders
+ * END -- never enqueue a render that waits (on an event or a host callback) for a pending build. */
 int splats_update_begin(const float* color, const float* depth, const wr_camera* src_camera,
                         int W, int H, float r_scale);
 int splats_update_commit(void);
@@ -271,6 +274,11 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *     given up: work that the CALLER enqueues between two such render calls is not guaranteed to
  *     be complete before the second render starts writing its image (the render reads nothing
  *     of the caller's, so this only matters if that work writes the same image).
+ *     With the option on, the first kernel of a splats_update that directly follows a render
+ *     (scene bounds: it reads the caller's depth buffer and touches nothing a render uses) also
+ *     starts under that render's tail; the same caveat applies to work the caller enqueues
+ *     between the render and the update that writes the frame buffers with programmatic
+ *     dependent launches of its own.
  * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
 #define SPLATS_OPT_PDL         2
 #define SPLATS_OPT_OVERLAP     3

@@ -9,6 +9,7 @@ only compiles it and marshals numpy arrays.
 from __future__ import annotations
 
 import ctypes
+import os
 import subprocess
 from pathlib import Path
 
@@ -39,6 +40,8 @@ def build(force: bool = False) -> Path:
     """g++ -O2 -ffp-contract=off: the only fused multiply-adds are explicit fmaf().
     -mfma (when the host has it) merely inlines fmaf(); the result is the same
     correctly rounded value libm's fmaf() returns."""
+    if os.environ.get("ORACLE_SANITIZE"):
+        return _build_sanitized()
     stamp = _HERE / ".built_with_fma"
     want_fma = _cpu_has_fma()
     stale = (not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime
@@ -54,6 +57,22 @@ def build(force: bool = False) -> Path:
         elif stamp.exists():
             stamp.unlink()
     return _LIB
+
+
+def _build_sanitized() -> Path:
+    """ORACLE_SANITIZE=1: the same source with -fsanitize=address,undefined, in its own
+    file.  Run the pins with
+        ORACLE_SANITIZE=1 LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)" \
+        ASAN_OPTIONS=detect_leaks=0 UBSAN_OPTIONS=halt_on_error=1 python -m pytest tests -q -m "not gpu"
+    (the preload is needed because the interpreter itself is not instrumented)."""
+    global _LIB
+    out = _HERE / "libsplatoracle_san.so"
+    if not out.exists() or out.stat().st_mtime < _SRC.stat().st_mtime:
+        cmd = ["g++", "-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+               "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", str(_SRC), "-o", str(out)]
+        subprocess.run(cmd, check=True)
+    _LIB = out
+    return out
 
 
 def lib():

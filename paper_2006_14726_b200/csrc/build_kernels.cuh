@@ -78,8 +78,13 @@ constexpr int ROUNDS = WARP_PX / 32;                      // 8
 // number of valid pixels per tile (for the compaction) and in total.
 template <class Src>
 __global__ void __launch_bounds__(BUILD_THREADS)
-bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* __restrict__ tile_count) {
-  pdl_wait();
+bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* __restrict__ tile_count, int wait_at_start) {
+  // wait_at_start = 0: the kernel before this one in the stream is a render.  Nothing here touches
+  // what a render reads or writes (it reads the caller's frame and writes the next frame's state,
+  // the tile counts and the per-pixel splats, all of which the previous update has finished with:
+  // the render's blocks only start after that update is complete), so the blocks may run under the
+  // render's tail; one thread waits at the end so that this kernel still completes after it.
+  if (wait_at_start) pdl_wait();
   pdl_trigger();
   __shared__ float s_red[6][BUILD_THREADS / 32];
   __shared__ uint32_t s_cnt[BUILD_THREADS / 32];
@@ -149,6 +154,7 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
       }
     }
   }
+  if (!wait_at_start && tid == 0) pdl_wait();
 }
 
 // ------------------------------------------------------------------------------------ a2

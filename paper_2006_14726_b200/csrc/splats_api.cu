@@ -42,12 +42,14 @@ struct Context {
   // renders launched since the last fully serialising launch on the stream (see do_render)
   static constexpr int MAX_OVERLAP = 8;
   int render_streak = 0;
+  bool last_was_render = false;         // the last thing enqueued on the stream by this library is a render launched with PDL
   bool serialize_next_render = false;   // set when renders may be in flight that the bookkeeping below no longer knows
   const char* inflight_lo[MAX_OVERLAP] = {};
   const char* inflight_hi[MAX_OVERLAP] = {};
   uint64_t* key[2] = {nullptr, nullptr};
   uint32_t* val[2] = {nullptr, nullptr};
   uint64_t* status = nullptr;       // [max sort tiles][256]
+  size_t status_bytes = 0;
   // Two complete BVHs: build f writes set[f & 1] while the renders may still read the other one
   // (splats_update_begin / splats_update_commit); splats, colours, ids, nodes in sorted order.
   struct BvhSet {
@@ -276,7 +278,10 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   if (!async) c->render_streak = 0;   // (a decoupled build runs on its own stream: the renders in flight stay tracked)
   // bounds_kernel waits for its predecessor at its first instruction; overlapping renders
   // complete in launch order (render.cuh), so everything before it in the stream is complete
-  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count);
+  // after a render launched by this library (and nothing else since) the bounds kernel may start under its tail
+  const int bounds_wait = (pdl && c->overlap && !async && c->last_was_render) ? 0 : 1;
+  c->last_was_render = false;
+  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count, bounds_wait);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 8 ? tiles : c->num_sms * 8;
   launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
@@ -284,6 +289,10 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   if (prof) m[2] = c->mark();
   const int max_sort_tiles = P > 0 ? (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE) : 1;
   const int sgrid = max_sort_tiles < c->sort_grid ? max_sort_tiles : c->sort_grid;
+  if (c->epoch > 0xffffff00u) {   // the look-back words carry a 32-bit epoch: start over with a clean array before it wraps
+    cudaMemsetAsync(c->status, 0, c->status_bytes, s);
+    c->epoch = 0;
+  }
   SortArgs sa;
   sa.key[0] = c->key[0]; sa.key[1] = c->key[1];
   sa.val[0] = c->val[0]; sa.val[1] = c->val[1];
@@ -420,6 +429,7 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   else if (first_hit) launch(pdl, render_kernel<1, true, false>, grid, RENDER_THREADS, 0, c->stream, prm);
   else launch(pdl, render_kernel<KBUF, false, false>, grid, RENDER_THREADS, 0, c->stream, prm);
   if (c->profiling) c->spans.push_back({5, m0, c->mark()});
+  c->last_was_render = pdl;
   c->launches += 1;
   CU(cudaGetLastError());
   return SPLATS_OK;
@@ -487,7 +497,8 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     if (e == cudaSuccess) e = dmalloc(&c->pyr, 2 * off);
     if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_pyr, &c->pyr_layout, sizeof(PyramidLayout));
   }
-  if (e == cudaSuccess) e = cudaMemset(c->status, 0, status_rows * RADIX * sizeof(uint64_t));
+  c->status_bytes = status_rows * RADIX * sizeof(uint64_t);
+  if (e == cudaSuccess) e = cudaMemset(c->status, 0, c->status_bytes);
   if (e == cudaSuccess) {
     FrameState init;
     memset(&init, 0, sizeof(init));
@@ -615,6 +626,7 @@ int splats_render_points(const wr_camera* dst_camera, int W2, int H2, int point_
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
   c->render_streak = 0;
+  c->last_was_render = false;
   points_kernel<false><<<grid, POINT_THREADS, 0, c->stream>>>(p);
   points_kernel<true><<<grid, POINT_THREADS, 0, c->stream>>>(p);
   points_background_kernel<<<grid, POINT_THREADS, 0, c->stream>>>(p);
@@ -661,6 +673,7 @@ int splats_march(const float* volume, int n, const wr_transfer* tf, const wr_cam
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
   c->render_streak = 0;
+  c->last_was_render = false;
   march_kernel<<<grid, MARCH_THREADS, 0, c->stream>>>(p);
   if (c->profiling) c->spans.push_back({8, m0, c->mark()});
   c->launches += 1;
@@ -688,6 +701,7 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
   size_t m0 = 0;
   if (c->profiling) m0 = c->mark();
   c->render_streak = 0;
+  c->last_was_render = false;
   pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, c->stream>>>(a, c->pack_tile_count);
   const int grid2 = a.num_tiles < c->num_sms * 4 ? a.num_tiles : c->num_sms * 4;
   pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->pack_tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
@@ -731,6 +745,7 @@ int splats_update_packed_host(const unsigned long long* samples_host, const unsi
   }
   CU(cudaEventRecord(c->in_uploaded[u], c->h2d_stream));
   CU(cudaStreamWaitEvent(c->stream, c->in_uploaded[u], 0));
+  c->last_was_render = false;
   src.samples = reinterpret_cast<const uint64_t*>(c->stage_color[u]);
   PackedGather g;
   g.samples = src.samples;
@@ -758,6 +773,7 @@ int splats_update_host(const float* color_host, const float* depth_host, const w
   CU(cudaMemcpyAsync(c->stage_depth[u], depth_host, P * sizeof(float), cudaMemcpyHostToDevice, c->h2d_stream));
   CU(cudaEventRecord(c->in_uploaded[u], c->h2d_stream));
   CU(cudaStreamWaitEvent(c->stream, c->in_uploaded[u], 0));
+  c->last_was_render = false;
   rc = do_update_frame(c, c->stage_color[u], c->stage_depth[u], src_camera, W, H, r_scale);
   if (rc) return rc;
   CU(cudaEventRecord(c->in_free[u], c->stream));
@@ -774,9 +790,11 @@ int splats_render_host(const wr_camera* dst_camera, int W2, int H2, float* out_r
   if (rc) return rc;
   const int r = (int)(c->n_readbacks % Context::N_OUT);
   if (c->n_readbacks >= (unsigned)Context::N_OUT) CU(cudaStreamWaitEvent(c->stream, c->out_free[r], 0));
+  c->last_was_render = false;
   rc = do_render(c, dst_camera, W2, H2, c->stage_out[r]);
   if (rc) return rc;
   CU(cudaEventRecord(c->out_rendered[r], c->stream));
+  c->last_was_render = false;   // an event record follows the render in the stream
   CU(cudaStreamWaitEvent(c->d2h_stream, c->out_rendered[r], 0));
   CU(cudaMemcpyAsync(out_rgba_host, c->stage_out[r], (size_t)W2 * H2 * 4 * sizeof(float), cudaMemcpyDeviceToHost,
                      c->d2h_stream));
@@ -802,9 +820,11 @@ int splats_render_host_rgba8(const wr_camera* dst_camera, int W2, int H2, unsign
   if (rc) return rc;
   const int r = (int)(c->n_readbacks % Context::N_OUT);
   if (c->n_readbacks >= (unsigned)Context::N_OUT) CU(cudaStreamWaitEvent(c->stream, c->out_free[r], 0));
+  c->last_was_render = false;
   rc = do_render(c, dst_camera, W2, H2, c->stage_out[r], false, true);
   if (rc) return rc;
   CU(cudaEventRecord(c->out_rendered[r], c->stream));
+  c->last_was_render = false;   // an event record follows the render in the stream
   CU(cudaStreamWaitEvent(c->d2h_stream, c->out_rendered[r], 0));
   CU(cudaMemcpyAsync(out_rgba8_host, c->stage_out[r], (size_t)W2 * H2 * sizeof(unsigned), cudaMemcpyDeviceToHost, c->d2h_stream));
   CU(cudaEventRecord(c->out_free[r], c->d2h_stream));

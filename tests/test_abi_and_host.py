@@ -98,3 +98,30 @@ def test_replicas_host_logic_two_gloo_ranks(tmp_path):
                        capture_output=True, text=True, env=env, timeout=240)
     assert r.returncode == 0, r.stdout + r.stderr
     assert r.stdout.count("ok") == 2
+
+
+_SPAWNER = r"""
+import sys
+sys.path.insert(0, {root!r})
+from paper_2006_14726_b200 import replicas
+N = 2
+if replicas.needs_spawn(N):          # started plainly: start the N ranks ourselves (what `bench.py --gpus N` does)
+    raise SystemExit(replicas.spawn(__file__, [], N))
+world, rank, local = replicas.init("gloo")
+assert world == N
+replicas.barrier()
+assert replicas.max_over_ranks(float(rank + 1)) == float(N)
+replicas.shutdown()
+print("spawned ok", rank)
+"""
+
+
+def test_replicas_self_spawn_two_gloo_ranks(tmp_path):
+    # `python bench.py --gpus N` without torchrun: the script starts its own ranks (127.0.0.1, free port)
+    script = tmp_path / "spawner.py"
+    script.write_text(_SPAWNER.format(root=str(ROOT)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    r = subprocess.run([sys.executable, str(script)], capture_output=True, text=True, env=env, timeout=240)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("spawned ok") == 2
