@@ -4,6 +4,7 @@
 // fallback (every entry point fails with SPLATS_ECUDA / SPLATS_ESTATE without a device).
 #include "../../include/splats.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -330,7 +331,7 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     if (prof) m[4] = c->mark();
     int nt_log = 0;
     while ((1 << nt_log) < tgrid) ++nt_log;
-    const int sgrid2 = (tgrid * TT_QMAX + SPINE_THREADS - 1) / SPINE_THREADS;   // enough for a full queue; idle blocks exit at once
+    const int sgrid2 = std::min(c->num_sms * 8, (tgrid * TT_QMAX + 7) / 8);   // persistent, one warp per queued node; idle blocks exit at once
     launch(pdl, tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
            (const float4*)bs.sphere, (const float4*)c->pyr, bs.nodes, (const uint8_t*)c->tile_min, (const uint16_t*)c->tile_fb, nt_log);
   } else {

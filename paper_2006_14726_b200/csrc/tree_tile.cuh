@@ -21,9 +21,10 @@
 // crosses a tile edge; they are strict prefix / suffix minima of the tile's deltas, <= 2 x 97 per
 // tile -- are queued with what is known about them.  The block also writes, for every threshold
 // v, the position of the first / last split of the tile with d < v.
-// tree_spine_kernel: finishes the queued nodes: the missing range end is the first (last) split
-// with a smaller delta in the nearest tile that has one (a search over one byte per tile in
-// shared memory, then one table look-up); boxes by range queries on the global pyramid.
+// tree_spine_kernel: finishes the queued nodes, one warp each: the missing range end is the first
+// (last) split with a smaller delta in the nearest tile that has one (a search over one byte per
+// tile in shared memory, then one table look-up); the two child boxes are range queries on the
+// global pyramid whose <= 76 independent pieces are spread over the lanes (one round trip).
 // Same tree, same numbering, same boxes as the other two modes, bit for bit.
 #pragma once
 #include "lbvh.cuh"
@@ -476,28 +477,33 @@ struct TileMins {
   }
 };
 
-// Box of the sorted leaves [l, r), l < r: ragged ends (< 8 leaves each) from the spheres, the rest
-// from the global pyramid, levels >= PYR_BASE.  The entry addresses do not depend on loaded data.
-__device__ __forceinline__ void range_box_base(const float4* __restrict__ sphere, const float4* __restrict__ pyr, uint32_t l, uint32_t r, BoxAcc& A) {
-  A.init();
-  uint32_t lb = (l + (1u << PYR_BASE) - 1) >> PYR_BASE, rb = r >> PYR_BASE;
-  if (lb >= rb) {   // no aligned block inside: < 2 x 8 leaves
-    for (uint32_t i = l; i < r; ++i) A.add_sphere(__ldg(sphere + i));
+// One of the 38 independent pieces of the box of the sorted leaves [l, r), l < r: pieces 0..13 are the
+// ragged ends (< 8 leaves each, or all of a range without an aligned block of 8) read from the spheres,
+// piece 14 + j is level PYR_BASE + j of the global pyramid (at most two entries per level).  The
+// addresses depend only on l and r, so a warp issues all pieces of a node's two child boxes at once.
+constexpr int RANGE_PIECES = 14 + (PYR_MAX_LEVELS - PYR_BASE + 1);
+__device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, const float4* __restrict__ pyr, uint32_t l, uint32_t r,
+                                            int piece, BoxAcc& A) {
+  const uint32_t lb = (l + (1u << PYR_BASE) - 1) >> PYR_BASE, rb = r >> PYR_BASE;
+  const bool small = lb >= rb;   // no aligned block inside: < 2 x 8 leaves, all read directly
+  if (piece < 14) {
+    uint32_t i;
+    if (small) i = l + piece;
+    else if (piece < 7) { i = l + piece; if (i >= (lb << PYR_BASE)) return; }
+    else i = (rb << PYR_BASE) + (piece - 7);
+    if (i < r) A.add_sphere(__ldg(sphere + i));
     return;
   }
-  for (uint32_t i = l; i < (lb << PYR_BASE); ++i) A.add_sphere(__ldg(sphere + i));
-  for (uint32_t i = rb << PYR_BASE; i < r; ++i) A.add_sphere(__ldg(sphere + i));
-#pragma unroll 4
-  for (int k = PYR_BASE; k <= PYR_MAX_LEVELS; ++k) {
-    if (lb >= rb) break;
-    const float4* lev = pyr + 2 * (size_t)c_pyr.off[k];
-    if (lb & 1u) { A.add(__ldg(lev + 2 * (size_t)lb), __ldg(lev + 2 * (size_t)lb + 1)); ++lb; }
-    if (rb & 1u) { --rb; A.add(__ldg(lev + 2 * (size_t)rb), __ldg(lev + 2 * (size_t)rb + 1)); }
-    lb >>= 1;
-    rb >>= 1;
-  }
+  if (small) return;
+  const int k = PYR_BASE + (piece - 14);
+  const uint32_t lk = (l + (1u << k) - 1) >> k, rk = r >> k;   // the segment-tree walk's bounds when it reaches level k
+  if (lk >= rk) return;
+  const float4* lev = pyr + 2 * (size_t)c_pyr.off[k];
+  if (lk & 1u) A.add(__ldg(lev + 2 * (size_t)lk), __ldg(lev + 2 * (size_t)lk + 1));
+  if (rk & 1u) A.add(__ldg(lev + 2 * (size_t)(rk - 1)), __ldg(lev + 2 * (size_t)(rk - 1) + 1));
 }
 
+// One warp per queued node; persistent blocks (the per-tile minima are staged once per block).
 constexpr int SPINE_THREADS = 256;
 __global__ void __launch_bounds__(SPINE_THREADS)
 tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4* __restrict__ queue,
@@ -509,7 +515,9 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
   uint8_t* m = spine_smem;
   const int n = (int)st->n;
   const int qn = (int)st->spine_n;
-  if ((int)(blockIdx.x * SPINE_THREADS) >= qn) return;
+  constexpr int WPB = SPINE_THREADS / 32;
+  if ((int)(blockIdx.x * WPB) >= qn) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ntiles = (n + TT_LEAVES - 1) / TT_LEAVES;
   TileMins tm;
   tm.m = m;
@@ -522,7 +530,8 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
     for (int j = threadIdx.x; j < cnt; j += SPINE_THREADS) m[o1 + j] = min(m[o0 + 2 * j], m[o0 + 2 * j + 1]);
     __syncthreads();
   }
-  for (int e = blockIdx.x * SPINE_THREADS + threadIdx.x; e < qn; e += gridDim.x * SPINE_THREADS) {
+  for (int e = blockIdx.x * WPB + warp; e < qn; e += gridDim.x * WPB) {
+    // ---- the node's range (every lane computes the same values: broadcast loads, no divergence)
     const int4 ent = __ldg(queue + e);
     const int g = ent.x, t = g >> TT_LOG;
     const uint32_t v = (uint32_t)ent.w;
@@ -535,23 +544,41 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
       const int t2 = tm.right(t + 1, v);
       last = (t2 << TT_LOG) + (int)__ldg(tile_fb + (size_t)t2 * (2 * TT_VPAD) + v);
     }
+    // ---- both child boxes: 2 x RANGE_PIECES independent pieces spread over the lanes, then a warp reduction
+    BoxAcc L, R;
+    L.init();
+    R.init();
+    for (int piece = lane; piece < 2 * RANGE_PIECES; piece += 32) {
+      if (piece < RANGE_PIECES) range_piece(sphere, pyr, (uint32_t)first, (uint32_t)g + 1u, piece, L);
+      else range_piece(sphere, pyr, (uint32_t)g + 1u, (uint32_t)last + 1u, piece - RANGE_PIECES, R);
+    }
     const int dl = first > 0 ? delta(keys, n, first - 1, __ldg(keys + first - 1), first) : -1;
     const int dr = last < n - 1 ? delta(keys, n, last, __ldg(keys + last), last + 1) : -1;
     const int idx = dr > dl ? last : first;
-    BoxAcc L, R;
-    range_box_base(sphere, pyr, (uint32_t)first, (uint32_t)g + 1u, L);
-    range_box_base(sphere, pyr, (uint32_t)g + 1u, (uint32_t)last + 1u, R);
-    const int cnt_l = g - first + 1, cnt_r = last - g;
-    const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
-    const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-    float4* rec = reinterpret_cast<float4*>(nodes + idx);
-    rec[0] = make_float4(L.lo[0], L.lo[1], L.lo[2], L.hi[0]);
-    rec[1] = make_float4(L.hi[1], L.hi[2], R.lo[0], R.lo[1]);
-    rec[2] = make_float4(R.lo[2], R.hi[0], R.hi[1], R.hi[2]);
-    rec[3] = make_float4(__int_as_float(left), __int_as_float(right), 0.0f, 0.0f);
-    if (idx == 0) {
 #pragma unroll
-      for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        L.lo[a] = fminf(L.lo[a], __shfl_xor_sync(0xffffffffu, L.lo[a], o));
+        L.hi[a] = fmaxf(L.hi[a], __shfl_xor_sync(0xffffffffu, L.hi[a], o));
+        R.lo[a] = fminf(R.lo[a], __shfl_xor_sync(0xffffffffu, R.lo[a], o));
+        R.hi[a] = fmaxf(R.hi[a], __shfl_xor_sync(0xffffffffu, R.hi[a], o));
+      }
+    }
+    if (lane == 0) {
+      const int cnt_l = g - first + 1, cnt_r = last - g;
+      const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
+      const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
+      f8 ra, rb;
+      ra.v[0] = L.lo[0]; ra.v[1] = L.lo[1]; ra.v[2] = L.lo[2]; ra.v[3] = L.hi[0]; ra.v[4] = L.hi[1]; ra.v[5] = L.hi[2]; ra.v[6] = R.lo[0]; ra.v[7] = R.lo[1];
+      rb.v[0] = R.lo[2]; rb.v[1] = R.hi[0]; rb.v[2] = R.hi[1]; rb.v[3] = R.hi[2];
+      rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
+      stg_f8(nodes + idx, ra);
+      stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
+      if (idx == 0) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
+      }
     }
   }
 }
