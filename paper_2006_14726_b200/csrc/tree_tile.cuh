@@ -41,7 +41,10 @@ constexpr int TT_WARPS = TT_THREADS / 32;
 constexpr int TT_QMAX = 200;    // >= 2 x 97: strict prefix + suffix minima of byte-sized deltas
 constexpr int TT_VMAX = 97;     // delta + 1 lies in [0, 96]; 0 = "beyond the array"
 constexpr int TT_VPAD = 100;    // table stride
-constexpr int TT_CLIMB = 64;    // work lists up to this length are finished by climbing threads instead of block-wide rounds
+#ifndef SPLATS_TT_CLIMB
+#define SPLATS_TT_CLIMB 64
+#endif
+constexpr int TT_CLIMB = SPLATS_TT_CLIMB;    // work lists up to this length are finished by climbing threads instead of block-wide rounds
 constexpr int PYR_BASE = 3;     // lowest level of the global pyramid that the tiled mode writes and reads
 static_assert(TT_LOG >= 7 && TT_LOG <= 12, "tile of 128 .. 4096 leaves");
 
