@@ -230,17 +230,33 @@ int splats_count(unsigned* n_host);
  *   perm        N  uint32   splat ids (= source pixel indices) in sorted order
  *   children    (N-1)*2 int32; node ids: internal j -> j, leaf at sorted position i -> N-1+i
  *   parents     (2N-1) int32, indexed by node id; -1 for the root
- *   node_aabbs  (2N-1)*6 float32: lo xyz, hi xyz per node id
+ *   node_aabbs  (2N-1)*6 float32: lo xyz, hi xyz per node id -- the EXACT boxes (oracle step O7).
+ *               The traversal reads 16-bit quantised boxes (splats_export_qnodes); the default
+ *               (tiled) build computes the exact ones on the way but stores them only while
+ *               SPLATS_OPT_EXACT_NODES is on: without it node_aabbs != NULL fails with ESTATE.
  * Internal nodes use Karras' numbering (root 0; an internal child covering sorted range
  * [a,g] is node g when it is a left child, node a when it is a right child). */
 int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* parents,
                   float* node_aabbs);
 
-/* The boxes the traversal actually tests: for every internal node j (Karras numbering) the 12
- * floats stored in its record -- left child box lo xyz, hi xyz, then the right child's -- copied
- * verbatim (splats_export's node_aabbs are derived: a node's box there is the union of these two).
+/* The exact child boxes of every internal node j (Karras numbering): the 12 floats of its 64-byte
+ * record -- left child box lo xyz, hi xyz, then the right child's -- copied verbatim
+ * (splats_export's node_aabbs are derived: a node's box there is the union of these two).  Needs
+ * SPLATS_OPT_EXACT_NODES during the build (ESTATE otherwise), like node_aabbs.
  *   child_boxes  dev, (N-1)*12 float32.  Synchronises.  Parity only. */
 int splats_export_child_boxes(float* child_boxes);
+
+/* The records the traversal actually reads, copied verbatim: for every internal node j eight
+ * uint32 -- words 0..2: axis x, y, z of the left child box, q_lo | q_hi << 16; words 3..5: the right
+ * child's; words 6, 7: left / right link (>= 0: internal node; < 0: the leaf at sorted position
+ * link & 0x3ffffff).  The 16-bit codes quantise the exact child boxes (oracle step O7) over the
+ * frame [lo - rmax, hi + rmax] (lo / hi: bounds of the splat centres, rmax: the largest radius),
+ * lower planes rounded down, upper planes rounded up (S13): a quantised box
+ * contains the exact one and the image is unchanged, the records are half the size.
+ *   qnodes  dev, (N-1)*8 uint32 (may be NULL)
+ *   frame   dev, 7 float32: lo xyz, hi xyz, rmax (may be NULL)
+ * Synchronises.  Parity only. */
+int splats_export_qnodes(unsigned* qnodes, float* frame);
 
 /* Export the splats themselves in sorted order (dev pointers, may be NULL): sphere N*4
  * float32 (cx, cy, cz, r), rgba N*4 float32; and the scene bounds (min/max of the centres)
@@ -250,8 +266,11 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 /* Implementation variants (same results, bit for bit; for A/B measurement).  Takes effect at
  * the next splats_update.
  *   SPLATS_OPT_REFIT: how step a5 (node boxes) is computed.
- *     SPLATS_REFIT_PYRAMID (default): a bottom-up min/max pyramid over the sorted leaf boxes,
- *       then every node reads its two child boxes as range queries (no atomics, no fences).
+ *     SPLATS_REFIT_TILED (default): one block per 1024 sorted leaves builds every subtree inside its
+ *       tile bottom-up in shared memory (boxes and topology together); the few nodes that span
+ *       tiles are finished by a second kernel with range queries on a min/max pyramid.
+ *     SPLATS_REFIT_PYRAMID: a bottom-up min/max pyramid over the sorted leaf boxes, Karras'
+ *       per-node searches, then every node reads its two child boxes as range queries.
  *     SPLATS_REFIT_ATOMIC: one thread per leaf climbs the tree; the second arrival at a node's
  *       atomic counter forms the union and continues (the classic LBVH refit).
  *   SPLATS_OPT_SORT: how step a3 (order by (code, id)) is computed.
@@ -261,6 +280,9 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *       redo the sort with all 8 passes.
  *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
  *     SPLATS_SORT_LSD8_LAUNCHES: one launch per pass.
+ *   SPLATS_OPT_EXACT_NODES (default 0): the tiled build also stores the exact float32 child boxes
+ *     (64 bytes per node) beside the quantised traversal records, for splats_export /
+ *     splats_export_child_boxes.  The other two refit modes always store them.
  *   SPLATS_OPT_PDL (default 1): launch the kernels of splats_update / splats_render as
  *     programmatic dependent launches (each kernel waits on its predecessor at its first
  *     instruction; only the launch latency overlaps).  0 = ordinary stream launches.
@@ -282,6 +304,7 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  * Errors: EINVAL for an unknown option or value, ESTATE without a context. */
 #define SPLATS_OPT_PDL         2
 #define SPLATS_OPT_OVERLAP     3
+#define SPLATS_OPT_EXACT_NODES 4
 #define SPLATS_OPT_REFIT       0
 #define SPLATS_REFIT_PYRAMID   0
 #define SPLATS_REFIT_ATOMIC    1

@@ -22,6 +22,7 @@ OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
 OPT_PDL = 2
 OPT_OVERLAP = 3
+OPT_EXACT_NODES = 4
 
 
 class SplatsError(RuntimeError):
@@ -77,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.splats_export.argtypes = [_vp, _vp, _vp, _vp, _vp]
         L.splats_export_splats.argtypes = [_vp, _vp, _vp]
         L.splats_export_child_boxes.argtypes = [_vp]
+        L.splats_export_qnodes.argtypes = [_vp, _vp]
         L.splats_set_profiling.argtypes = [_ci]
         L.splats_set_option.argtypes = [_ci, _ci]
         L.splats_set_radius.argtypes = [_ci, ctypes.c_float]
@@ -244,19 +246,31 @@ def splats_count() -> int:
     return int(n.value)
 
 
-def splats_export():
-    """dict of CUDA tensors: keys (int64 view of uint64), perm, children, parents, node_aabbs."""
+def splats_export(aabbs: bool = True):
+    """dict of CUDA tensors: keys (int64 view of uint64), perm, children, parents, node_aabbs
+    (the exact boxes: they need OPT_EXACT_NODES during the build; aabbs=False skips them)."""
     n = splats_count()
     dev = torch.device("cuda", torch.cuda.current_device())
     keys = torch.empty(n, dtype=torch.int64, device=dev)
     perm = torch.empty(n, dtype=torch.int32, device=dev)
     children = torch.empty((max(n - 1, 0), 2), dtype=torch.int32, device=dev)
     parents = torch.empty(max(2 * n - 1, 0), dtype=torch.int32, device=dev)
-    aabbs = torch.empty((max(2 * n - 1, 0), 6), dtype=torch.float32, device=dev)
+    boxes = torch.empty((max(2 * n - 1, 0), 6), dtype=torch.float32, device=dev) if aabbs else None
     if n:
         _check(lib().splats_export(keys.data_ptr(), perm.data_ptr(), children.data_ptr() if n > 1 else None,
-                                   parents.data_ptr(), aabbs.data_ptr()))
-    return dict(N=n, keys=keys, perm=perm, children=children, parents=parents, node_aabbs=aabbs)
+                                   parents.data_ptr(), boxes.data_ptr() if aabbs else None))
+    return dict(N=n, keys=keys, perm=perm, children=children, parents=parents, node_aabbs=boxes)
+
+
+def splats_export_qnodes():
+    """(N-1, 8) int32 CUDA tensor (uint32 bit patterns): the 32-byte records the traversal reads;
+    and frame = 7 float32: bounds of the centres lo xyz, hi xyz and the largest radius."""
+    n = splats_count()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    q = torch.empty((max(n - 1, 0), 8), dtype=torch.int32, device=dev)
+    frame = torch.empty(7, dtype=torch.float32, device=dev)
+    _check(lib().splats_export_qnodes(q.data_ptr() if n > 1 else None, frame.data_ptr()))
+    return dict(N=n, qnodes=q, frame=frame)
 
 
 def splats_export_child_boxes():

@@ -43,12 +43,14 @@ struct FrameSource {
   __device__ __forceinline__ Raw load(int64_t i) const { return __ldg(depth + i); }
   __device__ __forceinline__ Raw invalid() const { return 0.0f; }
   __device__ __forceinline__ bool valid(Raw t) const { return depth_valid(t); }
-  __device__ __forceinline__ void bounds_centre(Raw t, int64_t i, int x, int y, float p[3]) const {
+  __device__ __forceinline__ float bounds_centre(Raw t, int64_t i, int x, int y, float p[3]) const {   // returns the radius
     float len;
     splat_centre(cam, x, y, t, p, len);
     const float z = div_(t, len);
     const float alpha = rp.mode == 2 ? __ldg(&color[i].w) : 0.0f;
-    sphere_px[i] = make_float4(p[0], p[1], p[2], splat_radius(rp, z, alpha));
+    const float r = splat_radius(rp, z, alpha);
+    sphere_px[i] = make_float4(p[0], p[1], p[2], r);
+    return r;
   }
   __device__ __forceinline__ void key_centre(Raw, int64_t i, float p[3]) const {
     const float4 sp = __ldcg(sphere_px + i);   // written by the previous kernel of this stream
@@ -63,7 +65,10 @@ struct PackedSource {
   __device__ __forceinline__ Raw load(int64_t i) const { return __ldg(samples + i); }
   __device__ __forceinline__ Raw invalid() const { return 0ull; }
   __device__ __forceinline__ bool valid(Raw w) const { return (w >> 48) != 0ull; }
-  __device__ __forceinline__ void bounds_centre(Raw w, int64_t, int, int, float p[3]) const { decode_centre(w, q, p); }
+  __device__ __forceinline__ float bounds_centre(Raw w, int64_t, int, int, float p[3]) const {
+    decode_centre(w, q, p);
+    return decode_radius(w, q);
+  }
   __device__ __forceinline__ void key_centre(Raw w, int64_t, float p[3]) const { decode_centre(w, q, p); }
 };
 
@@ -74,10 +79,11 @@ constexpr int WARP_PX = TILE_PX / (BUILD_THREADS / 32);   // 256
 constexpr int ROUNDS = WARP_PX / 32;                      // 8
 
 // ------------------------------------------------------------------------------------ a1
-// Scene bounds = component-wise min/max of the valid splat centres (Eq. 1),
+// Scene bounds = component-wise min/max of the valid splat centres (Eq. 1), the
+// largest radius (with the bounds: the frame of the quantised node boxes, common.cuh QNode),
 // number of valid pixels per tile (for the compaction) and in total.
 template <class Src>
-__global__ void __launch_bounds__(BUILD_THREADS)
+__global__ void __launch_bounds__(BUILD_THREADS, 6)
 bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* __restrict__ tile_count, int wait_at_start) {
   // wait_at_start = 0: the kernel before this one in the stream is a render.  Nothing here touches
   // what a render reads or writes (it reads the caller's frame and writes the next frame's state,
@@ -86,12 +92,12 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
   // render's tail; one thread waits at the end so that this kernel still completes after it.
   if (wait_at_start) pdl_wait();
   pdl_trigger();
-  __shared__ float s_red[6][BUILD_THREADS / 32];
+  __shared__ float s_red[7][BUILD_THREADS / 32];
   __shared__ uint32_t s_cnt[BUILD_THREADS / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t base = (int64_t)blockIdx.x * TILE_PX + (int64_t)warp * WARP_PX + lane;
   const float INF = __int_as_float(0x7f800000);
-  float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
+  float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF}, rmax = 0.0f;
   uint32_t cnt = 0;
   typename Src::Raw t[ROUNDS];
 #pragma unroll
@@ -102,7 +108,7 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
   for (int k = 0; k < ROUNDS; ++k) {
     if (src.valid(t[k])) {
       float p[3];
-      src.bounds_centre(t[k], base + 32 * k, x, y, p);
+      rmax = fmaxf(rmax, src.bounds_centre(t[k], base + 32 * k, x, y, p));
 #pragma unroll
       for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], p[a]); hi[a] = fmaxf(hi[a], p[a]); }
       ++cnt;
@@ -117,11 +123,13 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
       lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
       hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
     }
+    rmax = fmaxf(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
     cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
   }
   if (lane == 0) {
 #pragma unroll
     for (int a = 0; a < 3; ++a) { s_red[a][warp] = lo[a]; s_red[3 + a][warp] = hi[a]; }
+    s_red[6][warp] = rmax;
     s_cnt[warp] = cnt;
   }
   __syncthreads();
@@ -133,6 +141,7 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
       lo[a] = lane < NW ? s_red[a][lane] : INF;
       hi[a] = lane < NW ? s_red[3 + a][lane] : -INF;
     }
+    rmax = lane < NW ? s_red[6][lane] : 0.0f;
 #pragma unroll
     for (int o = NW / 2; o > 0; o >>= 1) {
 #pragma unroll
@@ -140,6 +149,7 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
         lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
         hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
       }
+      rmax = fmaxf(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
       cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     }
     if (lane == 0) {
@@ -150,6 +160,7 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
           atomicMin(&st->lo[a], f2ord(lo[a]));
           atomicMax(&st->hi[a], f2ord(hi[a]));
         }
+        atomicMax(&st->rmax, f2ord(rmax));
         atomicAdd(&st->n, cnt);
       }
     }
@@ -193,7 +204,7 @@ __device__ __forceinline__ uint64_t morton63(const float p[3], const float lo[3]
 // 32 consecutive pixels whose high digits mostly agree, so runs of equal digits are counted once.
 // Block 0 also re-arms the next frame's FrameState.
 template <class Src>
-__global__ void __launch_bounds__(BUILD_THREADS)
+__global__ void __launch_bounds__(BUILD_THREADS, 6)
 unproject_kernel(const Src src, int64_t P, int num_tiles,
                  FrameState* __restrict__ st, FrameState* __restrict__ st_next,
                  const uint32_t* __restrict__ tile_count, uint64_t* __restrict__ keys0,
@@ -214,8 +225,14 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
     if (tid == 5) st_next->sort_bar = 0u;
     if (tid == 6) st_next->sort_fallback = 0u;
     if (tid == 7) st_next->spine_n = 0u;
+    if (tid == 8) st_next->rmax = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
+  }
+  if (blockIdx.x == 0 && tid == 32) {   // bounds and largest radius are final: the frame of the quantised node boxes
+    const QFrame q = derive_qframe(st);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { st->qf[a] = q.lo[a]; st->qf[3 + a] = q.s[a]; st->qf[6 + a] = q.c[a]; }
   }
 #pragma unroll
   for (int d = 0; d < 8; ++d) s_hist[d][tid] = 0u;

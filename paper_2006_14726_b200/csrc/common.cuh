@@ -146,7 +146,9 @@ struct FrameState {
   uint32_t sort_bar;       // grid barrier counter of the sort launch (init 0)
   uint32_t sort_fallback;  // set when the hybrid sort has to redo all 8 passes (init 0)
   uint32_t spine_n;        // nodes queued by tree_tile_kernel for tree_spine_kernel (init 0)
-  uint32_t pad_[3];
+  uint32_t rmax;           // ordered-uint max of the valid splats' radii (init 0): with lo / hi the frame of the quantised node boxes
+  uint32_t pad_[2];
+  float qf[12];            // QFrame (lo, s, c; below) derived once per frame by unproject_kernel from lo / hi / rmax
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
 
@@ -191,6 +193,73 @@ struct __align__(64) Node {
   unsigned flag;
 };
 static_assert(sizeof(Node) == 64, "node record must be 64 bytes");
+
+// ---- traversal record (S13): 32 bytes, ONE 256-bit load per node visit.
+// The twelve planes of the two child boxes are quantised to 16 bits over the frame
+// [lo - rmax, hi + rmax] (lo / hi = bounds of the splat centres, rmax = largest radius: all three
+// are known before the tree is built), lower planes rounded down, upper planes rounded up, so a
+// quantised box always contains the exact one; the exact boxes are what the build computes
+// (S7) and, with SPLATS_OPT_EXACT_NODES, also stores (Node).
+//   w[a]     = q_lo | q_hi << 16 of axis a of the left child, w[3 + a] of the right child
+//   w[6], w[7] = left / right link, as in Node
+struct __align__(32) QNode {
+  uint32_t w[8];
+};
+static_assert(sizeof(QNode) == 32, "traversal record must be 32 bytes");
+
+struct QFrame {
+  float lo[3];   // lo_a - rmax
+  float s[3];    // 65535 / ext_a (encode), 0 for a zero extent
+  float c[3];    // ext_a / 65535 (decode)
+};
+// derived once per frame (unproject_kernel, when lo / hi / rmax are final) and stored in FrameState::qf
+__device__ __forceinline__ QFrame derive_qframe(const FrameState* st) {
+  QFrame q;
+  const float rmax = ord2f(st->rmax);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    q.lo[a] = sub_(ord2f(st->lo[a]), rmax);
+    const float ext = sub_(add_(ord2f(st->hi[a]), rmax), q.lo[a]);
+    q.s[a] = ext > 0.0f ? div_(65535.0f, ext) : 0.0f;
+    q.c[a] = div_(ext, 65535.0f);
+  }
+  return q;
+}
+__device__ __forceinline__ QFrame load_qframe(const FrameState* st) {
+  QFrame q;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) { q.lo[a] = __ldcg(&st->qf[a]); q.s[a] = __ldcg(&st->qf[3 + a]); q.c[a] = __ldcg(&st->qf[6 + a]); }
+  return q;
+}
+// one axis of one child box: lower plane rounded down, upper plane rounded up, both clamped to 16 bits.
+// floor / ceil without the conversion unit: for 0 <= u <= 65535, 2^23 + u rounded down (up) to float32 is
+// 2^23 + floor(u) (ceil(u)) exactly, and its low mantissa bits are the integer.
+__device__ __forceinline__ uint32_t quant_planes(float lo, float hi, float qlo, float s) {
+  const float ul = fminf(fmaxf(mul_(sub_(lo, qlo), s), 0.0f), 65535.0f);   // fmaxf(NaN, 0) = 0
+  const float uh = fminf(fmaxf(mul_(sub_(hi, qlo), s), 0.0f), 65535.0f);
+  const uint32_t a = __float_as_uint(__fadd_rd(ul, 8388608.0f)), b = __float_as_uint(__fadd_ru(uh, 8388608.0f));
+  return __byte_perm(a, b, 0x5410);   // a's low half | b's low half << 16
+}
+// L, R: lo xyz, hi xyz of the two child boxes
+__device__ __forceinline__ void store_qnode(QNode* dst, const float* L, const float* R, int left, int right, const QFrame& q) {
+  uint32_t w[8];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    w[a] = quant_planes(L[a], L[3 + a], q.lo[a], q.s[a]);
+    w[3 + a] = quant_planes(R[a], R[3 + a], q.lo[a], q.s[a]);
+  }
+  w[6] = (uint32_t)left;
+  w[7] = (uint32_t)right;
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "l"(dst), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]) : "memory");
+}
+struct u8x { uint32_t v[8]; };
+__device__ __forceinline__ u8x ldg_u8(const void* p) {   // read-only path (LDG.E.256.CONSTANT)
+  u8x r;
+  asm("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+      : "=r"(r.v[0]), "=r"(r.v[1]), "=r"(r.v[2]), "=r"(r.v[3]), "=r"(r.v[4]), "=r"(r.v[5]), "=r"(r.v[6]), "=r"(r.v[7]) : "l"(p));
+  return r;
+}
 
 __device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) {
   uint64_t v;

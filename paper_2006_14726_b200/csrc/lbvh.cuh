@@ -430,10 +430,28 @@ boxes_kernel(const int4* __restrict__ ranges, const float4* __restrict__ sphere,
 }
 
 // Canonical export for the bit-exact acceptance checks (include/splats.h, splats_export).
+// The other two refit modes (SPLATS_REFIT_PYRAMID, SPLATS_REFIT_ATOMIC) produce exact 64-byte
+// records; the traversal reads the 32-byte quantised ones (common.cuh, QNode): one more pass.
+__global__ void __launch_bounds__(LBVH_THREADS)
+quantise_nodes_kernel(const Node* __restrict__ nodes, const FrameState* __restrict__ st, QNode* __restrict__ qnodes) {
+  pdl_wait();
+  pdl_trigger();
+  const int n = (int)st->n;
+  const QFrame q = load_qframe(st);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n - 1; i += gridDim.x * blockDim.x) {
+    const float4* rec = reinterpret_cast<const float4*>(nodes + i);
+    const float4 a = __ldcg(rec), b = __ldcg(rec + 1), c = __ldcg(rec + 2), d = __ldcg(rec + 3);
+    const float L[6] = {a.x, a.y, a.z, a.w, b.x, b.y}, R[6] = {b.z, b.w, c.x, c.y, c.z, c.w};
+    store_qnode(qnodes + i, L, R, __float_as_int(d.x), __float_as_int(d.y), q);
+  }
+}
+
 // Parent links are not part of the traversal structure: they are derived here from the
 // child links (parents[] must be pre-filled with -1 by the caller; the root keeps it).
+// Topology comes from the traversal records; the exact boxes from the 64-byte records, which
+// exist only when the build wrote them (`nodes` may be null: then aabbs must be null too).
 __global__ void __launch_bounds__(LBVH_THREADS)
-export_kernel(const Node* __restrict__ nodes, const float4* __restrict__ sphere,
+export_kernel(const QNode* __restrict__ qnodes, const Node* __restrict__ nodes, const float4* __restrict__ sphere,
               const FrameState* __restrict__ st, int* __restrict__ children, int* __restrict__ parents,
               float* __restrict__ aabbs) {
   const int n = (int)st->n;
@@ -444,15 +462,14 @@ export_kernel(const Node* __restrict__ nodes, const float4* __restrict__ sphere,
       box_of_sphere(sphere[i], bx, bx + 3);
     }
     if (i < n - 1) {
-      const Node nd = nodes[i];
       // canonical Karras links from the traversal links (common.cuh, Node)
-      const uint32_t l = (uint32_t)nd.left, r = (uint32_t)nd.right;
-      int cl = nd.left, cr = nd.right;
-      if (nd.left < 0) {
+      const uint32_t l = qnodes[i].w[6], r = qnodes[i].w[7];
+      int cl = (int)l, cr = (int)r;
+      if (cl < 0) {
         const int f = (int)leaf_range_first(l), c = (int)leaf_range_count(l);
         cl = c == 1 ? n - 1 + f : f + c - 1;
       }
-      if (nd.right < 0) {
+      if (cr < 0) {
         const int f = (int)leaf_range_first(r), c = (int)leaf_range_count(r);
         cr = c == 1 ? n - 1 + f : f;
       }
@@ -465,6 +482,7 @@ export_kernel(const Node* __restrict__ nodes, const float4* __restrict__ sphere,
         parents[cr] = i;
       }
       if (aabbs) {
+        const Node nd = nodes[i];
         float* bx = aabbs + 6 * (size_t)i;
 #pragma unroll
         for (int a = 0; a < 3; ++a) {

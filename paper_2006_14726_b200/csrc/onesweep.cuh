@@ -381,11 +381,27 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
   }
 }
 
-// The tile size follows N (known on the device only): small frames are latency bound, so they
-// get small tiles (more blocks busy, shorter ranking chains); large ones get 4096-element tiles.
+// The tile size follows N (known on the device only).  One wave (every tile has a resident block):
+// the smallest tile that still gives one wave -- small frames are latency bound, so they get the
+// most blocks busy and the shortest ranking chains.  Several waves: the tile size that wastes the
+// least of the last wave (cost model: waves x (items per thread + a fixed per-tile part)).
 #ifndef SPLATS_SORT_BLOCKS
 #define SPLATS_SORT_BLOCKS 2
 #endif
+#ifndef SPLATS_SORT_FIXED
+#define SPLATS_SORT_FIXED 6
+#endif
+__device__ __forceinline__ int sort_pick_items(uint32_t n, uint32_t grid) {
+  int best = SORT_MAX_ITEMS;
+  uint32_t best_cost = 0xffffffffu;
+  for (int items = 4; items <= SORT_MAX_ITEMS; items += 2) {
+    const uint32_t tiles = (n + SORT_THREADS * items - 1) / (SORT_THREADS * items);
+    if (tiles <= grid) return items;   // the smallest single-wave size
+    const uint32_t cost = ((tiles + grid - 1) / grid) * (uint32_t)(items + SPLATS_SORT_FIXED);
+    if (cost <= best_cost) { best_cost = cost; best = items; }
+  }
+  return best;
+}
 __global__ void __launch_bounds__(SORT_THREADS, SPLATS_SORT_BLOCKS)
 onesweep_kernel(SortArgs a) {
   pdl_wait();
@@ -393,17 +409,19 @@ onesweep_kernel(SortArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
   const uint32_t n = a.st->n;
-  const uint32_t slots = gridDim.x * SORT_THREADS;
-#ifndef SPLATS_SORT_MAX_ITEMS
-#define SPLATS_SORT_MAX_ITEMS 16
-#endif
-  if (n <= slots * 4u) run_sort<4>(s, a, n);
+  switch (sort_pick_items(n, gridDim.x)) {
+    case 4: run_sort<4>(s, a, n); break;
+    case 6: run_sort<6>(s, a, n); break;
+    case 8: run_sort<8>(s, a, n); break;
 #if SPLATS_SORT_MAX_ITEMS >= 16
-  else if (n <= slots * 8u) run_sort<8>(s, a, n);
-  else run_sort<16>(s, a, n);
+    case 10: run_sort<10>(s, a, n); break;
+    case 12: run_sort<12>(s, a, n); break;
+    case 14: run_sort<14>(s, a, n); break;
+    default: run_sort<16>(s, a, n); break;
 #else
-  else run_sort<8>(s, a, n);
+    default: run_sort<8>(s, a, n); break;
 #endif
+  }
 }
 
 }  // namespace sw

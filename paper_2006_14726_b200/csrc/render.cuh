@@ -37,7 +37,7 @@ constexpr uint32_t STACK_DONE = 0xffffffffu;  // not a legal leaf-range code (fi
 
 struct RenderParams {
   DevCamera cam;
-  const Node* nodes;
+  const QNode* qnodes;   // 32-byte traversal records (common.cuh)
   const float4* sphere;
   const float4* rgba;
   const uint32_t* ids;
@@ -170,6 +170,7 @@ render_kernel(RenderParams prm) {
   for (int a = 0; a < 3; ++a)
     m = fmaxf(m, fmaxf(fabsf(o[a]), fmaxf(fabsf(prm.st->root_lo[a]), fabsf(prm.st->root_hi[a]))));
   const float pad = 4e-5f * m;
+  const QFrame qf = load_qframe(prm.st);
 
   if (warp == 0) {
     int rect[4] = {0, 0, 0, 0};
@@ -221,15 +222,24 @@ render_kernel(RenderParams prm) {
   float d[3], len;
   pixel_ray(cam, min(x, cam.W - 1), min(y, cam.H - 1), d, len);
 
-  // Conservative slab test (free arithmetic): one FMA per plane,
-  // (plane -+ pad - o) / d = plane * idir - (o +- pad) * idir.
-  float idir[3], oip[3], oim[3];
+  // Conservative slab test (free arithmetic).  A plane of a child box is stored as a 16-bit code q
+  // (plane = qf.lo + q qf.c, S13); as_float(0x4B000000 | q) = 2^23 + q exactly, so
+  //   t = (plane -+ pad - o) / d = (2^23 + q) * (c / d) + ((qf.lo - o) / d -+ pad / |d| - 2^23 c / d)
+  // is ONE byte permute + ONE FMA per plane, and the permute also picks the near / far plane of the
+  // axis by the sign of d (no min / max per axis).  The constant's rounding error is half a code
+  // step in plane units, so the box is padded by one more step than the exact boxes were.
+  float qa[3], bn[3], bf[3];
+  uint32_t seln[3], self[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const float dd = fabsf(d[a]) < 1e-30f ? copysignf(1e-30f, d[a]) : d[a];  // no Inf * 0 in the FMAs
-    idir[a] = 1.0f / dd;
-    oip[a] = (o[a] + pad) * idir[a];
-    oim[a] = (o[a] - pad) * idir[a];
+    const float idir = 1.0f / dd;
+    qa[a] = qf.c[a] * idir;
+    const float b0 = fmaf(-8388608.0f, qa[a], (qf.lo[a] - o[a]) * idir), pd = (pad + qf.c[a]) * fabsf(idir);
+    bn[a] = b0 - pd;
+    bf[a] = b0 + pd;
+    seln[a] = dd >= 0.0f ? 0x7610u : 0x7632u;   // low half = lower plane, high half = upper plane
+    self[a] = dd >= 0.0f ? 0x7632u : 0x7610u;
   }
 
   float C[3] = {0.0f, 0.0f, 0.0f}, A = 0.0f;
@@ -257,26 +267,23 @@ render_kernel(RenderParams prm) {
 
       uint32_t node = n == 1 ? leaf_range_code(0u, 1u) : 0u;
       while (true) {
-        // ---- internal nodes: both child boxes come with the node (2 x 32-byte loads)
+        // ---- internal nodes: both child boxes come with the node (one 32-byte load)
         while ((int)node >= 0) {
-          const f8 ra = ldg_f8(prm.nodes + node), rb = ldg_f8(reinterpret_cast<const char*>(prm.nodes + node) + 32);
-          const float4 n0 = make_float4(ra.v[0], ra.v[1], ra.v[2], ra.v[3]), n1 = make_float4(ra.v[4], ra.v[5], ra.v[6], ra.v[7]);
-          const float4 n2 = make_float4(rb.v[0], rb.v[1], rb.v[2], rb.v[3]), n3 = make_float4(rb.v[4], rb.v[5], rb.v[6], rb.v[7]);
+          const u8x rec = ldg_u8(prm.qnodes + node);
           STAT_ADD(0, 1);
           STAT_MAX(5, sp);
-          // left box: lo (n0.x n0.y n0.z) hi (n0.w n1.x n1.y); right box: lo (n1.z n1.w n2.x) hi (n2.y n2.z n2.w)
-          float a0 = fmaf(n0.x, idir[0], -oip[0]), a1 = fmaf(n0.w, idir[0], -oim[0]);
-          float b0 = fmaf(n0.y, idir[1], -oip[1]), b1 = fmaf(n1.x, idir[1], -oim[1]);
-          float c0 = fmaf(n0.z, idir[2], -oip[2]), c1 = fmaf(n1.y, idir[2], -oim[2]);
-          const float tnl = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), t_lo));
-          const float tfl = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), t_hi));
-          a0 = fmaf(n1.z, idir[0], -oip[0]); a1 = fmaf(n2.y, idir[0], -oim[0]);
-          b0 = fmaf(n1.w, idir[1], -oip[1]); b1 = fmaf(n2.z, idir[1], -oim[1]);
-          c0 = fmaf(n2.x, idir[2], -oip[2]); c1 = fmaf(n2.w, idir[2], -oim[2]);
-          const float tnr = fmaxf(fmaxf(fminf(a0, a1), fminf(b0, b1)), fmaxf(fminf(c0, c1), t_lo));
-          const float tfr = fminf(fminf(fmaxf(a0, a1), fmaxf(b0, b1)), fminf(fmaxf(c0, c1), t_hi));
+#define QPLANE(w, sel) __uint_as_float(__byte_perm((w), 0x4B000000u, (sel)))
+          const float tnl = fmaxf(fmaxf(fmaf(QPLANE(rec.v[0], seln[0]), qa[0], bn[0]), fmaf(QPLANE(rec.v[1], seln[1]), qa[1], bn[1])),
+                                  fmaxf(fmaf(QPLANE(rec.v[2], seln[2]), qa[2], bn[2]), t_lo));
+          const float tfl = fminf(fminf(fmaf(QPLANE(rec.v[0], self[0]), qa[0], bf[0]), fmaf(QPLANE(rec.v[1], self[1]), qa[1], bf[1])),
+                                  fminf(fmaf(QPLANE(rec.v[2], self[2]), qa[2], bf[2]), t_hi));
+          const float tnr = fmaxf(fmaxf(fmaf(QPLANE(rec.v[3], seln[0]), qa[0], bn[0]), fmaf(QPLANE(rec.v[4], seln[1]), qa[1], bn[1])),
+                                  fmaxf(fmaf(QPLANE(rec.v[5], seln[2]), qa[2], bn[2]), t_lo));
+          const float tfr = fminf(fminf(fmaf(QPLANE(rec.v[3], self[0]), qa[0], bf[0]), fmaf(QPLANE(rec.v[4], self[1]), qa[1], bf[1])),
+                                  fminf(fmaf(QPLANE(rec.v[5], self[2]), qa[2], bf[2]), t_hi));
+#undef QPLANE
           const bool hl = tnl <= tfl, hr = tnr <= tfr;
-          const uint32_t cl = __float_as_uint(n3.x), cr = __float_as_uint(n3.y);
+          const uint32_t cl = rec.v[6], cr = rec.v[7];
           if (hl && hr) {
             const bool left_first = tnl <= tnr;
             const uint32_t far = left_first ? cr : cl;

@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -57,7 +58,10 @@ struct Context {
     float4* sphere = nullptr;
     float4* rgba = nullptr;
     uint32_t* ids = nullptr;
-    Node* nodes = nullptr;
+    QNode* qnodes = nullptr;    // 32-byte traversal records, always written
+    Node* nodes = nullptr;      // exact 64-byte records: written by the pyramid / atomic refit modes, and by the
+                                // tiled mode only while SPLATS_OPT_EXACT_NODES is on
+    bool has_exact = false;     // `nodes` holds the exact records of this set's current BVH
   } set[2];
   int cur_set = 0, cur_state = 0;   // what splats_render* reads
   // a build enqueued by splats_update_begin that splats_update_commit has not made current yet
@@ -77,6 +81,7 @@ struct Context {
   int sort_mode = SPLATS_SORT_HYBRID;
   int radius_mode = SPLATS_RADIUS_FOOTPRINT;
   bool pdl = true;                  // programmatic dependent launches between the hot-path kernels
+  bool exact_nodes = false;         // SPLATS_OPT_EXACT_NODES
   bool overlap = false;             // consecutive independent renders may run concurrently (SPLATS_OPT_OVERLAP)
   float radius_param = 0.0f;
   // staging for the *_host calls: copies run on their own streams, double / triple buffered,
@@ -187,7 +192,7 @@ void free_all(Context* c) {
   cudaFree(c->state); cudaFree(c->tile_count); cudaFree(c->pack_tile_count); cudaFree(c->sched); cudaFree(c->traced);
   cudaFree(c->key[0]); cudaFree(c->key[1]); cudaFree(c->val[0]); cudaFree(c->val[1]);
   cudaFree(c->status);
-  for (int i = 0; i < 2; ++i) { cudaFree(c->set[i].sphere); cudaFree(c->set[i].rgba); cudaFree(c->set[i].ids); cudaFree(c->set[i].nodes); }
+  for (int i = 0; i < 2; ++i) { cudaFree(c->set[i].sphere); cudaFree(c->set[i].rgba); cudaFree(c->set[i].ids); cudaFree(c->set[i].qnodes); cudaFree(c->set[i].nodes); }
   if (c->build_stream) cudaStreamDestroy(c->build_stream);
   if (c->ev_begin) cudaEventDestroy(c->ev_begin);
   if (c->ev_built) cudaEventDestroy(c->ev_built);
@@ -268,7 +273,7 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   const int tset = (int)(c->frame & 1u), tstate = (int)(c->frame % 3u);
   FrameState* st = c->state + tstate;
   FrameState* st_next = c->state + (tstate + 1) % 3;
-  const Context::BvhSet& bs = c->set[tset];
+  Context::BvhSet& bs = c->set[tset];
   const int tiles = P > 0 ? (int)((P + TILE_PX - 1) / TILE_PX) : 1;
   cudaStream_t s = async ? c->build_stream : c->stream;
   const bool prof = c->profiling && !async;   // per-stage events live on the caller's stream
@@ -322,18 +327,24 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
                                                        c->leaf_parent);
     if (prof) m[4] = c->mark();
     refit_kernel<<<lgrid, LBVH_THREADS, 0, s>>>(bs.sphere, c->leaf_parent, bs.nodes, st);
+    quantise_nodes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>((const Node*)bs.nodes, (const FrameState*)st, bs.qnodes);
+    c->launches += 1;
+    bs.has_exact = true;
   } else if (c->refit_mode == SPLATS_REFIT_TILED) {
     // gather + leaf boxes + pyramid + every node whose range lies inside one tile of sorted leaves;
     // then the few nodes that span tiles (lbvh.cuh)
     const int tgrid = P > 0 ? (int)((P + TT_LEAVES - 1) / TT_LEAVES) : 1;
     launch(pdl, tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
-           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.nodes, c->ranges, c->tile_min, c->tile_fb);
+           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.qnodes, c->exact_nodes ? bs.nodes : (Node*)nullptr, c->ranges, c->tile_min,
+           c->tile_fb);
+    bs.has_exact = c->exact_nodes;
     if (prof) m[4] = c->mark();
     int nt_log = 0;
     while ((1 << nt_log) < tgrid) ++nt_log;
     const int sgrid2 = std::min(c->num_sms * 8, (tgrid * TT_QMAX + 7) / 8);   // persistent, one warp per queued node; idle blocks exit at once
     launch(pdl, tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
-           (const float4*)bs.sphere, (const float4*)c->pyr, bs.nodes, (const uint8_t*)c->tile_min, (const uint16_t*)c->tile_fb, nt_log);
+           (const float4*)bs.sphere, (const float4*)c->pyr, bs.qnodes, c->exact_nodes ? bs.nodes : (Node*)nullptr, (const uint8_t*)c->tile_min,
+           (const uint16_t*)c->tile_fb, nt_log);
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
     launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
@@ -341,7 +352,9 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     // the hierarchy (keys only) runs beside the pyramid (ids only); boxes_kernel joins them
     launch(pdl, hierarchy_kernel, lgrid, LBVH_THREADS, 0, s, (const uint64_t*)c->key[0], (const FrameState*)st, c->ranges, pdl ? 0 : 1);
     launch(pdl, boxes_kernel, lgrid, LBVH_THREADS, 0, s, (const int4*)c->ranges, (const float4*)bs.sphere, (const float4*)c->pyr, st, bs.nodes);
-    c->launches += 1;
+    launch(pdl, quantise_nodes_kernel, lgrid, LBVH_THREADS, 0, s, (const Node*)bs.nodes, (const FrameState*)st, bs.qnodes);
+    c->launches += 2;
+    bs.has_exact = true;
   }
   if (prof) m[5] = c->mark();
   c->launches += 4 + sort_launches;
@@ -378,7 +391,7 @@ int do_update_frame(Context* c, const float* color, const float* depth, const wr
 int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool first_hit = false, bool rgba8 = false) {
   RenderParams prm;
   prm.cam = make_camera(cam, W2, H2);
-  prm.nodes = c->set[c->cur_set].nodes;
+  prm.qnodes = c->set[c->cur_set].qnodes;
   prm.sphere = c->set[c->cur_set].sphere;
   prm.rgba = c->set[c->cur_set].rgba;
   prm.ids = c->set[c->cur_set].ids;
@@ -479,6 +492,7 @@ int splats_create(void* cuda_stream, int max_W, int max_H) {
     e = dmalloc(&c->set[i].sphere, cap);
     if (e == cudaSuccess) e = dmalloc(&c->set[i].rgba, cap);
     if (e == cudaSuccess) e = dmalloc(&c->set[i].ids, cap);
+    if (e == cudaSuccess) e = dmalloc(&c->set[i].qnodes, cap);
     if (e == cudaSuccess) e = dmalloc(&c->set[i].nodes, cap);
   }
   if (e == cudaSuccess) e = dmalloc(&c->leaf_parent, cap);
@@ -854,10 +868,12 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   if (n == 0) return SPLATS_OK;
   if (keys) CU(cudaMemcpyAsync(keys, c->key[0], (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream));
   if (perm) CU(cudaMemcpyAsync(perm, c->set[c->cur_set].ids, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
+  if (node_aabbs && !c->set[c->cur_set].has_exact)
+    return fail(SPLATS_ESTATE, "splats_export: the exact node boxes were not stored by the last build (set SPLATS_OPT_EXACT_NODES before the update)");
   if (children || parents || node_aabbs) {
     if (parents) CU(cudaMemsetAsync(parents, 0xff, (size_t)(2 * n - 1) * sizeof(int), c->stream));
     const int grid = (int)((n + LBVH_THREADS - 1) / LBVH_THREADS);
-    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->set[c->cur_set].nodes, c->set[c->cur_set].sphere, c->state + c->cur_state, children, parents,
+    export_kernel<<<grid, LBVH_THREADS, 0, c->stream>>>(c->set[c->cur_set].qnodes, c->set[c->cur_set].nodes, c->set[c->cur_set].sphere, c->state + c->cur_state, children, parents,
                                                         node_aabbs);
     c->launches += 1;
     CU(cudaGetLastError());
@@ -871,6 +887,8 @@ int splats_export_child_boxes(float* child_boxes) {
   Context* c = g_ctx;
   if (!child_boxes) return fail(SPLATS_EINVAL, "null pointer argument");
   if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export_child_boxes before any update");
+  if (!c->set[c->cur_set].has_exact)
+    return fail(SPLATS_ESTATE, "splats_export_child_boxes: the exact node boxes were not stored by the last build (set SPLATS_OPT_EXACT_NODES before the update)");
   unsigned n = 0;
   int rc = splats_count(&n);
   if (rc) return rc;
@@ -878,6 +896,31 @@ int splats_export_child_boxes(float* child_boxes) {
   // the first 48 bytes of every 64-byte record, exactly as the traversal reads them
   CU(cudaMemcpy2DAsync(child_boxes, 12 * sizeof(float), c->set[c->cur_set].nodes, sizeof(Node), 12 * sizeof(float), n - 1,
                        cudaMemcpyDeviceToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return SPLATS_OK;
+}
+
+int splats_export_qnodes(unsigned* qnodes, float* frame) {
+  if (!g_ctx) return fail(SPLATS_ESTATE, "no context");
+  Context* c = g_ctx;
+  if (!c->has_bvh) return fail(SPLATS_ENOBVH, "splats_export_qnodes before any update");
+  unsigned n = 0;
+  int rc = splats_count(&n);
+  if (rc) return rc;
+  // the records exactly as the traversal reads them
+  if (qnodes && n > 1) CU(cudaMemcpyAsync(qnodes, c->set[c->cur_set].qnodes, (size_t)(n - 1) * sizeof(QNode), cudaMemcpyDeviceToDevice, c->stream));
+  if (frame) {   // bounds of the centres and the largest radius: what the quantisation frame is derived from
+    FrameState hs;
+    CU(cudaMemcpyAsync(&hs, c->state + c->cur_state, offsetof(FrameState, hist), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    auto dec = [](uint32_t u) { uint32_t b = (u & 0x80000000u) ? (u & 0x7fffffffu) : ~u; float f; memcpy(&f, &b, 4); return f; };
+    float h[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (n) {
+      for (int a = 0; a < 3; ++a) { h[a] = dec(hs.lo[a]); h[3 + a] = dec(hs.hi[a]); }
+      h[6] = dec(hs.rmax);
+    }
+    CU(cudaMemcpyAsync(frame, h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+  }
   CU(cudaStreamSynchronize(c->stream));
   return SPLATS_OK;
 }
@@ -926,6 +969,10 @@ int splats_set_option(int option, int value) {
       if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_OVERLAP takes 0 or 1");
       g_ctx->overlap = value != 0;
       g_ctx->serialize_next_render = true;
+      return SPLATS_OK;
+    case SPLATS_OPT_EXACT_NODES:
+      if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_EXACT_NODES takes 0 or 1");
+      g_ctx->exact_nodes = value != 0;
       return SPLATS_OK;
     case SPLATS_OPT_PDL:
       if (value != 0 && value != 1) return fail(SPLATS_EINVAL, "SPLATS_OPT_PDL takes 0 or 1");

@@ -148,7 +148,10 @@ template <class Gather>
 __global__ void __launch_bounds__(TT_THREADS)
 tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
                  float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, float4* pyr,
-                 Node* __restrict__ nodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min, uint16_t* __restrict__ tile_fb) {
+                 QNode* __restrict__ qnodes, Node* __restrict__ nodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min,
+                 uint16_t* __restrict__ tile_fb) {
+  // qnodes: the traversal records (always); nodes: the exact 64-byte records, null unless
+  // SPLATS_OPT_EXACT_NODES is on (parity tests, splats_export)
   pdl_wait();
   pdl_trigger();
   extern __shared__ __align__(16) unsigned char tt_smem_raw[];
@@ -159,6 +162,7 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int base = blockIdx.x * TT_LEAVES;
   const float INF = __int_as_float(0x7f800000);
+  const QFrame qf = load_qframe(st);
 
   // ---- (1) interleaved over the tile (coalesced): deltas of the adjacent pairs (l, l + 1), + 1;
   // gather of the splats into sorted order; leaf boxes -> staging
@@ -298,33 +302,17 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
       if (g >= 0) s.wl[at + pos + __popc(m & ((1u << lane) - 1))] = (uint16_t)g;
     }
   };
-  // a finished node: write its record, report upwards; returns the parent if that completed it
+  // a finished node reports upwards; returns the parent if that completed it.  (Its record is written
+  // after the rounds, from the slots: nothing but the propagation is on the rounds' critical path.)
   auto finish = [&](int l) -> int {
     const int ls = tt_slot(l);
     const int p = s.cend[0][ls], q = s.cend[1][ls];
-    Box6 L, R;
+    Box6 U, R;
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { L.v[a] = s.cbox[0][a][ls]; R.v[a] = s.cbox[1][a][ls]; }
-    const int first = base + p + 1, last = base + q, g = base + l;
-    Box6 U = L;
+    for (int a = 0; a < 6; ++a) { U.v[a] = s.cbox[0][a][ls]; R.v[a] = s.cbox[1][a][ls]; }
     U.merge(R);
     bool il;
-    const int up = tile_report(s, p, q, U, il);
-    const int idx = il ? last : first;
-    const int cnt_l = g - first + 1, cnt_r = last - g;
-    const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
-    const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-    f8 ra, rb;
-    ra.v[0] = L.v[0]; ra.v[1] = L.v[1]; ra.v[2] = L.v[2]; ra.v[3] = L.v[3]; ra.v[4] = L.v[4]; ra.v[5] = L.v[5]; ra.v[6] = R.v[0]; ra.v[7] = R.v[1];
-    rb.v[0] = R.v[2]; rb.v[1] = R.v[3]; rb.v[2] = R.v[4]; rb.v[3] = R.v[5];
-    rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
-    stg_f8(nodes + idx, ra);
-    stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
-    if (idx == 0) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { st->root_lo[a] = U.v[a]; st->root_hi[a] = U.v[3 + a]; }
-    }
-    return up;
+    return tile_report(s, p, q, U, il);
   };
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -367,15 +355,43 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   }
   __syncthreads();
 
-  // ---- the splits of the tile whose node is not complete: queue them with what is known
-#pragma unroll
+  // ---- every split of the tile, dense: a complete node (both children arrived) is written out as its
+  // traversal record (and, on request, the exact 64-byte record); an incomplete one is queued with
+  // what is known
+#pragma unroll 1
   for (int j = 0; j < 4; ++j) {
     const int l = tid + j * TT_THREADS, g = base + l;
     if (g + 1 >= n) continue;
     const uint32_t arr = (s.arrived[l >> 2] >> (8 * (l & 3))) & 3u;
-    if (arr == 3u) continue;
-    const uint32_t slot = atomicAdd(&s.qn, 1u);
-    s.q[slot] = make_int4(g, (arr & 1u) ? base + s.cend[0][tt_slot(l)] + 1 : -1, (arr & 2u) ? base + s.cend[1][tt_slot(l)] : -1, (int)s.d[l]);
+    const int ls = tt_slot(l);
+    if (arr != 3u) {
+      const uint32_t slot = atomicAdd(&s.qn, 1u);
+      s.q[slot] = make_int4(g, (arr & 1u) ? base + s.cend[0][ls] + 1 : -1, (arr & 2u) ? base + s.cend[1][ls] : -1, (int)s.d[l]);
+      continue;
+    }
+    const int p = s.cend[0][ls], q = s.cend[1][ls];
+    float L[6], R[6];
+#pragma unroll
+    for (int a = 0; a < 6; ++a) { L[a] = s.cbox[0][a][ls]; R[a] = s.cbox[1][a][ls]; }
+    const uint32_t dl = p < 0 ? s.dleft : s.d[p], dr = s.d[q];
+    const int first = base + p + 1, last = base + q;
+    const int idx = dr > dl ? last : first;   // Karras: a left child is numbered by its last leaf, a right child by its first
+    const int cnt_l = g - first + 1, cnt_r = last - g;
+    const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
+    const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
+    store_qnode(qnodes + idx, L, R, left, right, qf);
+    if (nodes) {
+      f8 ra, rb;
+      ra.v[0] = L[0]; ra.v[1] = L[1]; ra.v[2] = L[2]; ra.v[3] = L[3]; ra.v[4] = L[4]; ra.v[5] = L[5]; ra.v[6] = R[0]; ra.v[7] = R[1];
+      rb.v[0] = R[2]; rb.v[1] = R[3]; rb.v[2] = R[4]; rb.v[3] = R[5];
+      rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
+      stg_f8(nodes + idx, ra);
+      stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
+    }
+    if (idx == 0) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L[a], R[a]); st->root_hi[a] = fmaxf(L[3 + a], R[3 + a]); }
+    }
   }
   __syncthreads();
   const uint32_t qn = s.qn;
@@ -510,7 +526,7 @@ __device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, c
 constexpr int SPINE_THREADS = 256;
 __global__ void __launch_bounds__(SPINE_THREADS)
 tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4* __restrict__ queue,
-                  const float4* __restrict__ sphere, const float4* __restrict__ pyr, Node* __restrict__ nodes,
+                  const float4* __restrict__ sphere, const float4* __restrict__ pyr, QNode* __restrict__ qnodes, Node* __restrict__ nodes,
                   const uint8_t* __restrict__ tile_min, const uint16_t* __restrict__ tile_fb, int nt_log) {
   pdl_wait();
   pdl_trigger();
@@ -522,6 +538,8 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
   if ((int)(blockIdx.x * WPB) >= qn) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ntiles = (n + TT_LEAVES - 1) / TT_LEAVES;
+  const int qax = (lane < 3 ? lane : lane - 3) % 3;   // lanes 0..5 write one word of the traversal record each: their axis' frame
+  const float my_qlo = __ldcg(&st->qf[qax]), my_qs = __ldcg(&st->qf[3 + qax]);
   TileMins tm;
   tm.m = m;
   tm.log = nt_log;
@@ -568,17 +586,31 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
         R.hi[a] = fmaxf(R.hi[a], __shfl_xor_sync(0xffffffffu, R.hi[a], o));
       }
     }
-    if (lane == 0) {
+    {
       const int cnt_l = g - first + 1, cnt_r = last - g;
       const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
       const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-      f8 ra, rb;
-      ra.v[0] = L.lo[0]; ra.v[1] = L.lo[1]; ra.v[2] = L.lo[2]; ra.v[3] = L.hi[0]; ra.v[4] = L.hi[1]; ra.v[5] = L.hi[2]; ra.v[6] = R.lo[0]; ra.v[7] = R.lo[1];
-      rb.v[0] = R.lo[2]; rb.v[1] = R.hi[0]; rb.v[2] = R.hi[1]; rb.v[3] = R.hi[2];
-      rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
-      stg_f8(nodes + idx, ra);
-      stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
-      if (idx == 0) {
+      if (lane < 8) {   // one word of the traversal record per lane (every lane holds the reduced boxes): one 32-byte store
+        const int a = lane < 3 ? lane : lane - 3;
+        uint32_t w;
+        if (lane < 6) {
+          const float plo = lane < 3 ? (a == 0 ? L.lo[0] : a == 1 ? L.lo[1] : L.lo[2]) : (a == 0 ? R.lo[0] : a == 1 ? R.lo[1] : R.lo[2]);
+          const float phi = lane < 3 ? (a == 0 ? L.hi[0] : a == 1 ? L.hi[1] : L.hi[2]) : (a == 0 ? R.hi[0] : a == 1 ? R.hi[1] : R.hi[2]);
+          w = quant_planes(plo, phi, my_qlo, my_qs);
+        } else {
+          w = (uint32_t)(lane == 6 ? left : right);
+        }
+        qnodes[idx].w[lane] = w;
+      }
+      if (lane == 0 && nodes) {
+        f8 ra, rb;
+        ra.v[0] = L.lo[0]; ra.v[1] = L.lo[1]; ra.v[2] = L.lo[2]; ra.v[3] = L.hi[0]; ra.v[4] = L.hi[1]; ra.v[5] = L.hi[2]; ra.v[6] = R.lo[0]; ra.v[7] = R.lo[1];
+        rb.v[0] = R.lo[2]; rb.v[1] = R.hi[0]; rb.v[2] = R.hi[1]; rb.v[3] = R.hi[2];
+        rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
+        stg_f8(nodes + idx, ra);
+        stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
+      }
+      if (lane == 0 && idx == 0) {
 #pragma unroll
         for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
       }

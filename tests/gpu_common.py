@@ -15,8 +15,12 @@ RGBA_BAD_FRACTION = 1e-4  # ... with at most 0.01 % of pixels beyond that
 class Session:
     """One library context (the C ABI has a single global one)."""
 
-    def __init__(self, max_W, max_H):
+    def __init__(self, max_W, max_H, exact_nodes=True):
         sp.splats_create(max_W, max_H)
+        # the parity tests also want the exact float32 node boxes, which the default build computes but
+        # does not store (include/splats.h, SPLATS_OPT_EXACT_NODES); the traversal records are the same
+        # either way (tests/test_gpu_parity.py::test_exact_nodes_option_changes_nothing)
+        sp.splats_set_option(sp.OPT_EXACT_NODES, 1 if exact_nodes else 0)
 
     def close(self):
         sp.splats_destroy()
@@ -39,9 +43,34 @@ class Session:
         return out.cpu().numpy()
 
 
-def assert_bvh_bit_exact(sc):
-    """Morton codes, sorted permutation, topology, AABBs, splats: bit-exact against the oracle."""
-    ex = sp.splats_export()
+def quantised_records(sc):
+    """The 32-byte traversal records (include/splats.h, splats_export_qnodes, S13)
+    that follow from the oracle's exact tree: every plane of every child box quantised to 16 bits over
+    [lo - rmax, hi + rmax], lower planes rounded down, upper planes up, float32 operation by operation."""
+    n = sc["N"]
+    f32 = np.float32
+    rmax = f32(sc["sphere_sorted"][:, 3].max())
+    qlo = (sc["lo"].astype(f32) - rmax).astype(f32)
+    ext = ((sc["hi"].astype(f32) + rmax).astype(f32) - qlo).astype(f32)
+    with np.errstate(divide="ignore"):
+        s = np.where(ext > 0, (f32(65535.0) / ext).astype(f32), f32(0.0)).astype(f32)
+    boxes = sc["aabbs"][sc["children"]].astype(f32)               # (n-1, 2, 6): lo xyz, hi xyz of each child
+    ul = np.floor(((boxes[:, :, 0:3] - qlo).astype(f32) * s).astype(f32))
+    uh = np.ceil(((boxes[:, :, 3:6] - qlo).astype(f32) * s).astype(f32))
+    ql = np.clip(ul, 0, 65535).astype(np.uint32)
+    qh = np.clip(uh, 0, 65535).astype(np.uint32)
+    rec = np.zeros((n - 1, 8), dtype=np.uint32)
+    rec[:, 0:6] = (ql | (qh << np.uint32(16))).reshape(n - 1, 6)
+    ch = sc["children"].astype(np.int64)
+    leaf = ch >= n - 1
+    rec[:, 6:8] = np.where(leaf, 0x80000000 | (ch - (n - 1)), ch).astype(np.uint32)
+    return rec, np.concatenate([sc["lo"].astype(f32), sc["hi"].astype(f32), [rmax]]).astype(f32)
+
+
+def assert_bvh_bit_exact(sc, exact=True):
+    """Morton codes, sorted permutation, topology, AABBs (exact, and the quantised records the
+    traversal reads), splats: bit-exact against the oracle."""
+    ex = sp.splats_export(aabbs=exact)
     n = sc["N"]
     assert ex["N"] == n
     if n == 0:
@@ -50,11 +79,17 @@ def assert_bvh_bit_exact(sc):
     np.testing.assert_array_equal(ex["perm"].cpu().numpy().view(np.uint32), sc["sorted_ids"])
     np.testing.assert_array_equal(ex["children"].cpu().numpy(), sc["children"])
     np.testing.assert_array_equal(ex["parents"].cpu().numpy(), sc["parents"])
-    np.testing.assert_array_equal(ex["node_aabbs"].cpu().numpy().view(np.uint32), sc["aabbs"].view(np.uint32))
-    if n > 1:   # the stored child boxes the traversal reads, one by one (not only their union)
-        cb = sp.splats_export_child_boxes().cpu().numpy().view(np.uint32).reshape(n - 1, 2, 6)
-        want = sc["aabbs"].view(np.uint32)[sc["children"]]          # (n-1, 2, 6): box of each child node / leaf
-        np.testing.assert_array_equal(cb, want)
+    q = sp.splats_export_qnodes()
+    want_rec, want_frame = quantised_records(sc) if n > 1 else (np.zeros((0, 8), np.uint32), None)
+    if n > 1:   # what the traversal reads, word by word
+        np.testing.assert_array_equal(q["qnodes"].cpu().numpy().view(np.uint32), want_rec)
+        np.testing.assert_array_equal(q["frame"].cpu().numpy().view(np.uint32), want_frame.view(np.uint32))
+    if exact:
+        np.testing.assert_array_equal(ex["node_aabbs"].cpu().numpy().view(np.uint32), sc["aabbs"].view(np.uint32))
+        if n > 1:   # the exact child boxes of every record, one by one (not only their union)
+            cb = sp.splats_export_child_boxes().cpu().numpy().view(np.uint32).reshape(n - 1, 2, 6)
+            want = sc["aabbs"].view(np.uint32)[sc["children"]]          # (n-1, 2, 6): box of each child node / leaf
+            np.testing.assert_array_equal(cb, want)
     es = sp.splats_export_splats()
     np.testing.assert_array_equal(es["sphere"].cpu().numpy().view(np.uint32), sc["sphere_sorted"].view(np.uint32))
     np.testing.assert_array_equal(es["rgba"].cpu().numpy().view(np.uint32), sc["rgba_sorted"].view(np.uint32))

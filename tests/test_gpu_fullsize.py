@@ -75,7 +75,7 @@ def test_config3_bench_step_in_bench_launch_configuration():
     build = 14
     color, depth = synth.source_frame(cfg, build)
     sc = oracle.build_scene(color, depth, cfg.src_cams[build], cfg.W, cfg.H, cfg.r_scale)
-    with Session(cfg.W, cfg.H):
+    with Session(cfg.W, cfg.H, exact_nodes=False):   # the library's defaults, as bench.py runs it
         sp.splats_set_option(sp.OPT_OVERLAP, 1)
         dc, dd = torch.from_numpy(color).cuda(), torch.from_numpy(depth).cuda()
         outs = [torch.full((cfg.H, cfg.W, 4), -7.0, dtype=torch.float32, device="cuda") for _ in range(4)]
@@ -84,7 +84,7 @@ def test_config3_bench_step_in_bench_launch_configuration():
             for j in range(4):
                 sp.splats_render(cfg.dst_cams[4 * build + j], cfg.W, cfg.H, outs[j])
         torch.cuda.synchronize()
-        assert_bvh_bit_exact(sc)
+        assert_bvh_bit_exact(sc, exact=False)
         for j in range(4):
             ref = oracle.render(sc, cfg.dst_cams[4 * build + j], cfg.W, cfg.H, "bvh")
             assert_rgba_close(outs[j].cpu().numpy(), ref, f"display frame {4 * build + j}")

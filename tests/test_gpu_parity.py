@@ -492,3 +492,48 @@ def test_decoupled_build_begin_commit():
         # after the loop the current BVH is frame 0 again
         assert_bvh_bit_exact(scenes[0])
         assert_rgba_close(reuse.cpu().numpy(), oracle.render(scenes[0], cams[0], 160, 120, "bvh"), "reused image")
+
+
+def test_exact_nodes_option_changes_nothing():
+    # SPLATS_OPT_EXACT_NODES only adds the 64-byte exact records: keys, topology, the quantised
+    # traversal records and the images are the same with and without it; without it the exact boxes
+    # cannot be exported
+    cfg = synth.make_config(1)
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+    res = {}
+    for exact in (False, True):
+        with Session(cfg.W, cfg.H, exact_nodes=exact) as s:
+            s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+            assert_bvh_bit_exact(sc, exact=exact)
+            if not exact:
+                with pytest.raises(sp.SplatsError):
+                    sp.splats_export()
+                with pytest.raises(sp.SplatsError):
+                    sp.splats_export_child_boxes()
+            res[exact] = (sp.splats_export_qnodes()["qnodes"].cpu().numpy(), s.render(cfg.dst_cams[1], cfg.W, cfg.H))
+    assert np.array_equal(res[False][0], res[True][0])
+    assert np.array_equal(res[False][1], res[True][1])
+
+
+def test_quantised_boxes_contain_the_exact_ones():
+    # decode the traversal records in float64 and compare with the oracle's exact boxes: never smaller,
+    # at most one code step larger per plane (independent of quantised_records' float32 restatement)
+    W, H = 200, 120
+    color, depth, _ = synth.random_frame(W, H, 5, fill=0.8)
+    cam = synth.orbit_camera(20.0)
+    sc = oracle.build_scene(color, depth, cam, W, H, 1.5)
+    with Session(W, H) as s:
+        s.update(color, depth, cam, W, H, 1.5)
+        q = sp.splats_export_qnodes()
+    rec = q["qnodes"].cpu().numpy().view(np.uint32)
+    fr = q["frame"].cpu().numpy().astype(np.float64)
+    qlo = fr[0:3] - fr[6]
+    step = ((fr[3:6] + fr[6]) - qlo) / 65535.0
+    w = rec[:, 0:6].reshape(-1, 2, 3)
+    lo = qlo + (w & 0xffff) * step
+    hi = qlo + (w >> 16) * step
+    want = sc["aabbs"][sc["children"]].astype(np.float64)
+    eps = 1e-6 * np.abs(want).max()
+    assert np.all(lo <= want[:, :, 0:3] + eps) and np.all(hi >= want[:, :, 3:6] - eps)
+    assert np.all(lo >= want[:, :, 0:3] - step - eps) and np.all(hi <= want[:, :, 3:6] + step + eps)
