@@ -153,12 +153,16 @@ __global__ void __launch_bounds__(RENDER_THREADS, 1024 / RENDER_THREADS)
 render_kernel(RenderParams prm) {
   if (prm.wait_prev) pdl_wait();
   pdl_trigger();
-  __shared__ uint32_t s_node[SSTACK][RENDER_THREADS];
-  __shared__ float s_tn[SSTACK][RENDER_THREADS];
+  // stack entry = (node, entry distance) as one 8-byte word; [depth][thread]: conflict free.  Addressed through
+  // one precomputed shared-memory address (the compiler otherwise rebuilds it at every push and pop).
+  __shared__ uint2 s_stack[SSTACK][RENDER_THREADS];
   __shared__ int s_rect[4];
   uint32_t l_node[LSTACK];
   float l_tn[LSTACK];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t s_base;   // opaque to the compiler, or it is rematerialised (thread id, CTA id, shifts) at every use
+  asm volatile("mov.u32 %0, %1;" : "=r"(s_base) : "r"((uint32_t)__cvta_generic_to_shared(&s_stack[0][tid])));
+  constexpr uint32_t S_STRIDE = RENDER_THREADS * sizeof(uint2);
   const DevCamera& cam = prm.cam;
   const int n = (int)prm.st->n;
   const float INF = __int_as_float(0x7f800000);
@@ -259,8 +263,11 @@ render_kernel(RenderParams prm) {
       auto pop = [&]() -> uint32_t {  // next stack entry that is not culled by t_hi
         while (sp > 0) {
           --sp;
-          const float tn = sp < SSTACK ? s_tn[sp][tid] : l_tn[sp - SSTACK];
-          if (tn <= t_hi) return sp < SSTACK ? s_node[sp][tid] : l_node[sp - SSTACK];
+          uint32_t nd;
+          float tn;
+          if (sp < SSTACK) asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(nd), "=f"(tn) : "r"(s_base + sp * S_STRIDE));
+          else { nd = l_node[sp - SSTACK]; tn = l_tn[sp - SSTACK]; }
+          if (tn <= t_hi) return nd;
         }
         return STACK_DONE;
       };
@@ -289,7 +296,7 @@ render_kernel(RenderParams prm) {
             const uint32_t far = left_first ? cr : cl;
             const float tfar = left_first ? tnr : tnl;
             node = left_first ? cl : cr;
-            if (sp < SSTACK) { s_node[sp][tid] = far; s_tn[sp][tid] = tfar; }
+            if (sp < SSTACK) asm volatile("st.shared.v2.b32 [%0], {%1, %2};" :: "r"(s_base + sp * S_STRIDE), "r"(far), "f"(tfar) : "memory");
             else { l_node[sp - SSTACK] = far; l_tn[sp - SSTACK] = tfar; }
             ++sp;
           } else if (hl) {
