@@ -24,6 +24,9 @@ constexpr int RENDER_THREADS = 32;   // one warp = one 8x4 tile per block: the f
 constexpr int KBUF = SPLATS_KBUF;
 constexpr int SSTACK = 12;  // deeper entries live in local memory; 12 leaves more of the SM's 256 KB to L1 than 16 (1 % per step)
 constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
+#ifndef SPLATS_POSTPONE
+#define SPLATS_POSTPONE 0
+#endif
 constexpr uint32_t EMPTY_LEAF = 0xffffffffu;
 constexpr uint32_t STACK_DONE = 0xffffffffu;  // not a legal leaf-range code (first < 2^26 - 1)
 
@@ -149,7 +152,10 @@ __device__ __forceinline__ void screen_rect(const DevCamera& cam, const float lo
 // OUT8 = true writes the pixel as RGBA8 (round(255 c), the colour format of the wire, S10) instead
 // of four float32: a quarter of the bytes for a client that only displays the image.
 template <int KBUF, bool FIRST, bool OUT8 = false>
-__global__ void __launch_bounds__(RENDER_THREADS, 1024 / RENDER_THREADS)
+#ifndef SPLATS_RENDER_BLOCKS
+#define SPLATS_RENDER_BLOCKS (1024 / RENDER_THREADS)
+#endif
+__global__ void __launch_bounds__(RENDER_THREADS, SPLATS_RENDER_BLOCKS)
 render_kernel(RenderParams prm) {
   if (prm.wait_prev) pdl_wait();
   pdl_trigger();
@@ -272,7 +278,7 @@ render_kernel(RenderParams prm) {
         return STACK_DONE;
       };
 
-      uint32_t node = n == 1 ? leaf_range_code(0u, 1u) : 0u;
+      uint32_t node = n == 1 ? leaf_range_code(0u, 1u) : 0u, pend = STACK_DONE;
       while (true) {
         // ---- internal nodes: both child boxes come with the node (one 32-byte load)
         while ((int)node >= 0) {
@@ -291,6 +297,7 @@ render_kernel(RenderParams prm) {
 #undef QPLANE
           const bool hl = tnl <= tfl, hr = tnr <= tfr;
           const uint32_t cl = rec.v[6], cr = rec.v[7];
+          bool need_pop = false;
           if (hl && hr) {
             const bool left_first = tnl <= tnr;
             const uint32_t far = left_first ? cr : cl;
@@ -304,39 +311,51 @@ render_kernel(RenderParams prm) {
           } else if (hr) {
             node = cr;
           } else {
-            node = pop();
+            need_pop = true;
           }
+#if SPLATS_POSTPONE
+          // a lane that reaches its first leaf keeps it for later and goes on with the next stack entry: the warp
+          // stays in this loop together for longer and tests two leaves per lane in the phase below
+          if (!need_pop && (int)node < 0 && pend == STACK_DONE) { pend = node; need_pop = true; }
+#endif
+          if (need_pop) node = pop();
         }
-        if (node == STACK_DONE) break;
-        // ---- leaf range: <= LEAF_MAX consecutive splats of the sorted order
-        const uint32_t first = leaf_range_first(node), cnt = leaf_range_count(node);
-        STAT_ADD(4, 1);
-        for (uint32_t j = 0; j < cnt; ++j) {
-          const uint32_t leaf = first + j;
-          const float4 s = __ldg(prm.sphere + leaf);
-          float t;
-          STAT_ADD(1, 1);
-          if (ray_sphere(o, d, s, t) && t <= t_hi &&
-              (t > cur_t || (t == cur_t && __ldg(prm.ids + leaf) > cur_id))) {
-            STAT_ADD(2, 1);
-            kb.insert(t, leaf, __ldg(&prm.rgba[leaf].w), prm.ids);
-            if (FIRST) {
-              t_hi = kb.t[0];  // nothing beyond the nearest hit so far matters
-            } else {
-              // distance at which the composite below (oracle step O9, same operations in the
-              // same order) reaches alpha >= 0.99: later hits cannot contribute
-              float a = A, t_cut = INF;
+        // ---- leaves: the postponed one, then the one the descent stopped at (<= LEAF_MAX consecutive splats each)
+#pragma unroll 1
+        for (int which = SPLATS_POSTPONE ? 0 : 1; which < 2; ++which) {
+          const uint32_t code = which == 0 ? pend : node;
+          if (code == STACK_DONE) continue;
+          const uint32_t first = leaf_range_first(code), cnt = leaf_range_count(code);
+          STAT_ADD(4, 1);
+          for (uint32_t j = 0; j < cnt; ++j) {
+            const uint32_t leaf = first + j;
+            const float4 s = __ldg(prm.sphere + leaf);
+            float t;
+            STAT_ADD(1, 1);
+            if (ray_sphere(o, d, s, t) && t <= t_hi &&
+                (t > cur_t || (t == cur_t && __ldg(prm.ids + leaf) > cur_id))) {
+              STAT_ADD(2, 1);
+              kb.insert(t, leaf, __ldg(&prm.rgba[leaf].w), prm.ids);
+              if (FIRST) {
+                t_hi = kb.t[0];  // nothing beyond the nearest hit so far matters
+              } else {
+                // distance at which the composite below (oracle step O9, same operations in the
+                // same order) reaches alpha >= 0.99: later hits cannot contribute
+                float a = A, t_cut = INF;
 #pragma unroll
-              for (int i = 0; i < KBUF; ++i) {
-                if (kb.leaf[i] != EMPTY_LEAF && t_cut == INF) {
-                  a = fma_(sub_(1.0f, a), kb.al[i], a);
-                  if (a >= 0.99f) t_cut = kb.t[i];
+                for (int i = 0; i < KBUF; ++i) {
+                  if (kb.leaf[i] != EMPTY_LEAF && t_cut == INF) {
+                    a = fma_(sub_(1.0f, a), kb.al[i], a);
+                    if (a >= 0.99f) t_cut = kb.t[i];
+                  }
                 }
+                t_hi = fminf(kb.t[KBUF - 1], t_cut);
               }
-              t_hi = fminf(kb.t[KBUF - 1], t_cut);
             }
           }
         }
+        pend = STACK_DONE;
+        if (node == STACK_DONE) break;
         node = pop();
       }
 
