@@ -158,7 +158,10 @@ constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
 // ends in buffer 0: the hybrid mode runs 4 passes (digits 4..7) up to HYBRID5_MIN elements and 5
 // passes (digits 3..7) above it, where the cells of the top 31 bits are coarser than the sample
 // pitch of a dense frame; an odd number of passes starts in buffer 1.
-constexpr uint32_t HYBRID5_MIN = 1u << 19;
+#ifndef SPLATS_HYBRID5_LOG
+#define SPLATS_HYBRID5_LOG 19
+#endif
+constexpr uint32_t HYBRID5_MIN = 1u << SPLATS_HYBRID5_LOG;
 __host__ __device__ __forceinline__ int hybrid_first_digit(uint32_t n) { return n > HYBRID5_MIN ? 3 : 4; }
 __host__ __device__ __forceinline__ int sort_input_buffer(int mode, uint32_t n) {
   return (mode == SORT_HYBRID && (hybrid_first_digit(n) & 1)) ? 1 : 0;

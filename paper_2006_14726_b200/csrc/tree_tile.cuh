@@ -353,6 +353,13 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
       l = finish(l);
     }
   }
+  // the last block to get here finishes the global pyramid at its end.  Only this thread's store of the tile's
+  // top pyramid entry (phase 2) has to be visible to it, so only this thread fences, long after that store
+  // (a fence by every thread at the end of the kernel waited for all of the block's stores: 10 % of the kernel)
+  if (tid == 0 && nblocks > 1) {
+    __threadfence();
+    s.last = atomicAdd(&st->pyr_done, 1u) == (uint32_t)nblocks - 1u;
+  }
   __syncthreads();
 
   // ---- every split of the tile, dense: a complete node (both children arrived) is written out as its
@@ -440,13 +447,8 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
     for (int w = 0; w < TT_WARPS; ++w) m = min(m, s.wmin[w]);
     tile_min[blockIdx.x] = (uint8_t)m;
   }
-  if (nblocks == 1) return;
-
-  // ---- the last block to finish builds the pyramid levels above TT_LOG
-  __threadfence();
-  if (tid == 0) s.last = atomicAdd(&st->pyr_done, 1u) == (uint32_t)nblocks - 1u;
-  __syncthreads();
-  if (!s.last) return;
+  // ---- the last block builds the pyramid levels above TT_LOG
+  if (nblocks == 1 || !s.last) return;
   __threadfence();
   pyramid_top(pyr, (uint32_t)nblocks, TT_LOG);
 }
