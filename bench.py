@@ -188,18 +188,20 @@ def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
     """Compulsory DRAM traffic per launch for the layout in DESIGN.md sec. 5 (bytes)."""
     passes = 5 if N > (1 << 19) else 4
     return {
-        "bounds": 4 * P + 4 * (P // 2048 + 1),
-        "unproject_morton_compact": 4 * P + 12 * N,
+        # depth read once; the splat (centre + radius) of every valid pixel and the tile counts written
+        "bounds": 4 * P + 16 * N + 4 * (P // 2048 + 1),
+        # depth and tile counts read again, the stored splat read for the Morton code, (key, id) written
+        "unproject_morton_compact": 4 * P + 16 * N + 12 * N,
         # hybrid onesweep (default): 4 (5 above 2^19 splats) passes over the top code bits x (read 12 N + write 12 N)
         # + the neighbour check reading the keys once (8 N); the all-8-pass fallback is not counted
         "sort": passes * 24 * N + 8 * N,
-        # tiled tree: ids 4 + keys 8 + gather (depth 4, colour 16) read; sphere 16 + rgba 16 + ids 4 + node records 64
-        # + pyramid levels >= 3 (32 / 7 per leaf) written
-        "tree_1": (4 + 8 + 4 + 16) * N + (16 + 16 + 4 + 64) * N + 32 * N // 7,
+        # tiled tree: ids 4 + keys 8 + gather (stored splat 16, colour 16) read; sphere 16 + rgba 16 + ids 4 +
+        # 32-byte traversal records + pyramid levels >= 3 (32 / 7 per leaf) written
+        "tree_1": (4 + 8 + 16 + 16) * N + (16 + 16 + 4 + 32) * N + 32 * N // 7,
         # spine: the few nodes that span tiles (about 2.5 % of N at 1024 leaves per tile): queue entry 16, four keys
-        # 32, ~12 pyramid entries 384, record 64 -- per queued node
-        "tree_2": int(0.025 * N) * (16 + 32 + 384 + 64),
-        "render": 16 * P2 + (64 + 16 + 16 + 4) * N,  # image written once + BVH/splats read once
+        # 32, ~12 pyramid entries 384, record 32 -- per queued node
+        "tree_2": int(0.025 * N) * (16 + 32 + 384 + 32),
+        "render": 16 * P2 + (32 + 16 + 16 + 4) * N,  # image written once + records/splats read once
     }
 
 
