@@ -55,6 +55,9 @@ struct SortArgs {
   int pass;          // SORT_SINGLE: the digit; input buffer = pass & 1
 };
 
+#ifndef SPLATS_RANK_BALLOT
+#define SPLATS_RANK_BALLOT 1
+#endif
 #ifndef SPLATS_SORT_MAX_ITEMS
 #define SPLATS_SORT_MAX_ITEMS 16
 #endif
@@ -152,7 +155,18 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
     for (int j = 0; j < ITEMS; ++j) {
       const bool valid = (wbase + j * 32) < n;
       const uint32_t dig = (uint32_t)(key[j] >> shift) & 0xff;
+#if SPLATS_RANK_BALLOT
+      // lanes with the same digit, from eight ballots: fixed latency and pipelined, where MATCH.ANY takes
+      // time in proportion to the number of distinct digits in the warp (about 30 of 32 here)
+      unsigned peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+      for (int b = 0; b < 8; ++b) {
+        const unsigned bal = __ballot_sync(0xffffffffu, (dig >> b) & 1u);
+        peers &= ((dig >> b) & 1u) ? bal : ~bal;
+      }
+#else
       const unsigned peers = __match_any_sync(0xffffffffu, valid ? dig : 0x100u);
+#endif
       const uint32_t before = __popc(peers & ((1u << lane) - 1));
       uint32_t base = 0;
       if (valid) base = s.warp_hist[warp][dig];

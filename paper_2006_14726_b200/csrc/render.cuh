@@ -24,6 +24,9 @@ constexpr int RENDER_THREADS = 32;   // one warp = one 8x4 tile per block: the f
 constexpr int KBUF = SPLATS_KBUF;
 constexpr int SSTACK = 12;  // deeper entries live in local memory; 12 leaves more of the SM's 256 KB to L1 than 16 (1 % per step)
 constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
+#ifndef SPLATS_PREFETCH
+#define SPLATS_PREFETCH 0
+#endif
 #ifndef SPLATS_POSTPONE
 #define SPLATS_POSTPONE 0
 #endif
@@ -283,6 +286,13 @@ render_kernel(RenderParams prm) {
         // ---- internal nodes: both child boxes come with the node (one 32-byte load)
         while ((int)node >= 0) {
           const u8x rec = ldg_u8(prm.qnodes + node);
+#if SPLATS_PREFETCH
+          // both child records are known before the slab arithmetic: start fetching them into L1
+          if ((int)rec.v[6] >= 0) asm volatile("prefetch.global.L1 [%0];" :: "l"(prm.qnodes + rec.v[6]));
+#if SPLATS_PREFETCH > 1
+          if ((int)rec.v[7] >= 0) asm volatile("prefetch.global.L1 [%0];" :: "l"(prm.qnodes + rec.v[7]));
+#endif
+#endif
           STAT_ADD(0, 1);
           STAT_MAX(5, sp);
 #define QPLANE(w, sel) __uint_as_float(__byte_perm((w), 0x4B000000u, (sel)))
