@@ -310,18 +310,26 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
 template <int ITEMS>
 __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, int num_tiles, int low) {
   constexpr int TILE = SORT_THREADS * ITEMS;
+  const int lane = threadIdx.x & 31;
   for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
     const uint32_t tile_base = (uint32_t)tile * TILE;
-#pragma unroll 4
+    // all keys of the thread first (ITEMS loads in flight); a lane's right neighbour is the next lane's key
+    uint64_t k[ITEMS], kx[ITEMS];
+#pragma unroll
     for (int j = 0; j < ITEMS; ++j) {
       const uint32_t idx = tile_base + j * SORT_THREADS + threadIdx.x;
-      if (idx >= n) continue;
-      const uint64_t k = __ldcg(key + idx);
-      const uint64_t kn = idx + 1 < n ? __ldcg(key + idx + 1) : ~k;
-      if ((k >> low) != (kn >> low)) continue;                     // common case: no run continues here
-      if (idx > 0 && (__ldcg(key + idx - 1) >> low) == (k >> low)) continue;  // not the head
+      k[j] = idx < n ? __ldcg(key + idx) : 0ull;
+      kx[j] = (lane == 31 && idx + 1 < n) ? __ldcg(key + idx + 1) : 0ull;
+    }
+#pragma unroll
+    for (int j = 0; j < ITEMS; ++j) {
+      const uint32_t idx = tile_base + j * SORT_THREADS + threadIdx.x;
+      const uint64_t kd = __shfl_down_sync(0xffffffffu, k[j], 1);
+      const uint64_t kn = lane == 31 ? kx[j] : kd;
+      if (idx + 1 >= n || (k[j] >> low) != (kn >> low)) continue;   // common case: no run continues here
+      if (idx > 0 && (__ldcg(key + idx - 1) >> low) == (k[j] >> low)) continue;  // not the head
       uint32_t len = 2;
-      while (len <= RUN_MAX && idx + len < n && (__ldcg(key + idx + len) >> low) == (k >> low)) ++len;
+      while (len <= RUN_MAX && idx + len < n && (__ldcg(key + idx + len) >> low) == (k[j] >> low)) ++len;
       if (len > RUN_MAX) {
         st->sort_fallback = 1u;
         continue;
