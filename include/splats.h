@@ -231,8 +231,8 @@ int splats_count(unsigned* n_host);
  *   children    (N-1)*2 int32; node ids: internal j -> j, leaf at sorted position i -> N-1+i
  *   parents     (2N-1) int32, indexed by node id; -1 for the root
  *   node_aabbs  (2N-1)*6 float32: lo xyz, hi xyz per node id -- the EXACT boxes (oracle step O7).
- *               The traversal reads 16-bit quantised boxes (splats_export_qnodes); the default
- *               (tiled) build computes the exact ones on the way but stores them only while
+ *               The traversal reads 16-bit quantised boxes (splats_export_qnodes) and the default
+ *               (tiled) build forms nothing else; the exact boxes exist only while
  *               SPLATS_OPT_EXACT_NODES is on: without it node_aabbs != NULL fails with ESTATE.
  * Internal nodes use Karras' numbering (root 0; an internal child covering sorted range
  * [a,g] is node g when it is a left child, node a when it is a right child). */
@@ -280,9 +280,10 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *       redo the sort with all 8 passes.
  *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
  *     SPLATS_SORT_LSD8_LAUNCHES: one launch per pass.
- *   SPLATS_OPT_EXACT_NODES (default 0): the tiled build also stores the exact float32 child boxes
- *     (64 bytes per node) beside the quantised traversal records, for splats_export /
- *     splats_export_child_boxes.  The other two refit modes always store them.
+ *   SPLATS_OPT_EXACT_NODES (default 0): after the tiled build, which carries quantised boxes only, the
+ *     update also runs the pyramid refit (Karras' per-node searches, exact float32 unions) to store the
+ *     exact child boxes (64 bytes per node) for splats_export / splats_export_child_boxes; the
+ *     traversal records are untouched.  The other two refit modes always store them.
  *   SPLATS_OPT_PDL (default 1): launch the kernels of splats_update / splats_render as
  *     programmatic dependent launches (each kernel waits on its predecessor at its first
  *     instruction; only the launch latency overlaps).  0 = ordinary stream launches.

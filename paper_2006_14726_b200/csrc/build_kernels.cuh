@@ -226,13 +226,21 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
     if (tid == 6) st_next->sort_fallback = 0u;
     if (tid == 7) st_next->spine_n = 0u;
     if (tid == 8) st_next->rmax = 0u;
+    if (tid == 9) st_next->tile_done = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
   }
   if (blockIdx.x == 0 && tid == 32) {   // bounds and largest radius are final: the frame of the quantised node boxes
     const QFrame q = derive_qframe(st);
+    const float rmax = ord2f(st->rmax);
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { st->qf[a] = q.lo[a]; st->qf[3 + a] = q.s[a]; st->qf[6 + a] = q.c[a]; }
+    for (int a = 0; a < 3; ++a) {
+      st->qf[a] = q.lo[a]; st->qf[3 + a] = q.s[a]; st->qf[6 + a] = q.c[a];
+      // the frame is also the scene box the renders cull against (the tiled build carries quantised boxes only;
+      // the pyramid / atomic refit modes overwrite it with the exact root box)
+      st->root_lo[a] = q.lo[a];
+      st->root_hi[a] = add_(ord2f(st->hi[a]), rmax);
+    }
   }
 #pragma unroll
   for (int d = 0; d < 8; ++d) s_hist[d][tid] = 0u;

@@ -147,7 +147,8 @@ struct FrameState {
   uint32_t sort_fallback;  // set when the hybrid sort has to redo all 8 passes (init 0)
   uint32_t spine_n;        // nodes queued by tree_tile_kernel for tree_spine_kernel (init 0)
   uint32_t rmax;           // ordered-uint max of the valid splats' radii (init 0): with lo / hi the frame of the quantised node boxes
-  uint32_t pad_[2];
+  uint32_t tile_done;      // blocks of tree_tile_kernel that have taken their pyramid ticket (init 0)
+  uint32_t pad_;
   float qf[12];            // QFrame (lo, s, c; below) derived once per frame by unproject_kernel from lo / hi / rmax
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
@@ -251,6 +252,56 @@ __device__ __forceinline__ void store_qnode(QNode* dst, const float* L, const fl
     w[a] = quant_planes(L[a], L[3 + a], q.lo[a], q.s[a]);
     w[3 + a] = quant_planes(R[a], R[3 + a], q.lo[a], q.s[a]);
   }
+  w[6] = (uint32_t)left;
+  w[7] = (uint32_t)right;
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               :: "l"(dst), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]) : "memory");
+}
+// A box as six 16-bit codes in three words, arranged so that the union is three packed unsigned minima:
+//   w0 = q_lo(x) | q_lo(y) << 16,  w1 = q_lo(z) | (65535 - q_hi(x)) << 16,  w2 = (65535 - q_hi(y)) | (65535 - q_hi(z)) << 16.
+// Quantisation (floor for lower, ceil for upper planes of a monotone float32 expression) is monotone, so
+// min / max commute with it: the tiled build carries boxes in this form from the leaves upwards and its
+// records equal the quantised exact boxes bit for bit.
+struct QBox {
+  uint32_t w[3];
+  __device__ __forceinline__ void init() { w[0] = w[1] = w[2] = 0xffffffffu; }
+  __device__ __forceinline__ void merge(const QBox& o) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) w[i] = __vminu2(w[i], o.w[i]);
+  }
+  __device__ __forceinline__ QBox shfl_down(int delta) const {
+    QBox o;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) o.w[i] = __shfl_down_sync(0xffffffffu, w[i], delta);
+    return o;
+  }
+  __device__ __forceinline__ QBox shfl_xor(int mask) const {
+    QBox o;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) o.w[i] = __shfl_xor_sync(0xffffffffu, w[i], mask);
+    return o;
+  }
+};
+__device__ __forceinline__ QBox quant_sphere(const float4 sp, const QFrame& q) {   // box of a splat: centre -+ radius (S2), quantised (S13)
+  const uint32_t x = quant_planes(sub_(sp.x, sp.w), add_(sp.x, sp.w), q.lo[0], q.s[0]);
+  const uint32_t y = quant_planes(sub_(sp.y, sp.w), add_(sp.y, sp.w), q.lo[1], q.s[1]);
+  const uint32_t z = quant_planes(sub_(sp.z, sp.w), add_(sp.z, sp.w), q.lo[2], q.s[2]);
+  QBox b;
+  b.w[0] = __byte_perm(x, y, 0x5410);            // lo x | lo y << 16
+  b.w[1] = __byte_perm(z, ~x, 0x7610);           // lo z | ~hi x << 16
+  b.w[2] = __byte_perm(~y, ~z, 0x7632);          // ~hi y | ~hi z << 16
+  return b;
+}
+// record words of one child: axis a -> q_lo | q_hi << 16
+__device__ __forceinline__ void qbox_words(const QBox& b, uint32_t out[3]) {
+  out[0] = __byte_perm(b.w[0], ~b.w[1], 0x7610);   // lo x | hi x << 16
+  out[1] = __byte_perm(b.w[0], ~b.w[2], 0x5432);   // lo y | hi y << 16
+  out[2] = __byte_perm(b.w[1], ~b.w[2], 0x7610);   // lo z | hi z << 16
+}
+__device__ __forceinline__ void store_qnode(QNode* dst, const QBox& L, const QBox& R, int left, int right) {
+  uint32_t w[8];
+  qbox_words(L, w);
+  qbox_words(R, w + 3);
   w[6] = (uint32_t)left;
   w[7] = (uint32_t)right;
   asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"

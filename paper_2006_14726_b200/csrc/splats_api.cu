@@ -335,16 +335,25 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     // then the few nodes that span tiles (lbvh.cuh)
     const int tgrid = P > 0 ? (int)((P + TT_LEAVES - 1) / TT_LEAVES) : 1;
     launch(pdl, tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
-           gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr, bs.qnodes, c->exact_nodes ? bs.nodes : (Node*)nullptr, c->ranges, c->tile_min,
-           c->tile_fb);
-    bs.has_exact = c->exact_nodes;
+           gather, st, bs.sphere, bs.rgba, bs.ids, reinterpret_cast<uint4*>(c->pyr), bs.qnodes, c->ranges, c->tile_min, c->tile_fb);
     if (prof) m[4] = c->mark();
     int nt_log = 0;
     while ((1 << nt_log) < tgrid) ++nt_log;
     const int sgrid2 = std::min(c->num_sms * 8, (tgrid * TT_QMAX + 7) / 8);   // persistent, one warp per queued node; idle blocks exit at once
     launch(pdl, tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
-           (const float4*)bs.sphere, (const float4*)c->pyr, bs.qnodes, c->exact_nodes ? bs.nodes : (Node*)nullptr, (const uint8_t*)c->tile_min,
-           (const uint16_t*)c->tile_fb, nt_log);
+           (const float4*)bs.sphere, (const uint4*)c->pyr, bs.qnodes, (const uint8_t*)c->tile_min, (const uint16_t*)c->tile_fb, nt_log);
+    bs.has_exact = false;
+    if (c->exact_nodes) {
+      // SPLATS_OPT_EXACT_NODES: the tiled build carries quantised boxes only, so the exact float32 records (parity
+      // tests, splats_export) come from the pyramid refit run after it on the same sorted keys: Karras' per-node
+      // searches and exact range unions.  It rewrites sphere / rgba / ids with the same values and leaves qnodes alone.
+      const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
+      leaf_pyramid_kernel<Gather><<<pgrid, PYR_THREADS, 0, s>>>(c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);
+      hierarchy_kernel<<<lgrid, LBVH_THREADS, 0, s>>>((const uint64_t*)c->key[0], (const FrameState*)st, c->ranges, 1);
+      boxes_kernel<<<lgrid, LBVH_THREADS, 0, s>>>((const int4*)c->ranges, (const float4*)bs.sphere, (const float4*)c->pyr, st, bs.nodes);
+      c->launches += 3;
+      bs.has_exact = true;
+    }
   } else {
     const int pgrid = P > 0 ? (int)((P + PYR_LEAVES - 1) / PYR_LEAVES) : 1;
     launch(pdl, leaf_pyramid_kernel<Gather>, pgrid, PYR_THREADS, 0, s, c->val[0], gather, st, bs.sphere, bs.rgba, bs.ids, c->pyr);

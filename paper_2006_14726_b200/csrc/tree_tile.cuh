@@ -11,13 +11,19 @@
 // at p otherwise, and in Karras' numbering the node over (p, q] is `q` in the first case and
 // `p + 1` in the second.
 //
+// Boxes are carried as QBox (common.cuh): six 16-bit codes in three words whose union is three packed
+// minima.  Quantisation is monotone, so the union of quantised boxes is the quantised exact union:
+// the records equal quantise(exact child boxes) (S13 of DESIGN.md) bit for bit, and no float box is
+// ever formed after the leaves.  (The exact float32 records of SPLATS_OPT_EXACT_NODES come from the
+// pyramid refit, lbvh.cuh, run after this one.)
+//
 // tree_tile_kernel: one block per TT_LEAVES consecutive sorted leaves.  It gathers the splats into
 // sorted order, writes the levels >= PYR_BASE of the global box pyramid (registers + shuffles),
 // and builds every subtree that lies inside the tile bottom-up in shared memory: a finished
 // subtree stores its box and the far end of its range in its parent's slot and sets its arrival
 // bit; the second arrival appends the parent to a work list; one round per tree level, each round
-// dense over the work list (no lane waits for a long node).  A node whose children both arrived
-// is written out as a finished 64-byte record.  The nodes with a missing child -- their range
+// dense over the work list (no lane waits for a long node).  After the rounds every node whose
+// children both arrived is written out as its 32-byte record.  The nodes with a missing child -- their range
 // crosses a tile edge; they are strict prefix / suffix minima of the tile's deltas, <= 2 x 97 per
 // tile -- are queued with what is known about them.  The block also writes, for every threshold
 // v, the position of the first / last split of the tile with d < v.
@@ -49,15 +55,15 @@ constexpr int PYR_BASE = 3;     // lowest level of the global pyramid that the t
 static_assert(TT_LOG >= 7 && TT_LOG <= 12, "tile of 128 .. 4096 leaves");
 
 struct TileSmem {
-  float cbox[2][6][TT_LEAVES];   // [side][component][split]: child boxes of the node that splits at l.
-                                 // cbox[0] doubles as the staging of the leaf boxes before round 0.
+  uint32_t cbox[2][3][TT_LEAVES];   // [side][word][split]: child boxes (QBox: six 16-bit codes) of the node that splits at l.
+                                    // cbox[0] doubles as the staging of the leaf boxes before round 0.
   int16_t cend[2][TT_LEAVES];    // far end of each child's range: tile-local p (left child) or q (right child)
   uint32_t arrived[TT_LEAVES / 4];   // one byte per split: bit 0 left child stored, bit 1 right child stored
   uint16_t wl[TT_LEAVES];        // finished nodes in completion order (each node enters once)
   uint8_t d[TT_LEAVES];          // delta + 1 of the pair (l, l + 1); 0 beyond the array
   uint32_t pos_first[TT_VPAD];   // first / last split of the tile with d == u
   int32_t pos_last[TT_VPAD];
-  float top[6][TT_WARPS];        // the warps' level-7 entries
+  uint32_t top[3][TT_WARPS];     // the warps' level-7 entries
   uint32_t wmin[TT_WARPS];       // the warps' smallest delta + 1
   int4 q[TT_QMAX];               // queued nodes: (split, first or -1, last or -1, delta + 1)
   uint32_t cnt[3];               // lengths of the work lists of rounds r % 3
@@ -70,45 +76,26 @@ struct TileSmem {
 // the work lists start with (4 leaves per thread, every other split finished) hit 32 different banks.
 __device__ __forceinline__ int tt_slot(int l) { return l ^ ((l >> 5) & 31); }
 
-struct Box6 {
-  float v[6];
-  __device__ __forceinline__ void init() {
-    const float INF = __int_as_float(0x7f800000);
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { v[a] = INF; v[3 + a] = -INF; }
-  }
-  __device__ __forceinline__ void merge(const Box6& o) {
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { v[a] = fminf(v[a], o.v[a]); v[3 + a] = fmaxf(v[3 + a], o.v[3 + a]); }
-  }
-  __device__ __forceinline__ Box6 shfl_down(int delta) const {
-    Box6 o;
-#pragma unroll
-    for (int a = 0; a < 6; ++a) o.v[a] = __shfl_down_sync(0xffffffffu, v[a], delta);
-    return o;
-  }
-};
-
-__device__ __forceinline__ void pyr_store(float4* pyr, int level, uint32_t index, const Box6& b) {
-  float4* e = pyr + 2 * ((size_t)c_pyr.off[level] + index);
-  __stcg(e, make_float4(b.v[0], b.v[1], b.v[2], 0.0f));
-  __stcg(e + 1, make_float4(b.v[3], b.v[4], b.v[5], 0.0f));
+// The global pyramid of the tiled mode holds QBox entries (16 bytes each, word 3 unused) in the buffer the
+// pyramid mode uses for its float boxes; same level offsets (c_pyr, in entries).
+__device__ __forceinline__ void pyr_store(uint4* pyr, int level, uint32_t index, const QBox& b) {
+  __stcg(pyr + (size_t)c_pyr.off[level] + index, make_uint4(b.w[0], b.w[1], b.w[2], 0u));
 }
 
 // Levels above `k_prev` of the global pyramid, by the last block of tree_tile_kernel to finish:
 // five levels per round trip (a warp loads 32 consecutive entries and merges them with shuffles).
-__device__ __forceinline__ void pyramid_top(float4* pyr, uint32_t cnt_prev, int k_prev) {
+__device__ __forceinline__ void pyramid_top(uint4* pyr, uint32_t cnt_prev, int k_prev) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   while (cnt_prev > 1) {
-    const float4* src = pyr + 2 * (size_t)c_pyr.off[k_prev];
+    const uint4* src = pyr + (size_t)c_pyr.off[k_prev];
     const uint32_t chunks = (cnt_prev + 31) >> 5;
     for (uint32_t c = warp; c < chunks; c += TT_WARPS) {
       const uint32_t j = c * 32 + lane;
-      Box6 b;
+      QBox b;
       b.init();
       if (j < cnt_prev) {
-        const float4 lo = __ldcg(src + 2 * (size_t)j), hi = __ldcg(src + 2 * (size_t)j + 1);
-        b.v[0] = lo.x; b.v[1] = lo.y; b.v[2] = lo.z; b.v[3] = hi.x; b.v[4] = hi.y; b.v[5] = hi.z;
+        const uint4 e = __ldcg(src + j);
+        b.w[0] = e.x; b.w[1] = e.y; b.w[2] = e.z;
       }
 #pragma unroll
       for (int s = 1; s <= 5; ++s) {
@@ -128,7 +115,7 @@ __device__ __forceinline__ void pyramid_top(float4* pyr, uint32_t cnt_prev, int 
 // Returns the parent's split if this was the second arrival (the parent is complete), -1 otherwise
 // or when the parent lies in the tile to the left.  `is_last` = Karras: the subtree's own node
 // index is its last leaf (it is a left child), else its first.
-__device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const Box6& b, bool& is_last) {
+__device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const QBox& b, bool& is_last) {
   const uint32_t dl = p < 0 ? s.dleft : s.d[p], dr = s.d[q];
   is_last = dr > dl;
   int g, side, far;
@@ -136,7 +123,7 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const Box6
   else { if (p < 0) return -1; g = p; side = 1; far = q; }
   const int gs = tt_slot(g);
 #pragma unroll
-  for (int a = 0; a < 6; ++a) s.cbox[side][a][gs] = b.v[a];
+  for (int a = 0; a < 3; ++a) s.cbox[side][a][gs] = b.w[a];
   s.cend[side][gs] = (int16_t)far;
   __threadfence_block();   // the slot is written before the arrival bit is visible
   const int sh = 8 * (g & 3);
@@ -147,11 +134,9 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const Box6
 template <class Gather>
 __global__ void __launch_bounds__(TT_THREADS)
 tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
-                 float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, float4* pyr,
-                 QNode* __restrict__ qnodes, Node* __restrict__ nodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min,
+                 float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, uint4* pyr,
+                 QNode* __restrict__ qnodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min,
                  uint16_t* __restrict__ tile_fb) {
-  // qnodes: the traversal records (always); nodes: the exact 64-byte records, null unless
-  // SPLATS_OPT_EXACT_NODES is on (parity tests, splats_export)
   pdl_wait();
   pdl_trigger();
   extern __shared__ __align__(16) unsigned char tt_smem_raw[];
@@ -161,7 +146,6 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   if ((int)blockIdx.x >= nblocks) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int base = blockIdx.x * TT_LEAVES;
-  const float INF = __int_as_float(0x7f800000);
   const QFrame qf = load_qframe(st);
 
   // ---- (1) interleaved over the tile (coalesced): deltas of the adjacent pairs (l, l + 1), + 1;
@@ -197,33 +181,30 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
     const int l = tid + j * TT_THREADS, i = base + l;
-    float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
+    QBox lb;
+    lb.init();
     if (i < n) {
       float4 sp, col;
       src.get(id[j], sp, col);
       sphere[i] = sp;
       rgba[i] = col;
       ids_out[i] = id[j];   // the BVH keeps its own copy: the sort buffers belong to the next build
-      box_of_sphere(sp, lo, hi);
+      lb = quant_sphere(sp, qf);
     }
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { s.cbox[0][a][l] = lo[a]; s.cbox[0][3 + a][l] = hi[a]; }
-  }
-  if (n == 1 && tid == 0) {   // the single leaf is the root
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { st->root_lo[a] = s.cbox[0][a][0]; st->root_hi[a] = s.cbox[0][3 + a][0]; }
+    for (int a = 0; a < 3; ++a) s.cbox[0][a][l] = lb.w[a];
   }
   __syncthreads();
 
   // ---- (2) consecutive: thread t owns the leaves 4t .. 4t+3.  Leaf boxes into registers; global
   // pyramid levels PYR_BASE .. TT_LOG by shuffles (levels 1, 2 exist only in registers).
-  Box6 leaf[4];
+  QBox leaf[4];
   {
-    float4 c[6];
+    uint4 c[3];
 #pragma unroll
-    for (int a = 0; a < 6; ++a) c[a] = *reinterpret_cast<const float4*>(&s.cbox[0][a][4 * tid]);
+    for (int a = 0; a < 3; ++a) c[a] = *reinterpret_cast<const uint4*>(&s.cbox[0][a][4 * tid]);
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { leaf[0].v[a] = c[a].x; leaf[1].v[a] = c[a].y; leaf[2].v[a] = c[a].z; leaf[3].v[a] = c[a].w; }
+    for (int a = 0; a < 3; ++a) { leaf[0].w[a] = c[a].x; leaf[1].w[a] = c[a].y; leaf[2].w[a] = c[a].z; leaf[3].w[a] = c[a].w; }
   }
   const int valid = min(TT_LEAVES, n - base);   // leaves of this tile = its splits, the last one of the array (d + 1 = 0) included
   // the tile's deltas: strict prefix / suffix minima (for the spine kernel's tables), smallest value
@@ -245,7 +226,7 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   if (lane == 0) pre_ex = 255u;
   if (lane == 31) suf_ex = 255u;
   {
-    Box6 b = leaf[0];
+    QBox b = leaf[0];
     b.merge(leaf[1]); b.merge(leaf[2]); b.merge(leaf[3]);   // level 2 entry (base >> 2) + tid
 #pragma unroll
     for (int sft = 1; sft <= 5; ++sft) {                        // levels 3 .. 7
@@ -256,16 +237,16 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
     }
     if (TT_LOG > 7 && lane == 0) {
 #pragma unroll
-      for (int a = 0; a < 6; ++a) s.top[a][warp] = b.v[a];
+      for (int a = 0; a < 3; ++a) s.top[a][warp] = b.w[a];
     }
   }
   __syncthreads();   // every thread holds its leaf boxes: cbox[0] is free for the rounds below
   if (TT_LOG > 7 && warp == 0) {                                // levels 8 .. TT_LOG from the warps' entries
-    Box6 b;
+    QBox b;
     b.init();
     if (lane < TT_WARPS) {
 #pragma unroll
-      for (int a = 0; a < 6; ++a) b.v[a] = s.top[a][lane];
+      for (int a = 0; a < 3; ++a) b.w[a] = s.top[a][lane];
     }
 #pragma unroll
     for (int sft = 1; sft <= TT_LOG - 7; ++sft) {
@@ -307,9 +288,9 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   auto finish = [&](int l) -> int {
     const int ls = tt_slot(l);
     const int p = s.cend[0][ls], q = s.cend[1][ls];
-    Box6 U, R;
+    QBox U, R;
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { U.v[a] = s.cbox[0][a][ls]; R.v[a] = s.cbox[1][a][ls]; }
+    for (int a = 0; a < 3; ++a) { U.w[a] = s.cbox[0][a][ls]; R.w[a] = s.cbox[1][a][ls]; }
     U.merge(R);
     bool il;
     return tile_report(s, p, q, U, il);
@@ -358,7 +339,7 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
   // (a fence by every thread at the end of the kernel waited for all of the block's stores: 10 % of the kernel)
   if (tid == 0 && nblocks > 1) {
     __threadfence();
-    s.last = atomicAdd(&st->pyr_done, 1u) == (uint32_t)nblocks - 1u;
+    s.last = atomicAdd(&st->tile_done, 1u) == (uint32_t)nblocks - 1u;
   }
   __syncthreads();
 
@@ -377,28 +358,16 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
       continue;
     }
     const int p = s.cend[0][ls], q = s.cend[1][ls];
-    float L[6], R[6];
+    QBox L, R;
 #pragma unroll
-    for (int a = 0; a < 6; ++a) { L[a] = s.cbox[0][a][ls]; R[a] = s.cbox[1][a][ls]; }
+    for (int a = 0; a < 3; ++a) { L.w[a] = s.cbox[0][a][ls]; R.w[a] = s.cbox[1][a][ls]; }
     const uint32_t dl = p < 0 ? s.dleft : s.d[p], dr = s.d[q];
     const int first = base + p + 1, last = base + q;
     const int idx = dr > dl ? last : first;   // Karras: a left child is numbered by its last leaf, a right child by its first
     const int cnt_l = g - first + 1, cnt_r = last - g;
     const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
     const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-    store_qnode(qnodes + idx, L, R, left, right, qf);
-    if (nodes) {
-      f8 ra, rb;
-      ra.v[0] = L[0]; ra.v[1] = L[1]; ra.v[2] = L[2]; ra.v[3] = L[3]; ra.v[4] = L[4]; ra.v[5] = L[5]; ra.v[6] = R[0]; ra.v[7] = R[1];
-      rb.v[0] = R[2]; rb.v[1] = R[3]; rb.v[2] = R[4]; rb.v[3] = R[5];
-      rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
-      stg_f8(nodes + idx, ra);
-      stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
-    }
-    if (idx == 0) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L[a], R[a]); st->root_hi[a] = fmaxf(L[3 + a], R[3 + a]); }
-    }
+    store_qnode(qnodes + idx, L, R, left, right);
   }
   __syncthreads();
   const uint32_t qn = s.qn;
@@ -503,8 +472,8 @@ struct TileMins {
 // piece 14 + j is level PYR_BASE + j of the global pyramid (at most two entries per level).  The
 // addresses depend only on l and r, so a warp issues all pieces of a node's two child boxes at once.
 constexpr int RANGE_PIECES = 14 + (PYR_MAX_LEVELS - PYR_BASE + 1);
-__device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, const float4* __restrict__ pyr, uint32_t l, uint32_t r,
-                                            int piece, BoxAcc& A) {
+__device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, const uint4* __restrict__ pyr, const QFrame& qf,
+                                            uint32_t l, uint32_t r, int piece, QBox& A) {
   const uint32_t lb = (l + (1u << PYR_BASE) - 1) >> PYR_BASE, rb = r >> PYR_BASE;
   const bool small = lb >= rb;   // no aligned block inside: < 2 x 8 leaves, all read directly
   if (piece < 14) {
@@ -512,23 +481,31 @@ __device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, c
     if (small) i = l + piece;
     else if (piece < 7) { i = l + piece; if (i >= (lb << PYR_BASE)) return; }
     else i = (rb << PYR_BASE) + (piece - 7);
-    if (i < r) A.add_sphere(__ldg(sphere + i));
+    if (i < r) A.merge(quant_sphere(__ldg(sphere + i), qf));
     return;
   }
   if (small) return;
   const int k = PYR_BASE + (piece - 14);
   const uint32_t lk = (l + (1u << k) - 1) >> k, rk = r >> k;   // the segment-tree walk's bounds when it reaches level k
   if (lk >= rk) return;
-  const float4* lev = pyr + 2 * (size_t)c_pyr.off[k];
-  if (lk & 1u) A.add(__ldg(lev + 2 * (size_t)lk), __ldg(lev + 2 * (size_t)lk + 1));
-  if (rk & 1u) A.add(__ldg(lev + 2 * (size_t)(rk - 1)), __ldg(lev + 2 * (size_t)(rk - 1) + 1));
+  const uint4* lev = pyr + (size_t)c_pyr.off[k];
+  if (lk & 1u) {
+    const uint4 e = __ldg(lev + lk);
+    QBox b; b.w[0] = e.x; b.w[1] = e.y; b.w[2] = e.z;
+    A.merge(b);
+  }
+  if (rk & 1u) {
+    const uint4 e = __ldg(lev + (rk - 1));
+    QBox b; b.w[0] = e.x; b.w[1] = e.y; b.w[2] = e.z;
+    A.merge(b);
+  }
 }
 
 // One warp per queued node; persistent blocks (the per-tile minima are staged once per block).
 constexpr int SPINE_THREADS = 256;
 __global__ void __launch_bounds__(SPINE_THREADS)
 tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4* __restrict__ queue,
-                  const float4* __restrict__ sphere, const float4* __restrict__ pyr, QNode* __restrict__ qnodes, Node* __restrict__ nodes,
+                  const float4* __restrict__ sphere, const uint4* __restrict__ pyr, QNode* __restrict__ qnodes,
                   const uint8_t* __restrict__ tile_min, const uint16_t* __restrict__ tile_fb, int nt_log) {
   pdl_wait();
   pdl_trigger();
@@ -540,8 +517,7 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
   if ((int)(blockIdx.x * WPB) >= qn) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ntiles = (n + TT_LEAVES - 1) / TT_LEAVES;
-  const int qax = (lane < 3 ? lane : lane - 3) % 3;   // lanes 0..5 write one word of the traversal record each: their axis' frame
-  const float my_qlo = __ldcg(&st->qf[qax]), my_qs = __ldcg(&st->qf[3 + qax]);
+  const QFrame qf = load_qframe(st);
   TileMins tm;
   tm.m = m;
   tm.log = nt_log;
@@ -568,54 +544,26 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
       last = (t2 << TT_LOG) + (int)__ldg(tile_fb + (size_t)t2 * (2 * TT_VPAD) + v);
     }
     // ---- both child boxes: 2 x RANGE_PIECES independent pieces spread over the lanes, then a warp reduction
-    BoxAcc L, R;
+    QBox L, R;
     L.init();
     R.init();
     for (int piece = lane; piece < 2 * RANGE_PIECES; piece += 32) {
-      if (piece < RANGE_PIECES) range_piece(sphere, pyr, (uint32_t)first, (uint32_t)g + 1u, piece, L);
-      else range_piece(sphere, pyr, (uint32_t)g + 1u, (uint32_t)last + 1u, piece - RANGE_PIECES, R);
+      if (piece < RANGE_PIECES) range_piece(sphere, pyr, qf, (uint32_t)first, (uint32_t)g + 1u, piece, L);
+      else range_piece(sphere, pyr, qf, (uint32_t)g + 1u, (uint32_t)last + 1u, piece - RANGE_PIECES, R);
     }
     const int dl = first > 0 ? delta(keys, n, first - 1, __ldg(keys + first - 1), first) : -1;
     const int dr = last < n - 1 ? delta(keys, n, last, __ldg(keys + last), last + 1) : -1;
     const int idx = dr > dl ? last : first;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        L.lo[a] = fminf(L.lo[a], __shfl_xor_sync(0xffffffffu, L.lo[a], o));
-        L.hi[a] = fmaxf(L.hi[a], __shfl_xor_sync(0xffffffffu, L.hi[a], o));
-        R.lo[a] = fminf(R.lo[a], __shfl_xor_sync(0xffffffffu, R.lo[a], o));
-        R.hi[a] = fmaxf(R.hi[a], __shfl_xor_sync(0xffffffffu, R.hi[a], o));
-      }
+      L.merge(L.shfl_xor(o));
+      R.merge(R.shfl_xor(o));
     }
-    {
+    if (lane == 0) {
       const int cnt_l = g - first + 1, cnt_r = last - g;
       const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
       const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
-      if (lane < 8) {   // one word of the traversal record per lane (every lane holds the reduced boxes): one 32-byte store
-        const int a = lane < 3 ? lane : lane - 3;
-        uint32_t w;
-        if (lane < 6) {
-          const float plo = lane < 3 ? (a == 0 ? L.lo[0] : a == 1 ? L.lo[1] : L.lo[2]) : (a == 0 ? R.lo[0] : a == 1 ? R.lo[1] : R.lo[2]);
-          const float phi = lane < 3 ? (a == 0 ? L.hi[0] : a == 1 ? L.hi[1] : L.hi[2]) : (a == 0 ? R.hi[0] : a == 1 ? R.hi[1] : R.hi[2]);
-          w = quant_planes(plo, phi, my_qlo, my_qs);
-        } else {
-          w = (uint32_t)(lane == 6 ? left : right);
-        }
-        qnodes[idx].w[lane] = w;
-      }
-      if (lane == 0 && nodes) {
-        f8 ra, rb;
-        ra.v[0] = L.lo[0]; ra.v[1] = L.lo[1]; ra.v[2] = L.lo[2]; ra.v[3] = L.hi[0]; ra.v[4] = L.hi[1]; ra.v[5] = L.hi[2]; ra.v[6] = R.lo[0]; ra.v[7] = R.lo[1];
-        rb.v[0] = R.lo[2]; rb.v[1] = R.hi[0]; rb.v[2] = R.hi[1]; rb.v[3] = R.hi[2];
-        rb.v[4] = __int_as_float(left); rb.v[5] = __int_as_float(right); rb.v[6] = 0.0f; rb.v[7] = 0.0f;
-        stg_f8(nodes + idx, ra);
-        stg_f8(reinterpret_cast<char*>(nodes + idx) + 32, rb);
-      }
-      if (lane == 0 && idx == 0) {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { st->root_lo[a] = fminf(L.lo[a], R.lo[a]); st->root_hi[a] = fmaxf(L.hi[a], R.hi[a]); }
-      }
+      store_qnode(qnodes + idx, L, R, left, right);
     }
   }
 }

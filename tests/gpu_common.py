@@ -17,9 +17,10 @@ class Session:
 
     def __init__(self, max_W, max_H, exact_nodes=True):
         sp.splats_create(max_W, max_H)
-        # the parity tests also want the exact float32 node boxes, which the default build computes but
-        # does not store (include/splats.h, SPLATS_OPT_EXACT_NODES); the traversal records are the same
-        # either way (tests/test_gpu_parity.py::test_exact_nodes_option_changes_nothing)
+        # the parity tests also want the exact float32 node boxes; the default (tiled) build carries only
+        # the quantised ones, so with this option the update runs the exact pyramid refit as well
+        # (include/splats.h, SPLATS_OPT_EXACT_NODES); the traversal records are the same either way
+        # (tests/test_gpu_parity.py::test_exact_nodes_option_changes_nothing)
         sp.splats_set_option(sp.OPT_EXACT_NODES, 1 if exact_nodes else 0)
 
     def close(self):

@@ -88,3 +88,33 @@ def test_config3_bench_step_in_bench_launch_configuration():
         for j in range(4):
             ref = oracle.render(sc, cfg.dst_cams[4 * build + j], cfg.W, cfg.H, "bvh")
             assert_rgba_close(outs[j].cpu().numpy(), ref, f"display frame {4 * build + j}")
+
+
+def test_dense_1080p_leg_of_the_bench():
+    # bench.py's `dense` leg: synth.dense_frame 1920x1080 (N = P), the library's defaults, its two cameras
+    W, H = 1920, 1080
+    color, depth, cam = synth.dense_frame(W, H, 0)
+    sc = oracle.build_scene(color, depth, cam, W, H, 1.0)
+    assert sc["N"] == W * H
+    with Session(W, H, exact_nodes=False) as s:
+        s.update(color, depth, cam, W, H, 1.0)
+        assert_bvh_bit_exact(sc, exact=False)
+        _check_renders(s, sc, [synth.orbit_camera(0.0), synth.orbit_camera(3.0)], W, H, False, 100_000, 128, 50)
+
+
+def test_table1_shape_leg_of_the_bench():
+    # bench.py's `table1_shape` leg: 1024x1024, 59.5 % of the samples valid, all-hit and
+    # first-hit queries of its three views
+    cfg = synth.table1_config()
+    color, depth = synth.source_frame(cfg, 0)
+    sc = oracle.build_scene(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+    assert abs(sc["N"] / (cfg.W * cfg.H) - 0.595) < 0.005
+    with Session(cfg.W, cfg.H) as s:
+        s.update(color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale)
+        assert_bvh_bit_exact(sc)
+        _check_renders(s, sc, cfg.dst_cams, cfg.W, cfg.H, False, 100_000, 128, 60)
+        rng = np.random.default_rng(61)
+        for cam in cfg.dst_cams:
+            px = rng.choice(cfg.W * cfg.H, size=50_000, replace=False).astype(np.int64)
+            got = s.render(cam, cfg.W, cfg.H, first_hit=True).reshape(-1, 4)[px]
+            assert np.array_equal(got, oracle.render(sc, cam, cfg.W, cfg.H, "bvh", pixels=px, first_hit=True))
