@@ -503,6 +503,10 @@ __device__ __forceinline__ void range_piece(const float4* __restrict__ sphere, c
 
 // One warp per queued node; persistent blocks (the per-tile minima are staged once per block).
 constexpr int SPINE_THREADS = 256;
+#ifndef SPLATS_SPINE_LANES
+#define SPLATS_SPINE_LANES 8
+#endif
+constexpr int SPINE_LANES = SPLATS_SPINE_LANES;   // 32, 16 or 8
 __global__ void __launch_bounds__(SPINE_THREADS)
 tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4* __restrict__ queue,
                   const float4* __restrict__ sphere, const uint4* __restrict__ pyr, QNode* __restrict__ qnodes,
@@ -514,7 +518,7 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
   const int n = (int)st->n;
   const int qn = (int)st->spine_n;
   constexpr int WPB = SPINE_THREADS / 32;
-  if ((int)(blockIdx.x * WPB) >= qn) return;
+  if ((int)(blockIdx.x * WPB * (32 / SPINE_LANES)) >= qn) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ntiles = (n + TT_LEAVES - 1) / TT_LEAVES;
   const QFrame qf = load_qframe(st);
@@ -529,37 +533,49 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
     for (int j = threadIdx.x; j < cnt; j += SPINE_THREADS) m[o1 + j] = min(m[o0 + 2 * j], m[o0 + 2 * j + 1]);
     __syncthreads();
   }
-  for (int e = blockIdx.x * WPB + warp; e < qn; e += gridDim.x * WPB) {
-    // ---- the node's range (every lane computes the same values: broadcast loads, no divergence)
-    const int4 ent = __ldg(queue + e);
+  // SPINE_LANES lanes per queued node (a warp works on 32 / SPINE_LANES nodes at once: the kernel is a chain of
+  // three dependent round trips per node, so nodes in flight are what counts)
+  constexpr int GPW = 32 / SPINE_LANES;                 // groups per warp
+  const int sub = lane / SPINE_LANES, sl = lane % SPINE_LANES;
+  const int stride = gridDim.x * WPB * GPW;
+  for (int e0 = (blockIdx.x * WPB + warp) * GPW; e0 < qn; e0 += stride) {
+    const int e = e0 + sub;
+    const bool act = e < qn;
+    // ---- the node's range (every lane of the group computes the same values: broadcast loads)
+    const int4 ent = act ? __ldg(queue + e) : make_int4(0, 0, 0, 1);
     const int g = ent.x, t = g >> TT_LOG;
     const uint32_t v = (uint32_t)ent.w;
     int first = ent.y, last = ent.z;
-    if (first < 0) {   // nearest split to the left, in an earlier tile, with a smaller delta
+    if (act && first < 0) {   // nearest split to the left, in an earlier tile, with a smaller delta
       const int t2 = tm.left(t - 1, v);
       first = t2 < 0 ? 0 : (t2 << TT_LOG) + (int)__ldg(tile_fb + (size_t)t2 * (2 * TT_VPAD) + TT_VPAD + v) + 1;
     }
-    if (last < 0) {    // the array ends with a split of delta + 1 = 0, so there always is one
+    if (act && last < 0) {    // the array ends with a split of delta + 1 = 0, so there always is one
       const int t2 = tm.right(t + 1, v);
       last = (t2 << TT_LOG) + (int)__ldg(tile_fb + (size_t)t2 * (2 * TT_VPAD) + v);
     }
-    // ---- both child boxes: 2 x RANGE_PIECES independent pieces spread over the lanes, then a warp reduction
+    // ---- both child boxes: 2 x RANGE_PIECES independent pieces spread over the group's lanes, then a reduction
     QBox L, R;
     L.init();
     R.init();
-    for (int piece = lane; piece < 2 * RANGE_PIECES; piece += 32) {
-      if (piece < RANGE_PIECES) range_piece(sphere, pyr, qf, (uint32_t)first, (uint32_t)g + 1u, piece, L);
-      else range_piece(sphere, pyr, qf, (uint32_t)g + 1u, (uint32_t)last + 1u, piece - RANGE_PIECES, R);
+    if (act) {
+      for (int piece = sl; piece < 2 * RANGE_PIECES; piece += SPINE_LANES) {
+        if (piece < RANGE_PIECES) range_piece(sphere, pyr, qf, (uint32_t)first, (uint32_t)g + 1u, piece, L);
+        else range_piece(sphere, pyr, qf, (uint32_t)g + 1u, (uint32_t)last + 1u, piece - RANGE_PIECES, R);
+      }
     }
-    const int dl = first > 0 ? delta(keys, n, first - 1, __ldg(keys + first - 1), first) : -1;
-    const int dr = last < n - 1 ? delta(keys, n, last, __ldg(keys + last), last + 1) : -1;
-    const int idx = dr > dl ? last : first;
+    int idx = 0;
+    if (act) {
+      const int dl = first > 0 ? delta(keys, n, first - 1, __ldg(keys + first - 1), first) : -1;
+      const int dr = last < n - 1 ? delta(keys, n, last, __ldg(keys + last), last + 1) : -1;
+      idx = dr > dl ? last : first;
+    }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
+    for (int o = SPINE_LANES / 2; o > 0; o >>= 1) {
       L.merge(L.shfl_xor(o));
       R.merge(R.shfl_xor(o));
     }
-    if (lane == 0) {
+    if (act && sl == 0) {
       const int cnt_l = g - first + 1, cnt_r = last - g;
       const int left = cnt_l <= LEAF_MAX ? (int)leaf_range_code((uint32_t)first, (uint32_t)cnt_l) : g;
       const int right = cnt_r <= LEAF_MAX ? (int)leaf_range_code((uint32_t)g + 1u, (uint32_t)cnt_r) : g + 1;
