@@ -196,11 +196,11 @@ def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
         # + the neighbour check reading the keys once (8 N); the all-8-pass fallback is not counted
         "sort": passes * 24 * N + 8 * N,
         # tiled tree: ids 4 + keys 8 + gather (stored splat 16, colour 16) read; sphere 16 + rgba 16 + ids 4 +
-        # 32-byte traversal records + pyramid levels >= 3 (32 / 7 per leaf) written
-        "tree_1": (4 + 8 + 16 + 16) * N + (16 + 16 + 4 + 32) * N + 32 * N // 7,
+        # 32-byte traversal records + quantised pyramid levels >= 3 (16 / 7 per leaf) written
+        "tree_1": (4 + 8 + 16 + 16) * N + (16 + 16 + 4 + 32) * N + 16 * N // 7,
         # spine: the few nodes that span tiles (about 2.5 % of N at 1024 leaves per tile): queue entry 16, four keys
-        # 32, ~12 pyramid entries 384, record 32 -- per queued node
-        "tree_2": int(0.025 * N) * (16 + 32 + 384 + 32),
+        # 32, ~12 pyramid entries 192, record 32 -- per queued node
+        "tree_2": int(0.025 * N) * (16 + 32 + 192 + 32),
         "render": 16 * P2 + (32 + 16 + 16 + 4) * N,  # image written once + records/splats read once
     }
 

@@ -24,6 +24,9 @@ constexpr int RENDER_THREADS = 32;   // one warp = one 8x4 tile per block: the f
 constexpr int KBUF = SPLATS_KBUF;
 constexpr int SSTACK = 12;  // deeper entries live in local memory; 12 leaves more of the SM's 256 KB to L1 than 16 (1 % per step)
 constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
+#ifndef SPLATS_TICKET_AHEAD
+#define SPLATS_TICKET_AHEAD 0
+#endif
 #ifndef SPLATS_PREFETCH
 #define SPLATS_PREFETCH 0
 #endif
@@ -207,7 +210,14 @@ render_kernel(RenderParams prm) {
   const int nwarps = gridDim.x * (RENDER_THREADS / 32);
   if (blockIdx.x == 0 && tid == 0) atomicAdd(prm.traced, (unsigned long long)ntiles * 32ull);
   int tile = blockIdx.x * (RENDER_THREADS / 32) + warp;
+#if SPLATS_TICKET_AHEAD
+  // the ticket for the next tile is taken before this one is traced: the atomic's round trip hides behind the traversal
+  unsigned nxt = 0;
+  for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, nxt, 0)) {
+  if (lane == 0) nxt = atomicAdd(prm.sched, 1u);
+#else
   for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, lane == 0 ? atomicAdd(prm.sched, 1u) : 0u, 0)) {
+#endif
   if (tile >= ntiles) {
     const int px0 = rx0 * 8, px1 = rx1 * 8, py0 = ry0 * 4, py1 = ry1 * 4;
     const int base = (tile - ntiles) * FILL_PX;
