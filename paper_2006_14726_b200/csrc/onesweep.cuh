@@ -161,8 +161,14 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
       unsigned peers = __ballot_sync(0xffffffffu, valid);
 #pragma unroll
       for (int b = 0; b < 8; ++b) {
-        const unsigned bal = __ballot_sync(0xffffffffu, (dig >> b) & 1u);
-        peers &= ((dig >> b) & 1u) ? bal : ~bal;
+        // bit test into a predicate, ballot, then one of two predicated ANDs (the compiler's own version builds
+        // a select mask per bit: 7 instructions instead of a ballot and two predicated ANDs)
+        asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
+            "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
+            "vote.sync.ballot.b32 t, p, 0xffffffff;\n\t"
+            "@p and.b32 %0, %0, t;\n\t"
+            "@!p lop3.b32 %0, %0, t, 0, 0x30;\n\t}"   // peers & ~t
+            : "+r"(peers) : "r"(dig), "r"(1u << b));
       }
 #else
       const unsigned peers = __match_any_sync(0xffffffffu, valid ? dig : 0x100u);
