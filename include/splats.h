@@ -274,10 +274,14 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *     SPLATS_REFIT_ATOMIC: one thread per leaf climbs the tree; the second arrival at a node's
  *       atomic counter forms the union and continues (the classic LBVH refit).
  *   SPLATS_OPT_SORT: how step a3 (order by (code, id)) is computed.
- *     SPLATS_SORT_HYBRID (default): one launch; 4 onesweep passes over the top 31 code bits,
- *       then a check that no two neighbours share them (true for one-sample-per-pixel frames);
- *       short runs are fixed up by a stable insertion sort, longer ones make the same launch
- *       redo the sort with all 8 passes.
+ *     SPLATS_SORT_HYBRID (default): one launch; 2 onesweep passes over the top 15 code bits (3 over the
+ *       top 23 above 2^19 splats), after which the array is a sequence of small buckets; every bucket is
+ *       then ordered by the next two digits in shared memory, window by window, and keys that still tie
+ *       there (none for one-sample-per-pixel frames) by the full code.  A bucket larger than a window
+ *       makes the launch fall back to the passes of SPLATS_SORT_HYBRID_LSD.
+ *     SPLATS_SORT_HYBRID_LSD: one launch; 4 onesweep passes over the top 31 code bits (5 over the top 39
+ *       above 2^19 splats), then a check that no two neighbours share them; short runs are fixed up by a
+ *       stable insertion sort, longer ones make the same launch redo the sort with all 8 passes.
  *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
  *     SPLATS_SORT_LSD8_LAUNCHES: one launch per pass.
  *   SPLATS_OPT_EXACT_NODES (default 0): after the tiled build, which carries quantised boxes only, the
@@ -314,6 +318,7 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
 #define SPLATS_SORT_HYBRID         0
 #define SPLATS_SORT_LSD8           1
 #define SPLATS_SORT_LSD8_LAUNCHES  2
+#define SPLATS_SORT_HYBRID_LSD     3
 int splats_set_option(int option, int value);
 
 /* How splats_update derives the radius of a splat (takes effect at the next update; SURVEY.md

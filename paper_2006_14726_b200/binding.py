@@ -18,7 +18,7 @@ from . import build as _build
 NUM_STAGES = 9
 STAGE_NAMES = ("bounds", "unproject_morton_compact", "sort", "tree_1", "tree_2", "render", "pack", "points", "march")
 OPT_REFIT, REFIT_PYRAMID, REFIT_ATOMIC, REFIT_TILED = 0, 0, 1, 2
-OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES = 1, 0, 1, 2
+OPT_SORT, SORT_HYBRID, SORT_LSD8, SORT_LSD8_LAUNCHES, SORT_HYBRID_LSD = 1, 0, 1, 2, 3
 RADIUS_FOOTPRINT, RADIUS_CONSTANT, RADIUS_OPACITY = 0, 1, 2
 OPT_PDL = 2
 OPT_OVERLAP = 3

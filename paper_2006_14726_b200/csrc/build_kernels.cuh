@@ -227,6 +227,7 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
     if (tid == 7) st_next->spine_n = 0u;
     if (tid == 8) st_next->rmax = 0u;
     if (tid == 9) st_next->tile_done = 0u;
+    if (tid == 10) st_next->sort_wfall = 0u;
 #pragma unroll
     for (int d = 0; d < 8; ++d) st_next->hist[d][tid] = 0u;
   }
@@ -248,7 +249,7 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
   // the sort ping-pongs between two buffers and must end in buffer 0 (onesweep.cuh)
   const uint32_t n_all = st->n;
   const bool odd = sort_input_buffer(sort_mode, n_all) != 0;
-  const int first_digit = sort_mode == SORT_HYBRID ? hybrid_first_digit(n_all) : 0;
+  const int first_digit = sort_is_hybrid(sort_mode) ? hybrid_first_digit(n_all) : 0;
   uint64_t* __restrict__ keys = odd ? keys1 : keys0;
   uint32_t* __restrict__ ids = odd ? ids1 : ids0;
   float lo[3], ext[3];

@@ -148,13 +148,14 @@ struct FrameState {
   uint32_t spine_n;        // nodes queued by tree_tile_kernel for tree_spine_kernel (init 0)
   uint32_t rmax;           // ordered-uint max of the valid splats' radii (init 0): with lo / hi the frame of the quantised node boxes
   uint32_t tile_done;      // blocks of tree_tile_kernel that have taken their pyramid ticket (init 0)
-  uint32_t pad_;
+  uint32_t sort_wfall;     // set when a window of the windowed hybrid sort does not fit: fall back to the LSD passes (init 0)
   float qf[12];            // QFrame (lo, s, c; below) derived once per frame by unproject_kernel from lo / hi / rmax
   uint32_t hist[8][256];  // digit histograms of the 8 radix passes (init 0)
 };
 
 // ---- sort modes (onesweep.cuh) and what the producer of the keys must know about them
-constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
+constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2, SORT_HYBRID_LSD = 3;
+__host__ __device__ __forceinline__ bool sort_is_hybrid(int mode) { return mode == SORT_HYBRID || mode == SORT_HYBRID_LSD; }
 // Which buffer unproject_kernel writes the unsorted pairs to, so that the sorted result always
 // ends in buffer 0: the hybrid mode runs 4 passes (digits 4..7) up to HYBRID5_MIN elements and 5
 // passes (digits 3..7) above it, where the cells of the top 31 bits are coarser than the sample
@@ -165,7 +166,8 @@ constexpr int SORT_HYBRID = 0, SORT_LSD8 = 1, SORT_SINGLE = 2;
 constexpr uint32_t HYBRID5_MIN = 1u << SPLATS_HYBRID5_LOG;
 __host__ __device__ __forceinline__ int hybrid_first_digit(uint32_t n) { return n > HYBRID5_MIN ? 3 : 4; }
 __host__ __device__ __forceinline__ int sort_input_buffer(int mode, uint32_t n) {
-  return (mode == SORT_HYBRID && (hybrid_first_digit(n) & 1)) ? 1 : 0;
+  if (mode == SORT_HYBRID) return 1;   // three global passes, then the buckets in place in buffer 0
+  return (mode == SORT_HYBRID_LSD && (hybrid_first_digit(n) & 1)) ? 1 : 0;
 }
 
 // 64-byte BVH node: both child boxes live in the parent, so one node fetch (four 16-byte

@@ -50,7 +50,7 @@ struct SortArgs {
   uint32_t* val[2];
   FrameState* st;
   uint64_t* status;
-  uint32_t epoch0;   // this launch may use epochs epoch0 .. epoch0 + 11
+  uint32_t epoch0;   // this launch may use epochs epoch0 .. epoch0 + 31
   int mode;
   int pass;          // SORT_SINGLE: the digit; input buffer = pass & 1
 };
@@ -68,9 +68,13 @@ struct SortSmem {
   int64_t bin_base[RADIX];                // global position of local slot 0 of each digit
   uint32_t digit_base[RADIX];             // exclusive scan of the global histogram
   uint32_t scan_tmp[SORT_WARPS];
-  uint64_t stage[SORT_THREADS * SORT_MAX_ITEMS];   // keys in tile-sorted order
+  uint64_t stage[SORT_THREADS * SORT_MAX_ITEMS];   // keys in tile-sorted order; window buffer A of the windowed sort
   uint32_t vstage[SORT_THREADS * SORT_MAX_ITEMS];  // values in tile-sorted order
+  uint64_t stage2[SORT_THREADS * SORT_MAX_ITEMS];  // window buffer B
+  uint32_t vstage2[SORT_THREADS * SORT_MAX_ITEMS];
+  int win[2];                                       // bounds of the current window
 };
+constexpr int WIN_MAX = SORT_THREADS * SORT_MAX_ITEMS;   // capacity of a window (4096 elements)
 
 // exclusive scan of one value per thread over the 256-thread block
 __device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* tmp /*[8]*/, uint32_t* total) {
@@ -107,6 +111,36 @@ __device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t nb, uint32_
     __threadfence();
   }
   __syncthreads();
+}
+
+// Stable rank of one key per lane among the keys of the same digit that this warp has seen so far in the
+// tile / window (warp_hist[warp] holds the running counts).
+__device__ __forceinline__ uint32_t warp_rank(SortSmem& s, uint32_t dig, bool valid, int lane, int warp) {
+#if SPLATS_RANK_BALLOT
+  // lanes with the same digit, from eight ballots: fixed latency and pipelined, where MATCH.ANY takes
+  // time in proportion to the number of distinct digits in the warp (about 30 of 32 here)
+  unsigned peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    // bit test into a predicate, ballot, then one of two predicated ANDs (the compiler's own version builds
+    // a select mask per bit: 7 instructions instead of a ballot and two predicated ANDs)
+    asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
+        "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
+        "vote.sync.ballot.b32 t, p, 0xffffffff;\n\t"
+        "@p and.b32 %0, %0, t;\n\t"
+        "@!p lop3.b32 %0, %0, t, 0, 0x30;\n\t}"   // peers & ~t
+        : "+r"(peers) : "r"(dig), "r"(1u << b));
+  }
+#else
+  const unsigned peers = __match_any_sync(0xffffffffu, valid ? dig : 0x100u);
+#endif
+  const uint32_t before = __popc(peers & ((1u << lane) - 1));
+  uint32_t base = 0;
+  if (valid) base = s.warp_hist[warp][dig];
+  __syncwarp();
+  if (valid && before == 0) s.warp_hist[warp][dig] = base + __popc(peers);
+  __syncwarp();
+  return base + before;
 }
 
 // One 8-bit pass over all tiles of this block: in -> out.
@@ -152,35 +186,8 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
     // ---- rank inside the warp, digit by digit, in index order (stable)
     uint32_t rank[ITEMS];
 #pragma unroll
-    for (int j = 0; j < ITEMS; ++j) {
-      const bool valid = (wbase + j * 32) < n;
-      const uint32_t dig = (uint32_t)(key[j] >> shift) & 0xff;
-#if SPLATS_RANK_BALLOT
-      // lanes with the same digit, from eight ballots: fixed latency and pipelined, where MATCH.ANY takes
-      // time in proportion to the number of distinct digits in the warp (about 30 of 32 here)
-      unsigned peers = __ballot_sync(0xffffffffu, valid);
-#pragma unroll
-      for (int b = 0; b < 8; ++b) {
-        // bit test into a predicate, ballot, then one of two predicated ANDs (the compiler's own version builds
-        // a select mask per bit: 7 instructions instead of a ballot and two predicated ANDs)
-        asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
-            "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
-            "vote.sync.ballot.b32 t, p, 0xffffffff;\n\t"
-            "@p and.b32 %0, %0, t;\n\t"
-            "@!p lop3.b32 %0, %0, t, 0, 0x30;\n\t}"   // peers & ~t
-            : "+r"(peers) : "r"(dig), "r"(1u << b));
-      }
-#else
-      const unsigned peers = __match_any_sync(0xffffffffu, valid ? dig : 0x100u);
-#endif
-      const uint32_t before = __popc(peers & ((1u << lane) - 1));
-      uint32_t base = 0;
-      if (valid) base = s.warp_hist[warp][dig];
-      __syncwarp();
-      if (valid && before == 0) s.warp_hist[warp][dig] = base + __popc(peers);
-      __syncwarp();
-      rank[j] = base + before;
-    }
+    for (int j = 0; j < ITEMS; ++j)
+      rank[j] = warp_rank(s, (uint32_t)(key[j] >> shift) & 0xff, (wbase + j * 32) < n, lane, warp);
     __syncthreads();
 
     // ---- bin `tid`: exclusive prefix over the warps, tile count
@@ -360,53 +367,159 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
   }
 }
 
+// ---- windowed hybrid sort (SORT_HYBRID, the default): after three global passes over the top digits the
+// array is a sequence of buckets of equal top 23 code bits (cells of 1/256 x 1/256 x 1/128 of the scene box: a
+// few to a few hundred samples of a one-sample-per-pixel frame), in order; what is left is to put every bucket
+// in order by (code, position): local work.  The array is cut into windows at bucket boundaries (window k =
+// [B(k T), B((k + 1) T)), B(x) = first bucket start >= x); a block loads a window into shared memory, every
+// thread takes an element and counts the keys of its bucket that come before it (stable, by the full code: no
+// fix-up afterwards), which is its place, and the window is written back in place.  No status words, no look-back, no grid barrier.  A bucket that does not fit (> WIN_BUCKET_MAX keys, or
+// a window > WIN_MAX) raises st->sort_wfall and the launch falls back to LSD passes.
+constexpr int WIN_G = 3;                 // global passes (digits 5, 6, 7)
+constexpr int WIN_BSHIFT = 8 * (8 - WIN_G);
+constexpr int WIN_BUCKET_MAX = 512;      // counting is quadratic in the bucket size
+static_assert(WIN_MAX <= (1 << (64 - 40)) && WIN_BSHIFT == 40, "comparison key = 40 code bits + position");
+
+constexpr int WIN_EXTRA = 512;           // a window is loaded with this many elements beyond its nominal end
+
+__device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_t* val, FrameState* st, uint32_t n) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t* heads = s.tile_off;   // one bit per loaded element: a bucket starts here (128 words)
+  // nominal window size: what the capacity allows, a quarter of it for small frames (more windows than blocks)
+  const uint32_t T = n > (uint32_t)gridDim.x * (WIN_MAX / 4) ? WIN_MAX - WIN_EXTRA : WIN_MAX / 4;
+  const uint32_t nwin = (n + T - 1) / T;
+  for (uint32_t k = blockIdx.x; k < nwin; k += gridDim.x) {
+    // ---- load [k T, (k + 1) T + WIN_EXTRA) in one go; the window proper, [B(k T), B((k + 1) T)), is found in it
+    const uint32_t g0 = k * T, gend = min(n, g0 + T + WIN_EXTRA), cnt = gend - g0;
+    for (uint32_t i = tid; i < cnt; i += SORT_THREADS) {
+      s.stage[i] = __ldcg(key + g0 + i);
+      s.vstage[i] = __ldcg(val + g0 + i);
+    }
+    const uint64_t kprev = g0 > 0 ? __ldcg(key + g0 - 1) : ~0ull;   // (code bits >= WIN_BSHIFT of ~0 match no real key: bit 63)
+    __syncthreads();
+    // bucket heads as a bit map (chunk c = elements 32 c .. 32 c + 31 of the loaded range)
+    const uint32_t nchunk = (cnt + 31) >> 5;
+    for (uint32_t c = warp; c < nchunk; c += SORT_WARPS) {
+      const uint32_t i = c * 32 + lane;
+      const bool head = i < cnt && ((i == 0 ? kprev : s.stage[i - 1]) >> WIN_BSHIFT) != (s.stage[i] >> WIN_BSHIFT);
+      const unsigned m = __ballot_sync(0xffffffffu, head);
+      if (lane == 0) heads[c] = m;
+      // comparison key inside a bucket: the 40 code bits below the bucket's, then the position (unique: no ties)
+      if (i < cnt) s.stage2[i] = (s.stage[i] << (64 - WIN_BSHIFT)) | i;
+    }
+    __syncthreads();
+    // first head >= x in the loaded range, cnt if none
+    auto first_head = [&](uint32_t x) -> uint32_t {
+      uint32_t c = x >> 5;
+      if (c >= nchunk) return cnt;
+      uint32_t w = heads[c] & (0xffffffffu << (x & 31));
+      while (!w) {
+        if (++c >= nchunk) return cnt;
+        w = heads[c];
+      }
+      return c * 32 + (uint32_t)__ffs(w) - 1u;
+    };
+    const uint32_t w0 = first_head(0);                                        // B(k T) - g0
+    const uint32_t w1 = g0 + T >= n ? cnt : first_head(T);                    // B((k + 1) T) - g0
+    if ((w0 == cnt && g0 + cnt < n) || (w1 == cnt && g0 + cnt < n)) {         // no boundary within WIN_EXTRA: a bucket too large
+      if (tid == 0) st->sort_wfall = 1u;
+      __syncthreads();
+      continue;
+    }
+    // one thread per element of the window: its bucket [p, q) from the bit map, its place = p + the number of keys
+    // of the bucket that come before it (smaller code, or the same code and an earlier position: stable)
+    for (uint32_t i = w0 + tid; i < w1; i += SORT_THREADS) {
+      int c = (int)(i >> 5);
+      uint32_t w = heads[c] & (0xffffffffu >> (31 - (i & 31)));   // heads at or before i in its chunk
+      while (!w) w = heads[--c];                                     // w0 is a head
+      const uint32_t p = (uint32_t)c * 32 + 31u - (uint32_t)__clz(w);
+      const uint32_t q = min(first_head(i + 1), w1);
+      if (q - p > WIN_BUCKET_MAX) {   // counting is quadratic: leave the bucket as it is and fall back
+        st->sort_wfall = 1u;
+        continue;
+      }
+      const uint64_t ti = s.stage2[i];
+      uint32_t rank = 0;
+#pragma unroll 4
+      for (uint32_t j = p; j < q; ++j) rank += s.stage2[j] < ti ? 1u : 0u;
+      __stcg(key + g0 + p + rank, s.stage[i]);   // everything is read from shared memory: writing in place is safe
+      __stcg(val + g0 + p + rank, s.vstage[i]);
+    }
+    __syncthreads();
+  }
+}
+
+// digit histograms that unproject_kernel did not count (digits lo .. hi - 1), from the keys in `key`
+__device__ __forceinline__ void count_digits(SortSmem& s, const uint64_t* key, FrameState* st, uint32_t n, uint32_t nb, int lo, int hi) {
+  const int tid = threadIdx.x;
+  if (lo >= hi) return;
+  for (int d = lo; d < hi; ++d) s.warp_hist[d][tid] = 0;
+  __syncthreads();
+  for (uint32_t idx = blockIdx.x * SORT_THREADS + tid; idx < n; idx += nb * SORT_THREADS) {
+    const uint64_t k = __ldcg(key + idx);
+    for (int d = lo; d < hi; ++d) atomicAdd(&s.warp_hist[d][(uint32_t)(k >> (8 * d)) & 0xff], 1u);
+  }
+  __syncthreads();
+  for (int d = lo; d < hi; ++d) {
+    const uint32_t h = s.warp_hist[d][tid];
+    if (h) atomicAdd(&st->hist[d][tid], h);
+  }
+}
+
 template <int ITEMS>
 __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_t n) {
   constexpr int TILE = SORT_THREADS * ITEMS;
   const int num_tiles = (int)((n + TILE - 1) / TILE);
   const uint32_t nb = min((uint32_t)gridDim.x, (uint32_t)num_tiles);  // blocks that own a tile
-  if (blockIdx.x >= nb) return;
   uint32_t* bar = &a.st->sort_bar;
   uint32_t round = 0, epoch = a.epoch0;
   if (a.mode == SORT_SINGLE) {
+    if (blockIdx.x >= nb) return;
     const int in = a.pass & 1;
     onesweep_pass<ITEMS>(s, a.key[in], a.val[in], a.key[in ^ 1], a.val[in ^ 1], a.st, a.pass, a.status, epoch, n, num_tiles);
     return;
   }
-  int first = a.mode == SORT_HYBRID ? hybrid_first_digit(n) : 0;
+  // LSD passes over the digits from .. 7, buffer `buf` -> ... ; a grid barrier after every pass
+  auto lsd = [&](int from, int& buf) {
+    for (int pass = from; pass < 8; ++pass) {
+      if (blockIdx.x < nb)
+        onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch, n, num_tiles);
+      ++epoch;
+      buf ^= 1;
+      grid_barrier(bar, gridDim.x, round);
+    }
+  };
+  int first = sort_is_hybrid(a.mode) ? hybrid_first_digit(n) : 0;
   int buf = sort_input_buffer(a.mode, n);
-  for (int pass = first;;) {
-    onesweep_pass<ITEMS>(s, a.key[buf], a.val[buf], a.key[buf ^ 1], a.val[buf ^ 1], a.st, pass, a.status, epoch++, n, num_tiles);
-    buf ^= 1;
-    if (++pass < 8) {
-      grid_barrier(bar, nb, round);
-      continue;
-    }
-    if (first == 0) break;  // all 8 digits sorted
-    grid_barrier(bar, nb, round);
-    fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
-    grid_barrier(bar, nb, round);
-    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) break;
-    // a long run of equal top bits: redo the sort with all 8 passes.  unproject_kernel counted only
-    // the digits >= first, so count the low ones here (a histogram does not depend on the order).
-    {
-      const int tid = threadIdx.x;
-      for (int d = 0; d < first; ++d) s.warp_hist[d][tid] = 0;
-      __syncthreads();
-      for (uint32_t idx = blockIdx.x * SORT_THREADS + tid; idx < n; idx += nb * SORT_THREADS) {
-        const uint64_t k = __ldcg(a.key[0] + idx);
-        for (int d = 0; d < first; ++d) atomicAdd(&s.warp_hist[d][(uint32_t)(k >> (8 * d)) & 0xff], 1u);
-      }
-      __syncthreads();
-      for (int d = 0; d < first; ++d) {
-        const uint32_t h = s.warp_hist[d][tid];
-        if (h) atomicAdd(&a.st->hist[d][tid], h);
-      }
-      grid_barrier(bar, nb, round);
-    }
-    first = 0;
-    pass = 0;
+  if (a.mode == SORT_HYBRID) {
+    // ---- three global passes over the top digits, then bucket by bucket in shared memory
+    lsd(8 - WIN_G, buf);                 // ends in buffer 0 (an odd number of passes from buffer 1)
+    window_phase(s, a.key[0], a.val[0], a.st, n);
+    grid_barrier(bar, gridDim.x, round);
+    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_wfall) == 0u) return;
+    // a bucket did not fit: LSD passes over the digits d0 .. 7 from where the array is now (every step so far
+    // was a stable permutation; d0 is even so that the result ends in buffer 0), then the global fix-up
+    const int d0 = first & ~1;
+    count_digits(s, a.key[0], a.st, n, gridDim.x, d0, first);
+    grid_barrier(bar, gridDim.x, round);
+    lsd(d0, buf);
+    if (blockIdx.x < nb) fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
+    grid_barrier(bar, gridDim.x, round);
+    first = d0;
+    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) return;
+  } else {
+    lsd(first, buf);
+    if (first == 0) return;  // all 8 digits sorted
+    if (blockIdx.x < nb) fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
+    grid_barrier(bar, gridDim.x, round);
+    if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_fallback) == 0u) return;
   }
+  // a long run of equal sorted bits: redo the sort with all 8 passes.  unproject_kernel counted only the digits
+  // >= first, so count the low ones here (a histogram does not depend on the order).
+  count_digits(s, a.key[0], a.st, n, gridDim.x, 0, first);
+  grid_barrier(bar, gridDim.x, round);
+  buf = 0;
+  lsd(0, buf);
 }
 
 // The tile size follows N (known on the device only).  One wave (every tile has a resident block):

@@ -22,12 +22,17 @@
 #include "render.cuh"
 #include "tree_tile.cuh"
 
+#ifndef SPLATS_PDL_MASK
+#define SPLATS_PDL_MASK 35
+#endif
+
 namespace {
 
 using namespace sw;
 
 constexpr int SORT_MIN_TILE = SORT_THREADS * 4;  // smallest tile of onesweep_kernel
-static_assert(SPLATS_SORT_HYBRID == SORT_HYBRID && SPLATS_SORT_LSD8 == SORT_LSD8 && SPLATS_SORT_LSD8_LAUNCHES == SORT_SINGLE,
+static_assert(SPLATS_SORT_HYBRID == SORT_HYBRID && SPLATS_SORT_LSD8 == SORT_LSD8 && SPLATS_SORT_LSD8_LAUNCHES == SORT_SINGLE &&
+              SPLATS_SORT_HYBRID_LSD == SORT_HYBRID_LSD,
               "public sort modes must match onesweep.cuh");
 
 struct Context {
@@ -281,16 +286,22 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   size_t m[6] = {0, 0, 0, 0, 0, 0};
   if (prof) m[0] = c->mark();
   const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
+  // Which kernels are launched as programmatic dependents (SPLATS_OPT_PDL): bounds (1), unproject (2), sort (4),
+  // tile (8), spine (16), the first render after an update (32).  A dependent's blocks become resident early and
+  // spin in griddepcontrol.wait: behind a short predecessor that hides the launch latency; behind a long one (sort,
+  // tile kernel) the waiting blocks cost more than the 3 us they save (measured: dense update 0.315 -> 0.302 ms,
+  // config 3 10.59 k -> 10.87 k frames/s with 35 instead of 63).
+  constexpr int pdl_mask = SPLATS_PDL_MASK;
   if (!async) c->render_streak = 0;   // (a decoupled build runs on its own stream: the renders in flight stay tracked)
   // bounds_kernel waits for its predecessor at its first instruction; overlapping renders
   // complete in launch order (render.cuh), so everything before it in the stream is complete
   // after a render launched by this library (and nothing else since) the bounds kernel may start under its tail
   const int bounds_wait = (pdl && c->overlap && !async && c->last_was_render) ? 0 : 1;
   c->last_was_render = false;
-  launch(pdl, bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count, bounds_wait);
+  launch(pdl && (pdl_mask & 1), bounds_kernel<Src>, tiles, BUILD_THREADS, 0, s, src, P, st, c->tile_count, bounds_wait);
   if (prof) m[1] = c->mark();
   const int grid2 = tiles < c->num_sms * 8 ? tiles : c->num_sms * 8;
-  launch(pdl, unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
+  launch(pdl && (pdl_mask & 2), unproject_kernel<Src>, grid2, BUILD_THREADS, 0, s, src, P, tiles, st, st_next, c->tile_count, c->key[0],
          c->val[0], c->key[1], c->val[1], c->sort_mode);
   if (prof) m[2] = c->mark();
   const int max_sort_tiles = P > 0 ? (int)((P + SORT_MIN_TILE - 1) / SORT_MIN_TILE) : 1;
@@ -316,8 +327,8 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   } else {
     sa.pass = 0;
     sa.epoch0 = c->epoch + 1;
-    c->epoch += 16;
-    launch(pdl, onesweep_kernel, sgrid, SORT_THREADS, c->sort_smem, s, sa);
+    c->epoch += 32;
+    launch(pdl && (pdl_mask & 4), onesweep_kernel, sgrid, SORT_THREADS, c->sort_smem, s, sa);
   }
   if (prof) m[3] = c->mark();
   const int lgrid_max = P > 0 ? (int)((P + LBVH_THREADS - 1) / LBVH_THREADS) : 1;
@@ -334,13 +345,13 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
     // gather + leaf boxes + pyramid + every node whose range lies inside one tile of sorted leaves;
     // then the few nodes that span tiles (lbvh.cuh)
     const int tgrid = P > 0 ? (int)((P + TT_LEAVES - 1) / TT_LEAVES) : 1;
-    launch(pdl, tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
+    launch(pdl && (pdl_mask & 8), tree_tile_kernel<Gather>, tgrid, TT_THREADS, sizeof(TileSmem), s, (const uint64_t*)c->key[0], (const uint32_t*)c->val[0],
            gather, st, bs.sphere, bs.rgba, bs.ids, reinterpret_cast<uint4*>(c->pyr), bs.qnodes, c->ranges, c->tile_min, c->tile_fb);
     if (prof) m[4] = c->mark();
     int nt_log = 0;
     while ((1 << nt_log) < tgrid) ++nt_log;
     const int sgrid2 = std::min(c->num_sms * 8, (tgrid * TT_QMAX + 7) / 8);   // persistent, one warp per queued node; idle blocks exit at once
-    launch(pdl, tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
+    launch(pdl && (pdl_mask & 16), tree_spine_kernel, sgrid2, SPINE_THREADS, (size_t)2 << nt_log, s, (const uint64_t*)c->key[0], st, (const int4*)c->ranges,
            (const float4*)bs.sphere, (const uint4*)c->pyr, bs.qnodes, (const uint8_t*)c->tile_min, (const uint16_t*)c->tile_fb, nt_log);
     bs.has_exact = false;
     if (c->exact_nodes) {
@@ -448,9 +459,11 @@ int do_render(Context* c, const wr_camera* cam, int W2, int H2, float* out, bool
   c->inflight_lo[c->render_streak] = out_lo;
   c->inflight_hi[c->render_streak] = out_hi;
   c->render_streak = (pdl && c->overlap) ? c->render_streak + 1 : 0;
-  if (rgba8) launch(pdl, render_kernel<KBUF, false, true>, grid, RENDER_THREADS, 0, c->stream, prm);
-  else if (first_hit) launch(pdl, render_kernel<1, true, false>, grid, RENDER_THREADS, 0, c->stream, prm);
-  else launch(pdl, render_kernel<KBUF, false, false>, grid, RENDER_THREADS, 0, c->stream, prm);
+  constexpr int pdl_mask = SPLATS_PDL_MASK;
+  const bool attr = pdl && (wait_prev == 0 || (pdl_mask & 32));
+  if (rgba8) launch(attr, render_kernel<KBUF, false, true>, grid, RENDER_THREADS, 0, c->stream, prm);
+  else if (first_hit) launch(attr, render_kernel<1, true, false>, grid, RENDER_THREADS, 0, c->stream, prm);
+  else launch(attr, render_kernel<KBUF, false, false>, grid, RENDER_THREADS, 0, c->stream, prm);
   if (c->profiling) c->spans.push_back({5, m0, c->mark()});
   c->last_was_render = pdl;
   c->launches += 1;
@@ -970,7 +983,7 @@ int splats_set_option(int option, int value) {
       g_ctx->refit_mode = value;
       return SPLATS_OK;
     case SPLATS_OPT_SORT:
-      if (value != SPLATS_SORT_HYBRID && value != SPLATS_SORT_LSD8 && value != SPLATS_SORT_LSD8_LAUNCHES)
+      if (value != SPLATS_SORT_HYBRID && value != SPLATS_SORT_LSD8 && value != SPLATS_SORT_LSD8_LAUNCHES && value != SPLATS_SORT_HYBRID_LSD)
         return fail(SPLATS_EINVAL, "unknown sort mode");
       g_ctx->sort_mode = value;
       return SPLATS_OK;

@@ -201,6 +201,9 @@ def test_hybrid_sort_fixup_and_fallback(outlier, kind):
     depth[depth > 0] = 3.0
     depth[0, 0] = outlier
     with Session(W, H) as s:
+        sp.splats_set_option(sp.OPT_SORT, sp.SORT_HYBRID_LSD)    # the LSD variant of the hybrid sort first ...
+        check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(4.0)], mode="bvh")
+        sp.splats_set_option(sp.OPT_SORT, sp.SORT_HYBRID)        # ... then the windowed one (default)
         sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(4.0)], mode="bvh")
         L = _top_runs(sc["sorted_codes"])
         if kind == "short":
@@ -212,17 +215,35 @@ def test_hybrid_sort_fixup_and_fallback(outlier, kind):
         check_scene(s, c2, d2, cam2, 100, 37, 1.0, [synth.orbit_camera(4.0)], [(64, 64)], mode="bvh")
 
 
-@pytest.mark.parametrize("mode", ["lsd8", "lsd8_launches"])
+@pytest.mark.parametrize("mode", ["lsd8", "lsd8_launches", "hybrid_lsd"])
 def test_sort_modes_give_the_same_order(mode):
     cfg = synth.make_config(1)
     color, depth = synth.source_frame(cfg, 0)
     with Session(cfg.W, cfg.H) as s:
-        sp.splats_set_option(sp.OPT_SORT, sp.SORT_LSD8 if mode == "lsd8" else sp.SORT_LSD8_LAUNCHES)
+        sp.splats_set_option(sp.OPT_SORT, {"lsd8": sp.SORT_LSD8, "lsd8_launches": sp.SORT_LSD8_LAUNCHES,
+                                           "hybrid_lsd": sp.SORT_HYBRID_LSD}[mode])
         check_scene(s, color, depth, cfg.src_cams[0], cfg.W, cfg.H, cfg.r_scale, cfg.dst_cams[:1], mode="bvh")
         c2, d2, cam2 = synth.random_frame(127, 65, seed=3, fill=0.4)
         check_scene(s, c2, d2, cam2, 127, 65, 2.0, [synth.orbit_camera(5.0)], mode="bvh")
         with pytest.raises(sp.SplatsError):
             sp.splats_set_option(sp.OPT_SORT, 9)
+
+
+@pytest.mark.parametrize("W,H", [(128, 80), (200, 150)])
+def test_windowed_sort_bucket_overflow_falls_back(W, H):
+    # all splats but one at one depth and an outlier far away: the top code bits agree for (almost) all of
+    # them, so one bucket of the windowed hybrid sort is larger than a window (4096): the launch must fall
+    # back to the LSD passes (and, the runs being long, to all eight) and give the same order
+    color, depth, cam = synth.random_frame(W, H, seed=33, fill=0.9)
+    depth[depth > 0] = 3.0
+    depth[0, 0] = 9000.0
+    with Session(W, H) as s:
+        sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(4.0)], mode="bvh", sample=2000)
+        assert sc["N"] > 8192
+        # and a well-behaved frame right after it: flags are re-armed
+        cfg = synth.make_config(0)
+        c2, d2 = synth.source_frame(cfg, 0)
+        check_scene(s, c2, d2, cfg.src_cams[0], cfg.W, cfg.H, 1.0, cfg.dst_cams[:1], mode="bvh")
 
 
 def test_dense_frame_five_pass_hybrid_sort_and_all_tile_sizes():
@@ -231,6 +252,9 @@ def test_dense_frame_five_pass_hybrid_sort_and_all_tile_sizes():
     W, H = 2304, 1000
     color, depth, cam = synth.dense_frame(W, H, seed=5)
     with Session(W, H) as s:
+        sp.splats_set_option(sp.OPT_SORT, sp.SORT_HYBRID_LSD)
+        check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(2.0)], mode="bvh", sample=1024)
+        sp.splats_set_option(sp.OPT_SORT, sp.SORT_HYBRID)
         sc, _ = check_scene(s, color, depth, cam, W, H, 1.0, [synth.orbit_camera(2.0)], mode="bvh", sample=4096)
         assert sc["N"] == W * H > (1 << 20)
         for (w, h) in ((1500, 800), (1400, 700), (900, 500), (640, 360)):
@@ -425,7 +449,7 @@ def test_seeded_fuzz_whole_path(seed):
     dst = synth.orbit_camera(float(rng.uniform(-30, 30)), float(rng.uniform(-15, 15)), float(rng.uniform(2.0, 5.0)))
     with Session(max(W, 200), max(H, 150)) as s:
         sp.splats_set_option(sp.OPT_OVERLAP, seed % 2)
-        sp.splats_set_option(sp.OPT_SORT, [sp.SORT_HYBRID, sp.SORT_HYBRID, sp.SORT_LSD8][seed % 3])
+        sp.splats_set_option(sp.OPT_SORT, [sp.SORT_HYBRID, sp.SORT_HYBRID_LSD, sp.SORT_LSD8][seed % 3])
         sc, _ = check_scene(s, color, depth, cam, W, H, r_scale, [dst, cam], [(W2, H2), (W2, H2)], mode="bvh", radius=radius)
         fh = s.render(dst, W2, H2, first_hit=True)
         assert np.array_equal(fh, oracle.render(sc, dst, W2, H2, "bvh", first_hit=True))
