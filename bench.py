@@ -186,15 +186,14 @@ def make_workload(config_index: int, n_groups: int | None):
 
 def algorithmic_bytes(P: int, N: int, P2: int) -> dict:
     """Compulsory DRAM traffic per launch for the layout in DESIGN.md sec. 5 (bytes)."""
-    passes = 5 if N > (1 << 19) else 4
     return {
         # depth read once; the splat (centre + radius) of every valid pixel and the tile counts written
         "bounds": 4 * P + 16 * N + 4 * (P // 2048 + 1),
         # depth and tile counts read again, the stored splat read for the Morton code, (key, id) written
         "unproject_morton_compact": 4 * P + 16 * N + 12 * N,
-        # hybrid onesweep (default): 4 (5 above 2^19 splats) passes over the top code bits x (read 12 N + write 12 N)
-        # + the neighbour check reading the keys once (8 N); the all-8-pass fallback is not counted
-        "sort": passes * 24 * N + 8 * N,
+        # windowed hybrid sort (default): 3 onesweep passes over the top 23 code bits x (read 12 N + write 12 N) + the
+        # window phase reading and writing every pair once more; the LSD fallback is not counted
+        "sort": 3 * 24 * N + 24 * N,
         # tiled tree: ids 4 + keys 8 + gather (stored splat 16, colour 16) read; sphere 16 + rgba 16 + ids 4 +
         # 32-byte traversal records + quantised pyramid levels >= 3 (16 / 7 per leaf) written
         "tree_1": (4 + 8 + 16 + 16) * N + (16 + 16 + 4 + 32) * N + 16 * N // 7,
