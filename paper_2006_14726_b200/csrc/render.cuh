@@ -22,8 +22,11 @@ constexpr int RENDER_THREADS = 32;   // one warp = one 8x4 tile per block: the f
 #define SPLATS_KBUF 4
 #endif
 constexpr int KBUF = SPLATS_KBUF;
-constexpr int SSTACK = 12;  // deeper entries live in local memory; 12 leaves more of the SM's 256 KB to L1 than 16 (1 % per step)
-constexpr int LSTACK = 84;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
+#ifndef SPLATS_SSTACK
+#define SPLATS_SSTACK 8
+#endif
+constexpr int SSTACK = SPLATS_SSTACK;  // deeper entries live in local memory; 8 leaves more of the SM's 256 KB to L1 (4 .. 16 measured: within 1 %)
+constexpr int LSTACK = 96 - SSTACK;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
 #ifndef SPLATS_TICKET_AHEAD
 #define SPLATS_TICKET_AHEAD 0
 #endif
