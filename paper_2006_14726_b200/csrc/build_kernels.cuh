@@ -299,7 +299,9 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
         if (v) {
           float p[3];
           src.key_centre(t[k], base + 32 * k, p);
-          code = morton63(p, lo, ext);
+          // the sort key is the 63-bit code shifted up by one: all 64 bits carry information, the top digit has eight
+          // significant bits instead of seven (one more bit per pass of the hybrid sorts; splats_export shifts back)
+          code = morton63(p, lo, ext) << 1;
           const uint32_t at = pos + __popc(act & ((1u << lane) - 1));
           keys[at] = code;
           ids[at] = (uint32_t)(base + 32 * k);

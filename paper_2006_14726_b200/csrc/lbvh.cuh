@@ -446,6 +446,13 @@ quantise_nodes_kernel(const Node* __restrict__ nodes, const FrameState* __restri
   }
 }
 
+// The sorted keys are kept as code << 1 (build_kernels.cuh): give the codes back.
+__global__ void __launch_bounds__(LBVH_THREADS)
+export_keys_kernel(const uint64_t* __restrict__ keys, const FrameState* __restrict__ st, uint64_t* __restrict__ out) {
+  const int n = (int)st->n;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) out[i] = keys[i] >> 1;
+}
+
 // Parent links are not part of the traversal structure: they are derived here from the
 // child links (parents[] must be pre-filled with -1 by the caller; the root keeps it).
 // Topology comes from the traversal records; the exact boxes from the 64-byte records, which

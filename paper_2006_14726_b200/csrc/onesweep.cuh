@@ -368,7 +368,7 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
 }
 
 // ---- windowed hybrid sort (SORT_HYBRID, the default): after three global passes over the top digits the
-// array is a sequence of buckets of equal top 23 code bits (cells of 1/256 x 1/256 x 1/128 of the scene box: a
+// array is a sequence of buckets of equal top 24 code bits (cells of 1/256 x 1/256 x 1/256 of the scene box: a
 // few to a few hundred samples of a one-sample-per-pixel frame), in order; what is left is to put every bucket
 // in order by (code, position): local work.  The array is cut into windows at bucket boundaries (window k =
 // [B(k T), B((k + 1) T)), B(x) = first bucket start >= x); a block loads a window into shared memory, every
@@ -404,7 +404,7 @@ __device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_
       const bool head = i < cnt && ((i == 0 ? kprev : s.stage[i - 1]) >> WIN_BSHIFT) != (s.stage[i] >> WIN_BSHIFT);
       const unsigned m = __ballot_sync(0xffffffffu, head);
       if (lane == 0) heads[c] = m;
-      // comparison key inside a bucket: the 40 code bits below the bucket's, then the position (unique: no ties)
+      // comparison key inside a bucket: the 39 code bits below the bucket's, then the position (unique: no ties)
       if (i < cnt) s.stage2[i] = (s.stage[i] << (64 - WIN_BSHIFT)) | i;
     }
     __syncthreads();

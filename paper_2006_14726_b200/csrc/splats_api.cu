@@ -888,7 +888,11 @@ int splats_export(unsigned long long* keys, unsigned* perm, int* children, int* 
   int rc = splats_count(&n);
   if (rc) return rc;
   if (n == 0) return SPLATS_OK;
-  if (keys) CU(cudaMemcpyAsync(keys, c->key[0], (size_t)n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream));
+  if (keys) {
+    export_keys_kernel<<<(int)((n + LBVH_THREADS - 1) / LBVH_THREADS), LBVH_THREADS, 0, c->stream>>>(
+        (const uint64_t*)c->key[0], (const FrameState*)(c->state + c->cur_state), reinterpret_cast<uint64_t*>(keys));
+    c->launches += 1;
+  }
   if (perm) CU(cudaMemcpyAsync(perm, c->set[c->cur_set].ids, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream));
   if (node_aabbs && !c->set[c->cur_set].has_exact)
     return fail(SPLATS_ESTATE, "splats_export: the exact node boxes were not stored by the last build (set SPLATS_OPT_EXACT_NODES before the update)");

@@ -186,14 +186,14 @@ def test_atomic_refit_mode_gives_the_same_tree():
 
 
 def _top_runs(codes):
-    hi = codes >> np.uint64(32)
+    hi = codes >> np.uint64(31)   # the top 32 code bits: what four passes of the LSD hybrid sort put in order
     brk = np.flatnonzero(np.r_[True, hi[1:] != hi[:-1], True])
     return np.diff(brk)
 
 
 @pytest.mark.parametrize("outlier,kind", [(300.0, "short"), (600.0, "short"), (2000.0, "long"), (5000.0, "long")])
 def test_hybrid_sort_fixup_and_fallback(outlier, kind):
-    # The hybrid sort orders by the top 31 code bits and repairs runs that share them: an outlier
+    # The LSD hybrid sort orders by the top 32 code bits and repairs runs that share them: an outlier
     # stretches the bounds until several splats fall into one cell of the top bits.  Short runs
     # (<= 32) are fixed in place, longer ones trigger the full 8-pass sort; same result either way.
     W, H = 64, 64
