@@ -169,14 +169,15 @@ bounds_kernel(const Src src, int64_t P, FrameState* __restrict__ st, uint32_t* _
 }
 
 // ------------------------------------------------------------------------------------ a2
-__device__ __forceinline__ uint64_t spread21(uint32_t v) {  // bit i -> bit 3i
-  uint64_t x = v & 0x1fffffu;
-  x = (x | (x << 32)) & 0x001f00000000ffffull;
-  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
-  x = (x | (x << 8)) & 0x100f00f00f00f00full;
-  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
-  x = (x | (x << 2)) & 0x1249249249249249ull;
+__device__ __forceinline__ uint32_t spread11(uint32_t x) {  // bit i -> bit 3i, 11 bits (32-bit operations)
+  x = (x | (x << 16)) & 0x070000ffu;
+  x = (x | (x << 8)) & 0x0700f00fu;
+  x = (x | (x << 4)) & 0x430c30c3u;
+  x = (x | (x << 2)) & 0x49249249u;
   return x;
+}
+__device__ __forceinline__ uint64_t spread21(uint32_t v) {  // bit i -> bit 3i: low 11 bits and high 10 bits on their own
+  return (uint64_t)spread11(v & 0x7ffu) | ((uint64_t)spread11((v >> 11) & 0x3ffu) << 33);
 }
 
 // 63-bit Morton code of centre p inside [lo, hi] (LBVH, PAPER.md:71 [LGS*09]); 21 bit per
@@ -249,7 +250,8 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
   // the sort ping-pongs between two buffers and must end in buffer 0 (onesweep.cuh)
   const uint32_t n_all = st->n;
   const bool odd = sort_input_buffer(sort_mode, n_all) != 0;
-  const int first_digit = sort_is_hybrid(sort_mode) ? hybrid_first_digit(n_all) : 0;
+  // lowest digit whose histogram the sort launch reads from here (it counts any others itself, on its fallback paths)
+  const int first_digit = sort_mode == SORT_HYBRID ? 8 - 3 : sort_mode == SORT_HYBRID_LSD ? hybrid_first_digit(n_all) : 0;
   uint64_t* __restrict__ keys = odd ? keys1 : keys0;
   uint32_t* __restrict__ ids = odd ? ids1 : ids0;
   float lo[3], ext[3];
@@ -306,17 +308,32 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
           keys[at] = code;
           ids[at] = (uint32_t)(base + 32 * k);
         }
-        // digit histograms: neighbouring pixels mostly share a digit, so each run of equal digits among
-        // consecutive valid lanes is counted by its first lane (one shared-memory atomic per run)
-        for (int d = first_digit; d < 8; ++d) {
-          const uint32_t dig = v ? (uint32_t)(code >> (8 * d)) & 0xff : 0x100u;
-          const uint32_t prev = __shfl_up_sync(0xffffffffu, dig, 1);
-          const bool head = v && (lane == 0 || prev != dig);
+        // digit histograms: neighbouring pixels mostly share their top digits, so each run of equal digits among
+        // consecutive valid lanes is counted by its first lane (one shared-memory atomic per run and digit)
+        if (first_digit == 5) {
+          // the windowed sort reads the digits 5 .. 7 only: runs of equal top 24 key bits, found once for all three
+          const uint32_t top = v ? (uint32_t)(code >> 40) : 0xffffffffu;
+          const uint32_t prev = __shfl_up_sync(0xffffffffu, top, 1);
+          const bool head = v && (lane == 0 || prev != top);
           const unsigned brk = __ballot_sync(0xffffffffu, head || !v);   // where runs start or are interrupted
           if (head) {
             const unsigned after = lane == 31 ? 0u : brk >> (lane + 1);
             const uint32_t run = after ? (uint32_t)__ffs(after) : 32u - lane;
-            atomicAdd(&s_hist[d][dig], run);
+            atomicAdd(&s_hist[5][top & 0xff], run);
+            atomicAdd(&s_hist[6][(top >> 8) & 0xff], run);
+            atomicAdd(&s_hist[7][top >> 16], run);
+          }
+        } else {
+          for (int d = first_digit; d < 8; ++d) {
+            const uint32_t dig = v ? (uint32_t)(code >> (8 * d)) & 0xff : 0x100u;
+            const uint32_t prev = __shfl_up_sync(0xffffffffu, dig, 1);
+            const bool head = v && (lane == 0 || prev != dig);
+            const unsigned brk = __ballot_sync(0xffffffffu, head || !v);   // where runs start or are interrupted
+            if (head) {
+              const unsigned after = lane == 31 ? 0u : brk >> (lane + 1);
+              const uint32_t run = after ? (uint32_t)__ffs(after) : 32u - lane;
+              atomicAdd(&s_hist[d][dig], run);
+            }
           }
         }
         pos += __popc(act);

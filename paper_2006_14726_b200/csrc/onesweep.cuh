@@ -378,6 +378,7 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
 constexpr int WIN_G = 3;                 // global passes (digits 5, 6, 7)
 constexpr int WIN_BSHIFT = 8 * (8 - WIN_G);
 constexpr int WIN_BUCKET_MAX = 512;      // counting is quadratic in the bucket size
+static_assert(WIN_G == 3, "unproject_kernel counts the digits 5 .. 7 for this mode");
 static_assert(WIN_MAX <= (1 << (64 - 40)) && WIN_BSHIFT == 40, "comparison key = 40 code bits + position");
 
 constexpr int WIN_EXTRA = 512;           // a window is loaded with this many elements beyond its nominal end
@@ -505,7 +506,7 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
     // a bucket did not fit: LSD passes over the digits d0 .. 7 from where the array is now (every step so far
     // was a stable permutation; d0 is even so that the result ends in buffer 0), then the global fix-up
     const int d0 = first & ~1;
-    count_digits(s, a.key[0], a.st, n, gridDim.x, d0, first);
+    count_digits(s, a.key[0], a.st, n, gridDim.x, d0, 8 - WIN_G);   // unproject_kernel counted the digits of the global passes only
     grid_barrier(bar, gridDim.x, round);
     lsd(d0, buf);
     if (blockIdx.x < nb) fixup_runs<ITEMS>(a.key[0], a.val[0], a.st, n, num_tiles, 8 * first);
