@@ -212,7 +212,9 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
                  uint32_t* __restrict__ ids0, uint64_t* __restrict__ keys1, uint32_t* __restrict__ ids1,
                  int sort_mode) {
   pdl_wait();
+#if SPLATS_LATE_TRIGGER < 2
   pdl_trigger();
+#endif
   __shared__ uint32_t s_hist[8][256];
   __shared__ uint32_t s_warp[BUILD_THREADS / 32];
   __shared__ uint32_t s_part[BUILD_THREADS / 32];

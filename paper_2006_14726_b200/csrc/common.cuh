@@ -25,6 +25,14 @@ __device__ __forceinline__ float sqrt_(float a) { return __fsqrt_rn(a); }
 // are no-ops.  pdl_trigger() lets the successor's blocks be scheduled once every block of this
 // grid has started (they then sit in pdl_wait), which hides the launch latency between the
 // short dependent kernels of one update.
+// Which kernels release their dependent launch early (griddepcontrol.launch_dependents at their start) and which
+// only when their blocks exit: 0 = all early; 1 = sort and tile kernel late; 2 = unproject too (default); 3 = spine
+// too.  A dependent's blocks become resident as soon as they are released and spin in their wait: behind a short
+// kernel that is harmless, behind a long one (sort, tile kernel) the waiting blocks take SM resources from the
+// kernel they wait for.  Released at exit, the dependent's launch latency still hides behind the predecessor's tail.
+#ifndef SPLATS_LATE_TRIGGER
+#define SPLATS_LATE_TRIGGER 2
+#endif
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 

@@ -552,7 +552,9 @@ __device__ __forceinline__ int sort_pick_items(uint32_t n, uint32_t grid) {
 __global__ void __launch_bounds__(SORT_THREADS, SPLATS_SORT_BLOCKS)
 onesweep_kernel(SortArgs a) {
   pdl_wait();
-  pdl_trigger();
+#if !SPLATS_LATE_TRIGGER
+  pdl_trigger();   // (with SPLATS_LATE_TRIGGER the dependent launch is released when the blocks exit)
+#endif
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SortSmem& s = *reinterpret_cast<SortSmem*>(smem_raw);
   const uint32_t n = a.st->n;

@@ -23,7 +23,7 @@
 #include "tree_tile.cuh"
 
 #ifndef SPLATS_PDL_MASK
-#define SPLATS_PDL_MASK 35
+#define SPLATS_PDL_MASK 63
 #endif
 
 namespace {
@@ -287,10 +287,9 @@ int do_update(Context* c, const Src& src, const Gather& gather, int64_t P, bool 
   if (prof) m[0] = c->mark();
   const bool pdl = c->pdl && !prof;   // per-stage events need the stages to be disjoint in time
   // Which kernels are launched as programmatic dependents (SPLATS_OPT_PDL): bounds (1), unproject (2), sort (4),
-  // tile (8), spine (16), the first render after an update (32).  A dependent's blocks become resident early and
-  // spin in griddepcontrol.wait: behind a short predecessor that hides the launch latency; behind a long one (sort,
-  // tile kernel) the waiting blocks cost more than the 3 us they save (measured: dense update 0.315 -> 0.302 ms,
-  // config 3 10.59 k -> 10.87 k frames/s with 35 instead of 63).
+  // tile (8), spine (16), the first render after an update (32).  Measured per kernel; with the early release of
+  // the dependents only behind short kernels (common.cuh, SPLATS_LATE_TRIGGER) all of them gain: dense update
+  // 0.291 -> 0.283 ms, config 3 11.0 k -> 11.2 k frames/s against 35 (sort, tile and spine as ordinary launches).
   constexpr int pdl_mask = SPLATS_PDL_MASK;
   if (!async) c->render_streak = 0;   // (a decoupled build runs on its own stream: the renders in flight stay tracked)
   // bounds_kernel waits for its predecessor at its first instruction; overlapping renders

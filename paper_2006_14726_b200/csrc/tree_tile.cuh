@@ -138,7 +138,9 @@ tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__
                  QNode* __restrict__ qnodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min,
                  uint16_t* __restrict__ tile_fb) {
   pdl_wait();
+#if !SPLATS_LATE_TRIGGER
   pdl_trigger();
+#endif
   extern __shared__ __align__(16) unsigned char tt_smem_raw[];
   TileSmem& s = *reinterpret_cast<TileSmem*>(tt_smem_raw);
   const int n = (int)st->n;
@@ -512,7 +514,9 @@ tree_spine_kernel(const uint64_t* __restrict__ keys, FrameState* st, const int4*
                   const float4* __restrict__ sphere, const uint4* __restrict__ pyr, QNode* __restrict__ qnodes,
                   const uint8_t* __restrict__ tile_min, const uint16_t* __restrict__ tile_fb, int nt_log) {
   pdl_wait();
+#if SPLATS_LATE_TRIGGER < 3
   pdl_trigger();
+#endif
   extern __shared__ __align__(16) unsigned char spine_smem[];
   uint8_t* m = spine_smem;
   const int n = (int)st->n;
