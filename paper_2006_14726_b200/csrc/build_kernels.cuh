@@ -253,7 +253,7 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
   const uint32_t n_all = st->n;
   const bool odd = sort_input_buffer(sort_mode, n_all) != 0;
   // lowest digit whose histogram the sort launch reads from here (it counts any others itself, on its fallback paths)
-  const int first_digit = sort_mode == SORT_HYBRID ? 8 - 3 : sort_mode == SORT_HYBRID_LSD ? hybrid_first_digit(n_all) : 0;
+  const int first_digit = sort_mode == SORT_HYBRID ? 8 - win_passes(n_all) : sort_mode == SORT_HYBRID_LSD ? hybrid_first_digit(n_all) : 0;
   uint64_t* __restrict__ keys = odd ? keys1 : keys0;
   uint32_t* __restrict__ ids = odd ? ids1 : ids0;
   float lo[3], ext[3];
@@ -313,7 +313,7 @@ unproject_kernel(const Src src, int64_t P, int num_tiles,
         // digit histograms: neighbouring pixels mostly share their top digits, so each run of equal digits among
         // consecutive valid lanes is counted by its first lane (one shared-memory atomic per run and digit)
         if (first_digit == 5) {
-          // the windowed sort reads the digits 5 .. 7 only: runs of equal top 24 key bits, found once for all three
+          // the windowed sort reads the digits 5 .. 7 only (up to 2^23 splats): runs of equal top 24 key bits, found once for all three
           const uint32_t top = v ? (uint32_t)(code >> 40) : 0xffffffffu;
           const uint32_t prev = __shfl_up_sync(0xffffffffu, top, 1);
           const bool head = v && (lane == 0 || prev != top);

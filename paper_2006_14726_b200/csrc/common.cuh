@@ -173,8 +173,10 @@ __host__ __device__ __forceinline__ bool sort_is_hybrid(int mode) { return mode 
 #endif
 constexpr uint32_t HYBRID5_MIN = 1u << SPLATS_HYBRID5_LOG;
 __host__ __device__ __forceinline__ int hybrid_first_digit(uint32_t n) { return n > HYBRID5_MIN ? 3 : 4; }
+// global passes of the windowed hybrid sort: the top 24 key bits, 32 above 2^23 splats (buckets stay at a few dozen keys)
+__host__ __device__ __forceinline__ int win_passes(uint32_t n) { return n > (1u << 23) ? 4 : 3; }
 __host__ __device__ __forceinline__ int sort_input_buffer(int mode, uint32_t n) {
-  if (mode == SORT_HYBRID) return 1;   // three global passes, then the buckets in place in buffer 0
+  if (mode == SORT_HYBRID) return win_passes(n) & 1;   // the global passes end in buffer 0, where the buckets are put in order in place
   return (mode == SORT_HYBRID_LSD && (hybrid_first_digit(n) & 1)) ? 1 : 0;
 }
 

@@ -375,15 +375,12 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
 // thread takes an element and counts the keys of its bucket that come before it (stable, by the full code: no
 // fix-up afterwards), which is its place, and the window is written back in place.  No status words, no look-back, no grid barrier.  A bucket that does not fit (> WIN_BUCKET_MAX keys, or
 // a window > WIN_MAX) raises st->sort_wfall and the launch falls back to LSD passes.
-constexpr int WIN_G = 3;                 // global passes (digits 5, 6, 7)
-constexpr int WIN_BSHIFT = 8 * (8 - WIN_G);
 constexpr int WIN_BUCKET_MAX = 512;      // counting is quadratic in the bucket size
-static_assert(WIN_G == 3, "unproject_kernel counts the digits 5 .. 7 for this mode");
-static_assert(WIN_MAX <= (1 << (64 - 40)) && WIN_BSHIFT == 40, "comparison key = 40 code bits + position");
+static_assert(WIN_MAX <= (1 << 24), "comparison key = the key bits below the bucket's (<= 40) + position");
 
 constexpr int WIN_EXTRA = 512;           // a window is loaded with this many elements beyond its nominal end
 
-__device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_t* val, FrameState* st, uint32_t n) {
+__device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, const int WIN_BSHIFT) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint32_t* heads = s.tile_off;   // one bit per loaded element: a bucket starts here (128 words)
   // nominal window size: what the capacity allows, a quarter of it for small frames (more windows than blocks)
@@ -396,13 +393,13 @@ __device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_
       s.stage[i] = __ldcg(key + g0 + i);
       s.vstage[i] = __ldcg(val + g0 + i);
     }
-    const uint64_t kprev = g0 > 0 ? __ldcg(key + g0 - 1) : ~0ull;   // (code bits >= WIN_BSHIFT of ~0 match no real key: bit 63)
+    const uint64_t kprev = g0 > 0 ? __ldcg(key + g0 - 1) : 0ull;
     __syncthreads();
     // bucket heads as a bit map (chunk c = elements 32 c .. 32 c + 31 of the loaded range)
     const uint32_t nchunk = (cnt + 31) >> 5;
     for (uint32_t c = warp; c < nchunk; c += SORT_WARPS) {
       const uint32_t i = c * 32 + lane;
-      const bool head = i < cnt && ((i == 0 ? kprev : s.stage[i - 1]) >> WIN_BSHIFT) != (s.stage[i] >> WIN_BSHIFT);
+      const bool head = i < cnt && ((i == 0 && g0 == 0) || ((i == 0 ? kprev : s.stage[i - 1]) >> WIN_BSHIFT) != (s.stage[i] >> WIN_BSHIFT));
       const unsigned m = __ballot_sync(0xffffffffu, head);
       if (lane == 0) heads[c] = m;
       // comparison key inside a bucket: the 39 code bits below the bucket's, then the position (unique: no ties)
@@ -499,8 +496,9 @@ __device__ __forceinline__ void run_sort(SortSmem& s, const SortArgs& a, uint32_
   int buf = sort_input_buffer(a.mode, n);
   if (a.mode == SORT_HYBRID) {
     // ---- three global passes over the top digits, then bucket by bucket in shared memory
-    lsd(8 - WIN_G, buf);                 // ends in buffer 0 (an odd number of passes from buffer 1)
-    window_phase(s, a.key[0], a.val[0], a.st, n);
+    const int WIN_G = win_passes(n);
+    lsd(8 - WIN_G, buf);                 // ends in buffer 0 (sort_input_buffer)
+    window_phase(s, a.key[0], a.val[0], a.st, n, 8 * (8 - WIN_G));
     grid_barrier(bar, gridDim.x, round);
     if (*reinterpret_cast<volatile uint32_t*>(&a.st->sort_wfall) == 0u) return;
     // a bucket did not fit: LSD passes over the digits d0 .. 7 from where the array is now (every step so far

@@ -118,3 +118,15 @@ def test_table1_shape_leg_of_the_bench():
             px = rng.choice(cfg.W * cfg.H, size=50_000, replace=False).astype(np.int64)
             got = s.render(cam, cfg.W, cfg.H, first_hit=True).reshape(-1, 4)[px]
             assert np.array_equal(got, oracle.render(sc, cam, cfg.W, cfg.H, "bvh", pixels=px, first_hit=True))
+
+
+def test_beyond_2_23_splats_four_global_sort_passes():
+    # more than 2^23 splats: the windowed sort runs four global passes (an even number: the other input buffer)
+    W, H = 4096, 2304
+    color, depth, cam = synth.dense_frame(W, H, 0)
+    sc = oracle.build_scene(color, depth, cam, W, H, 1.0)
+    assert sc["N"] == W * H > (1 << 23)
+    with Session(W, H, exact_nodes=False) as s:
+        s.update(color, depth, cam, W, H, 1.0)
+        assert_bvh_bit_exact(sc, exact=False)
+        _check_renders(s, sc, [synth.orbit_camera(2.0)], W, H, False, 20_000, 64, 70)
