@@ -274,12 +274,12 @@ int splats_export_splats(float* sphere, float* rgba, float* lo_hi);
  *     SPLATS_REFIT_ATOMIC: one thread per leaf climbs the tree; the second arrival at a node's
  *       atomic counter forms the union and continues (the classic LBVH refit).
  *   SPLATS_OPT_SORT: how step a3 (order by (code, id)) is computed.
- *     SPLATS_SORT_HYBRID (default): one launch; 2 onesweep passes over the top 15 code bits (3 over the
- *       top 23 above 2^19 splats), after which the array is a sequence of small buckets; every bucket is
- *       then ordered by the next two digits in shared memory, window by window, and keys that still tie
- *       there (none for one-sample-per-pixel frames) by the full code.  A bucket larger than a window
- *       makes the launch fall back to the passes of SPLATS_SORT_HYBRID_LSD.
- *     SPLATS_SORT_HYBRID_LSD: one launch; 4 onesweep passes over the top 31 code bits (5 over the top 39
+ *     SPLATS_SORT_HYBRID (default): one launch; 3 onesweep passes over the top 24 code bits (4 over the
+ *       top 32 above 2^23 splats), after which the array is a sequence of small buckets (a few to a few
+ *       dozen keys of a one-sample-per-pixel frame); every bucket is then put in order by (code, id) in
+ *       shared memory, window by window, by counting.  A bucket of more than 512 keys makes the launch
+ *       fall back to the passes of SPLATS_SORT_HYBRID_LSD from where the array is.
+ *     SPLATS_SORT_HYBRID_LSD: one launch; 4 onesweep passes over the top 32 code bits (5 over the top 40
  *       above 2^19 splats), then a check that no two neighbours share them; short runs are fixed up by a
  *       stable insertion sort, longer ones make the same launch redo the sort with all 8 passes.
  *     SPLATS_SORT_LSD8: all 8 passes in one launch (grid barriers between the passes).
