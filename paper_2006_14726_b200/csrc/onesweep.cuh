@@ -42,7 +42,11 @@ constexpr uint32_t VALUE_MASK = (1u << 30) - 1;
 #ifndef SPLATS_LOOKBACK
 #define SPLATS_LOOKBACK 8
 #endif
-constexpr int LOOKBACK = SPLATS_LOOKBACK;
+constexpr int LOOKBACK = SPLATS_LOOKBACK;       // status words per round trip of the two-level sum (one wave)
+#ifndef SPLATS_LOOKBACK_CHAIN
+#define SPLATS_LOOKBACK_CHAIN 4
+#endif
+constexpr int LOOKBACK_CHAIN = SPLATS_LOOKBACK_CHAIN;   // ... of the chained look-back (several waves): measured 2 .. 8
 constexpr int RUN_MAX = 32;           // longest run of equal top bits fixed up in place
 
 struct SortArgs {
@@ -268,20 +272,20 @@ __device__ __forceinline__ void onesweep_pass(SortSmem& s, const uint64_t* kin, 
       excl = s.digit_base[tid];
     } else {
       excl = 0;
-      // LOOKBACK predecessors per round trip: below a few million elements all tiles of a wave
+      // LOOKBACK_CHAIN predecessors per round trip: below a few million elements all tiles of a wave
       // publish their aggregates at about the same time, so the walk back to an inclusive
-      // prefix is a chain of about tiles / (2 LOOKBACK) L2 round trips.
+      // prefix is a chain of about tiles / (2 LOOKBACK_CHAIN) L2 round trips.
       int t = tile - 1;
       bool done = false;
       while (!done) {
-        uint64_t w[LOOKBACK];
+        uint64_t w[LOOKBACK_CHAIN];
 #pragma unroll
-        for (int k = 0; k < LOOKBACK; ++k)
+        for (int k = 0; k < LOOKBACK_CHAIN; ++k)
           w[k] = t - k >= 0 ? ld_volatile_u64(status + (size_t)(t - k) * RADIX + tid) : 0ull;
         bool stalled = false;
         int used = 0;
 #pragma unroll
-        for (int k = 0; k < LOOKBACK; ++k) {
+        for (int k = 0; k < LOOKBACK_CHAIN; ++k) {
           if (!done && !stalled) {
             if ((w[k] >> 32) != epoch || (w[k] & (FLAG_AGG | FLAG_INC)) == 0) {
               stalled = true;  // not published yet: poll again from this tile
@@ -375,10 +379,13 @@ __device__ __forceinline__ void fixup_runs(uint64_t* key, uint32_t* val, FrameSt
 // thread takes an element and counts the keys of its bucket that come before it (stable, by the full code: no
 // fix-up afterwards), which is its place, and the window is written back in place.  No status words, no look-back, no grid barrier.  A bucket that does not fit (> WIN_BUCKET_MAX keys, or
 // a window > WIN_MAX) raises st->sort_wfall and the launch falls back to LSD passes.
-constexpr int WIN_BUCKET_MAX = 512;      // counting is quadratic in the bucket size
+#ifndef SPLATS_WIN_EXTRA
+#define SPLATS_WIN_EXTRA 512
+#endif
+constexpr int WIN_BUCKET_MAX = SPLATS_WIN_EXTRA;      // counting is quadratic in the bucket size
 static_assert(WIN_MAX <= (1 << 24), "comparison key = the key bits below the bucket's (<= 40) + position");
 
-constexpr int WIN_EXTRA = 512;           // a window is loaded with this many elements beyond its nominal end
+constexpr int WIN_EXTRA = SPLATS_WIN_EXTRA;           // a window is loaded with this many elements beyond its nominal end
 
 __device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, const int WIN_BSHIFT) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
