@@ -398,6 +398,10 @@ __device__ __forceinline__ void write_node(const float4* __restrict__ sphere, co
 // runs beside leaf_pyramid_kernel (it is launched as a programmatic dependent that does not wait
 // for it at the start but at the end, so that the kernel after it is ordered after both), and
 // boxes_kernel then joins the two: ranges + pyramid -> node records.
+// Invariant behind wait_at_start = 0 (and behind renders / bounds_kernel that skip the wait): the kernel only reads
+// what a grid BEFORE its predecessor in the stream produced (here: the sorted keys, written by onesweep_kernel; the
+// predecessor is leaf_pyramid_kernel).  That grid has retired: every block of the predecessor passed its own
+// griddepcontrol.wait, i.e. saw that grid complete and flushed, before this kernel could be released.
 __global__ void __launch_bounds__(LBVH_THREADS)
 hierarchy_kernel(const uint64_t* __restrict__ keys, const FrameState* __restrict__ st, int4* __restrict__ ranges, int wait_at_start) {
   if (wait_at_start) pdl_wait();
