@@ -186,6 +186,29 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
                 float r_scale, const wr_quant* quant, unsigned long long* samples, unsigned* colors,
                 unsigned* count);
 
+/* splats_pack for callers that must not allocate: no context, no cudaMalloc / cudaFree / allocating
+ * library call, usable without splats_create (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid allocation).  Same result as splats_pack, bit for bit; the per-tile counts
+ * of the compaction, which splats_pack keeps in scratch memory of the context, live in a
+ * file-scope `static __device__` array of the library instead: 32 KiB, held by every GPU that
+ * loads the library until the process exits.
+ *   radius_mode, radius_param   as splats_set_radius (there is no context to read them from)
+ *   cuda_stream                 cudaStream_t (NULL = the default stream) the two launches go to
+ *   everything else             as splats_pack
+ * Limit: W*H <= SPLATS_NOALLOC_MAX_PIXELS (4096 x 4096); beyond it the call fails with EINVAL and
+ * does nothing.  The array is shared by every call and keeps the last call's contents; every
+ * word a call reads it has written first, so nothing has to be cleared -- but two calls that
+ * overlap on the GPU (different streams, or one device from two threads) race on it: serialise
+ * them.  The array's device address is looked up once per device (cudaGetSymbolAddress, with that
+ * device current) on the first call there, or ahead of time by splats_noalloc_setup (e.g. before
+ * a capture begins).  Errors: EINVAL (null / misaligned pointers, sizes, camera, r_scale, radius
+ * mode, box), ECUDA. */
+#define SPLATS_NOALLOC_MAX_PIXELS (4096 * 4096)
+int splats_noalloc_setup(void);
+int splats_pack_noalloc(const float* color, const float* depth, const wr_camera* src_camera, int W, int H,
+                        float r_scale, int radius_mode, float radius_param, const wr_quant* quant,
+                        unsigned long long* samples, unsigned* colors, unsigned* count, void* cuda_stream);
+
 /* Client side, the paper's literal entry point ("The client upon receiving the
  * data will build an LBVH"): build the splats and the BVH from n received samples.  Splat ids are
  * positions in the buffer; a sample whose radius field is 0 is dropped.  The buffers must stay

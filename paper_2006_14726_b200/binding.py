@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L.splats_march.argtypes = [_vp, _ci, ctypes.POINTER(wr_transfer), cam_p, _ci, _ci, _vp, _vp]
         L.splats_pack.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, ctypes.POINTER(wr_quant), _vp, _vp, _vp]
         L.splats_update_packed.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
+        L.splats_pack_noalloc.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float, _ci, ctypes.c_float, ctypes.POINTER(wr_quant),
+                                          _vp, _vp, _vp, _vp]
         L.splats_update_packed_host.argtypes = [_vp, _vp, ctypes.c_uint, ctypes.POINTER(wr_quant)]
         L.splats_update_host.argtypes = [_vp, _vp, cam_p, _ci, _ci, ctypes.c_float]
         L.splats_render_host.argtypes = [cam_p, _ci, _ci, _vp]
@@ -196,6 +198,30 @@ def splats_pack(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, H:
                              ctypes.byref(c), int(W), int(H), float(r_scale), ctypes.byref(q),
                              _dev_ptr(samples, torch.int64, W * H), _dev_ptr(colors, torch.int32, W * H),
                              _dev_ptr(count, torch.int32, 1)))
+
+
+NOALLOC_MAX_PIXELS = 4096 * 4096
+
+
+def splats_noalloc_setup() -> None:
+    """Look up the static scratch array's address on the current device ahead of the first splats_pack_noalloc."""
+    _check(lib().splats_noalloc_setup())
+
+
+def splats_pack_noalloc(color: torch.Tensor, depth: torch.Tensor, src_camera, W: int, H: int, r_scale: float, quant,
+                        samples: torch.Tensor, colors: torch.Tensor, count: torch.Tensor,
+                        radius_mode: int = 0, radius_param: float = 0.0, stream=None) -> None:
+    """splats_pack without a context and without any allocation (include/splats.h): W*H <= NOALLOC_MAX_PIXELS.
+    stream: a torch.cuda.Stream (default: torch's current stream)."""
+    c, q = _cam(src_camera), _quant(quant)
+    if int(W) * int(H) > NOALLOC_MAX_PIXELS:   # let the library say so: no buffer of that size is needed for the check
+        ptrs = [t.data_ptr() for t in (color, depth, samples, colors, count)]
+    else:
+        ptrs = [_dev_ptr(color, torch.float32, W * H * 4), _dev_ptr(depth, torch.float32, W * H),
+                _dev_ptr(samples, torch.int64, W * H), _dev_ptr(colors, torch.int32, W * H), _dev_ptr(count, torch.int32, 1)]
+    st = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+    _check(lib().splats_pack_noalloc(ptrs[0], ptrs[1], ctypes.byref(c), int(W), int(H), float(r_scale), int(radius_mode),
+                                     float(radius_param), ctypes.byref(q), ptrs[2], ptrs[3], ptrs[4], ctypes.c_void_p(st)))
 
 
 def splats_update_packed(samples: torch.Tensor, colors: torch.Tensor, n: int, quant) -> None:

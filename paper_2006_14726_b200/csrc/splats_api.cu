@@ -267,6 +267,40 @@ RadiusParams make_radius(const Context* c, const wr_camera* cam, int H, float r_
   return rp;
 }
 
+// ---- splats_pack_noalloc (include/splats.h): the compaction's per-tile counts in a file-scope device array
+// instead of context memory.  One word per tile of TILE_PX pixels; 32 KiB + one line, resident on every GPU that
+// loads this library until the process exits.  In host code the NAME of the array is a host-side stand-in, not
+// a device address: the kernels get the address that cudaGetSymbolAddress returns for the current device.
+constexpr int NOALLOC_MAX_TILES = SPLATS_NOALLOC_MAX_PIXELS / TILE_PX;
+static __device__ __align__(256) uint32_t g_noalloc_tile_count[NOALLOC_MAX_TILES + 64];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+struct NoallocDevice {
+  uint32_t* tile_count = nullptr;   // device address of g_noalloc_tile_count on this device
+  int num_sms = 0;
+};
+NoallocDevice g_noalloc[NOALLOC_MAX_DEVICES];
+
+// Once per device, with that device current.  No allocation: a symbol look-up and an attribute query.
+int noalloc_device(NoallocDevice** out) {
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(SPLATS_EINVAL, "splats_pack_noalloc: device index beyond 63");
+  NoallocDevice& d = g_noalloc[dev];
+  if (!d.tile_count) {
+    uint32_t* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_noalloc_tile_count);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_noalloc_tile_count)");
+    if (!ptr) return fail(SPLATS_ECUDA, "cudaGetSymbolAddress returned a null address for the static scratch array");
+    int sms = 0;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    d.num_sms = sms;
+    d.tile_count = ptr;
+  }
+  *out = &d;
+  return SPLATS_OK;
+}
+
 // The launch sequence of one update: a1 bounds, a2 keys + compaction, a3 sort, a4/a5 tree.
 // Src yields the splat centres of elements [0, P) (build_kernels.cuh), Gather the sphere and
 // colour of a splat id (lbvh.cuh).
@@ -743,6 +777,60 @@ int splats_pack(const float* color, const float* depth, const wr_camera* src_cam
   pack_write_kernel<<<grid2, BUILD_THREADS, 0, c->stream>>>(a, c->pack_tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
   if (c->profiling) c->spans.push_back({6, m0, c->mark()});
   c->launches += 2;
+  CU(cudaGetLastError());
+  return SPLATS_OK;
+}
+
+int splats_noalloc_setup(void) {
+  NoallocDevice* d = nullptr;
+  return noalloc_device(&d);
+}
+
+int splats_pack_noalloc(const float* color, const float* depth, const wr_camera* src_camera, int W, int H, float r_scale,
+                        int radius_mode, float radius_param, const wr_quant* quant, unsigned long long* samples,
+                        unsigned* colors, unsigned* count, void* cuda_stream) {
+  // needs no context and calls no cudaMalloc / cudaFree: everything it touches is the caller's or the static array
+  if (!color || !depth || !src_camera || !quant || !samples || !colors || !count) return fail(SPLATS_EINVAL, "null pointer argument");
+  if (W <= 0 || H <= 0) return fail(SPLATS_EINVAL, "W and H must be positive");
+  if ((int64_t)W * H > (int64_t)SPLATS_NOALLOC_MAX_PIXELS)
+    return fail(SPLATS_EINVAL, "splats_pack_noalloc: W*H = " + std::to_string((long long)W * H) + " exceeds the static scratch array's maximum of " +
+                                   std::to_string((long long)SPLATS_NOALLOC_MAX_PIXELS) + " pixels (SPLATS_NOALLOC_MAX_PIXELS); use splats_pack");
+  if (!finite_camera(src_camera)) return fail(SPLATS_EINVAL, "camera is not finite or tan_half_fovy <= 0");
+  if (!(r_scale > 0.0f) || !std::isfinite(r_scale)) return fail(SPLATS_EINVAL, "r_scale must be finite and > 0");
+  if ((reinterpret_cast<uintptr_t>(color) | reinterpret_cast<uintptr_t>(depth)) & 15u)
+    return fail(SPLATS_EINVAL, "color/depth must be 16-byte aligned");
+  if (radius_mode != SPLATS_RADIUS_FOOTPRINT && radius_mode != SPLATS_RADIUS_CONSTANT && radius_mode != SPLATS_RADIUS_OPACITY)
+    return fail(SPLATS_EINVAL, "unknown radius mode");
+  if (radius_mode == SPLATS_RADIUS_CONSTANT && !(radius_param > 0.0f && std::isfinite(radius_param)))
+    return fail(SPLATS_EINVAL, "constant radius must be finite and > 0");
+  if (radius_mode == SPLATS_RADIUS_OPACITY && !(radius_param >= 0.0f && radius_param <= 1.0f))
+    return fail(SPLATS_EINVAL, "opacity radius floor must be in [0, 1]");
+  PackArgs a;
+  if (!make_quant(quant, &a.q)) return fail(SPLATS_EINVAL, "quantisation box must be finite with hi > lo, r_max finite and > 0");
+  NoallocDevice* d = nullptr;
+  int rc = noalloc_device(&d);
+  if (rc) return rc;
+  a.color = reinterpret_cast<const float4*>(color);
+  a.depth = depth;
+  a.cam = make_camera(src_camera, W, H);
+  {  // as make_radius, with the mode and parameter of the call (separately rounded float32 operations)
+    const float param = radius_mode == SPLATS_RADIUS_FOOTPRINT ? 0.0f : radius_param;
+    a.rp.mode = radius_mode;
+    a.rp.k_r = radius_factor(src_camera, H, r_scale);
+    volatile float rc_ = r_scale * param;
+    volatile float w1 = 1.0f - param;
+    a.rp.r_const = rc_;
+    a.rp.f_min = param;
+    a.rp.w1 = w1;
+  }
+  a.P = (int64_t)W * H;
+  a.num_tiles = (int)((a.P + TILE_PX - 1) / TILE_PX);   // <= NOALLOC_MAX_TILES by the check above
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+  // the array keeps the previous call's counts; pack_count_kernel overwrites every word [0, num_tiles) that
+  // pack_write_kernel reads, so nothing has to be cleared
+  pack_count_kernel<<<a.num_tiles, BUILD_THREADS, 0, s>>>(a, d->tile_count);
+  const int grid2 = a.num_tiles < d->num_sms * 4 ? a.num_tiles : d->num_sms * 4;
+  pack_write_kernel<<<grid2, BUILD_THREADS, 0, s>>>(a, d->tile_count, reinterpret_cast<uint64_t*>(samples), colors, count);
   CU(cudaGetLastError());
   return SPLATS_OK;
 }
