@@ -561,3 +561,39 @@ def test_quantised_boxes_contain_the_exact_ones():
     eps = 1e-6 * np.abs(want).max()
     assert np.all(lo <= want[:, :, 0:3] + eps) and np.all(hi >= want[:, :, 3:6] - eps)
     assert np.all(lo >= want[:, :, 0:3] - step - eps) and np.all(hi <= want[:, :, 3:6] + step + eps)
+
+
+def test_alternating_frames_under_overlap_stress():
+    # ADVICE (round 1): kernels that skip griddepcontrol.wait read through the non-coherent path what an earlier
+    # grid produced.  Two frames of very different N alternate for ten updates, three renders behind each, all
+    # enqueued back to back with SPLATS_OPT_OVERLAP on and no synchronisation: the BVH sets, key buffers, frame
+    # states and status words are reused every other update, so a stale line or a kernel running ahead of its
+    # producer shows up as a wrong image or a wrong tree at the end.
+    cfg = synth.make_config(1)
+    W, H = cfg.W, cfg.H
+    colA, depA = synth.source_frame(cfg, 0)
+    camA = cfg.src_cams[0]
+    colB, depB, camB = synth.random_frame(W, H, seed=9, fill=0.35)
+    scenes = [oracle.build_scene(colA, depA, camA, W, H, 1.0), oracle.build_scene(colB, depB, camB, W, H, 1.0)]
+    assert scenes[1]["N"] > 3 * scenes[0]["N"]
+    cams = [synth.orbit_camera(3.0), synth.orbit_camera(-6.0, 2.0), synth.orbit_camera(11.0)]
+    rng = np.random.default_rng(3)
+    px = np.sort(rng.choice(W * H, size=30_000, replace=False)).astype(np.int64)
+    refs = [[oracle.render(sc, cam, W, H, "bvh", pixels=px) for cam in cams] for sc in scenes]
+    frames = [(torch.from_numpy(colA).cuda(), torch.from_numpy(depA).cuda(), camA),
+              (torch.from_numpy(colB).cuda(), torch.from_numpy(depB).cuda(), camB)]
+    n_updates = 10
+    with Session(W, H, exact_nodes=False):
+        sp.splats_set_option(sp.OPT_OVERLAP, 1)
+        outs = [[torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda") for _ in cams] for _ in range(n_updates)]
+        for it in range(n_updates):
+            dc, dd, cam = frames[it & 1]
+            sp.splats_update(dc, dd, cam, W, H, 1.0)
+            for j, c in enumerate(cams):
+                sp.splats_render(c, W, H, outs[it][j])
+        torch.cuda.synchronize()
+        assert_bvh_bit_exact(scenes[(n_updates - 1) & 1], exact=False)
+        for it in range(n_updates):
+            for j in range(len(cams)):
+                got = outs[it][j].cpu().numpy().reshape(-1, 4)[px]
+                assert_rgba_close(got, refs[it & 1][j], f"update {it}, camera {j}")
