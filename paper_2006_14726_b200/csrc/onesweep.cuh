@@ -394,7 +394,11 @@ __device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_
   const uint32_t T = n > (uint32_t)gridDim.x * (WIN_MAX / 4) ? WIN_MAX - WIN_EXTRA : WIN_MAX / 4;
   const uint32_t nwin = (n + T - 1) / T;
   for (uint32_t k = blockIdx.x; k < nwin; k += gridDim.x) {
-    // ---- load [k T, (k + 1) T + WIN_EXTRA) in one go; the window proper, [B(k T), B((k + 1) T)), is found in it
+    // ---- load [k T, (k + 1) T + WIN_EXTRA) in one go; the window proper, [B(k T), B((k + 1) T)), is found in it.
+    // The loaded range overlaps the neighbouring windows, which other blocks may be writing at the same time.
+    // That is harmless: outside its own window a block looks at the bucket bits of a key only (to find the heads),
+    // and a neighbour only permutes keys inside buckets, so those bits are the same before, during and after its
+    // writes (64-bit stores: a key is seen old or new, never torn); the windows proper are disjoint.
     const uint32_t g0 = k * T, gend = min(n, g0 + T + WIN_EXTRA), cnt = gend - g0;
     for (uint32_t i = tid; i < cnt; i += SORT_THREADS) {
       s.stage[i] = __ldcg(key + g0 + i);
