@@ -4,7 +4,9 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 legs may import this package.  The product (paper_2006_14726_b200) never does, and
 this package never imports the product.  The arithmetic lives in splat_oracle.cpp
 (single-threaded C++, float32 with the op order of DESIGN.md sec. 3); this file
-only compiles it and marshals numpy arrays.
+compiles it and marshals numpy arrays.  One step is stated here in numpy instead:
+quantise_child_boxes (O7b), the 16-bit storage format of the node boxes -- a reading
+of this repository (S13), not something the paper defines.
 """
 from __future__ import annotations
 
@@ -258,6 +260,39 @@ def build_scene_packed(samples, colours, quant):
     return dict(N=n, sphere=sphere, valid=valid, lo=lo, hi=hi, ids=ids, codes=codes, order=order,
                 sorted_ids=sorted_ids, sorted_codes=sorted_codes, sphere_sorted=sphere_sorted,
                 rgba_sorted=rgba_sorted, children=children, parents=parents, ranges=ranges, aabbs=aabbs)
+
+
+def quantise_child_boxes(scene):
+    """O7b (S13; the paper says nothing about how node boxes are stored): the traversal
+    records that follow from the exact tree of O6 / O7.  Frame: rmax = largest splat radius,
+    qlo_a = lo_a - rmax, ext_a = (hi_a + rmax) - qlo_a (lo / hi: bounds of the centres, O3),
+    s_a = 65535 / ext_a (0 for a zero extent).  A lower plane x of a child box becomes
+    clamp(floor((x - qlo_a) * s_a), 0, 65535), an upper plane clamp(ceil(...), 0, 65535); every
+    operation rounded to float32 on its own.  Returns (records, frame):
+      records  (N-1, 8) uint32 per internal node: words 0..2 = axis x, y, z of the left child box,
+               q_lo | q_hi << 16; words 3..5 the right child's; words 6, 7 = left / right link
+               (internal node index, or 0x80000000 | sorted position of a leaf)
+      frame    7 float32: lo xyz, hi xyz, rmax"""
+    n = scene["N"]
+    f32 = np.float32
+    if n < 2:
+        return np.zeros((0, 8), np.uint32), None
+    rmax = f32(scene["sphere_sorted"][:, 3].max())
+    lo, hi = scene["lo"].astype(f32), scene["hi"].astype(f32)
+    qlo = (lo - rmax).astype(f32)
+    ext = ((hi + rmax).astype(f32) - qlo).astype(f32)
+    with np.errstate(divide="ignore"):
+        s = np.where(ext > 0, (f32(65535.0) / ext).astype(f32), f32(0.0)).astype(f32)
+    boxes = scene["aabbs"][scene["children"]].astype(f32)               # (n-1, 2, 6): lo xyz, hi xyz of each child
+    ul = np.floor(((boxes[:, :, 0:3] - qlo).astype(f32) * s).astype(f32))
+    uh = np.ceil(((boxes[:, :, 3:6] - qlo).astype(f32) * s).astype(f32))
+    ql = np.clip(ul, 0, 65535).astype(np.uint32)
+    qh = np.clip(uh, 0, 65535).astype(np.uint32)
+    rec = np.zeros((n - 1, 8), dtype=np.uint32)
+    rec[:, 0:6] = (ql | (qh << np.uint32(16))).reshape(n - 1, 6)
+    ch = scene["children"].astype(np.int64)
+    rec[:, 6:8] = np.where(ch >= n - 1, 0x80000000 | (ch - (n - 1)), ch).astype(np.uint32)
+    return rec, np.concatenate([lo, hi, [rmax]]).astype(f32)
 
 
 def render(scene, cam, W2, H2, mode="bvh", pixels=None, return_hits=False, first_hit=False):

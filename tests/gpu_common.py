@@ -44,30 +44,6 @@ class Session:
         return out.cpu().numpy()
 
 
-def quantised_records(sc):
-    """The 32-byte traversal records (include/splats.h, splats_export_qnodes, S13)
-    that follow from the oracle's exact tree: every plane of every child box quantised to 16 bits over
-    [lo - rmax, hi + rmax], lower planes rounded down, upper planes up, float32 operation by operation."""
-    n = sc["N"]
-    f32 = np.float32
-    rmax = f32(sc["sphere_sorted"][:, 3].max())
-    qlo = (sc["lo"].astype(f32) - rmax).astype(f32)
-    ext = ((sc["hi"].astype(f32) + rmax).astype(f32) - qlo).astype(f32)
-    with np.errstate(divide="ignore"):
-        s = np.where(ext > 0, (f32(65535.0) / ext).astype(f32), f32(0.0)).astype(f32)
-    boxes = sc["aabbs"][sc["children"]].astype(f32)               # (n-1, 2, 6): lo xyz, hi xyz of each child
-    ul = np.floor(((boxes[:, :, 0:3] - qlo).astype(f32) * s).astype(f32))
-    uh = np.ceil(((boxes[:, :, 3:6] - qlo).astype(f32) * s).astype(f32))
-    ql = np.clip(ul, 0, 65535).astype(np.uint32)
-    qh = np.clip(uh, 0, 65535).astype(np.uint32)
-    rec = np.zeros((n - 1, 8), dtype=np.uint32)
-    rec[:, 0:6] = (ql | (qh << np.uint32(16))).reshape(n - 1, 6)
-    ch = sc["children"].astype(np.int64)
-    leaf = ch >= n - 1
-    rec[:, 6:8] = np.where(leaf, 0x80000000 | (ch - (n - 1)), ch).astype(np.uint32)
-    return rec, np.concatenate([sc["lo"].astype(f32), sc["hi"].astype(f32), [rmax]]).astype(f32)
-
-
 def assert_bvh_bit_exact(sc, exact=True):
     """Morton codes, sorted permutation, topology, AABBs (exact, and the quantised records the
     traversal reads), splats: bit-exact against the oracle."""
@@ -81,7 +57,7 @@ def assert_bvh_bit_exact(sc, exact=True):
     np.testing.assert_array_equal(ex["children"].cpu().numpy(), sc["children"])
     np.testing.assert_array_equal(ex["parents"].cpu().numpy(), sc["parents"])
     q = sp.splats_export_qnodes()
-    want_rec, want_frame = quantised_records(sc) if n > 1 else (np.zeros((0, 8), np.uint32), None)
+    want_rec, want_frame = oracle.quantise_child_boxes(sc)   # O7b, pinned in tests/test_oracle_tree.py
     if n > 1:   # what the traversal reads, word by word
         np.testing.assert_array_equal(q["qnodes"].cpu().numpy().view(np.uint32), want_rec)
         np.testing.assert_array_equal(q["frame"].cpu().numpy().view(np.uint32), want_frame.view(np.uint32))

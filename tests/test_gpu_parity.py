@@ -542,7 +542,7 @@ def test_exact_nodes_option_changes_nothing():
 
 def test_quantised_boxes_contain_the_exact_ones():
     # decode the traversal records in float64 and compare with the oracle's exact boxes: never smaller,
-    # at most one code step larger per plane (independent of quantised_records' float32 restatement)
+    # at most one code step larger per plane (independent of the oracle's float32 statement, oracle.quantise_child_boxes)
     W, H = 200, 120
     color, depth, _ = synth.random_frame(W, H, 5, fill=0.8)
     cam = synth.orbit_camera(20.0)

@@ -157,3 +157,76 @@ def test_refit_is_exact_union_over_ranges():
         # sorted order is by (code, id)
         key = sc["sorted_codes"].astype(object) * (2 ** 32) + sc["sorted_ids"].astype(object)
         assert all(key[i] < key[i + 1] for i in range(n - 1))
+
+
+# ---- O7b: the 16-bit storage format of the child boxes (S13)
+def _two_leaf_scene(c0, c1, r0, r1):
+    """Two splats by hand: centres c0, c1 (c0 sorts first), radii r0, r1; one internal node, two leaves."""
+    f32 = np.float32
+    sph = np.array([[*c0, r0], [*c1, r1]], dtype=f32)
+    lo, hi = sph[:, :3].min(0), sph[:, :3].max(0)
+    aabbs = np.zeros((3, 6), f32)                       # node 0 = root, nodes 1, 2 = leaves
+    for i in range(2):
+        aabbs[1 + i, :3] = sph[i, :3] - sph[i, 3]
+        aabbs[1 + i, 3:] = sph[i, :3] + sph[i, 3]
+    aabbs[0, :3], aabbs[0, 3:] = aabbs[1:, :3].min(0), aabbs[1:, 3:].max(0)
+    return dict(N=2, sphere_sorted=sph, lo=lo, hi=hi, aabbs=aabbs, children=np.array([[1, 2]], np.int32))
+
+
+def test_quantised_boxes_hand_worked():
+    # frame: lo = (0, 0, 0), hi = (3, 0, 0) + rmax = 1 -> qlo = -1, ext = (5, 2, 2), codes per unit = 13107, 32767.5, 32767.5
+    sc = _two_leaf_scene((0.0, 0.0, 0.0), (3.0, 0.0, 0.0), 1.0, 0.5)
+    rec, frame = oracle.quantise_child_boxes(sc)
+    assert frame.tolist() == [0.0, 0.0, 0.0, 3.0, 0.0, 0.0, 1.0]
+    w = rec[0]
+    # left child: box [-1, 1]^3 -> x: 0 .. 2 * 13107 = 26214; y, z: 0 .. 65535 (the whole extent)
+    assert (w[0] & 0xffff, w[0] >> 16) == (0, 26214)
+    assert (w[1] & 0xffff, w[1] >> 16) == (0, 65535) and w[2] == w[1]
+    # right child: box x [2.5, 3.5], y, z [-0.5, 0.5] -> x: floor(3.5 * 13107) = 45874 .. ceil(4.5 * 13107) = 58982;
+    # y, z: floor(0.5 * 32767.5) = 16383 .. ceil(1.5 * 32767.5) = 49152
+    assert (w[3] & 0xffff, w[3] >> 16) == (45874, 58982)
+    assert (w[4] & 0xffff, w[4] >> 16) == (16383, 49152) and w[5] == w[4]
+    assert (w[6], w[7]) == (0x80000000, 0x80000001)     # both children are leaves: sorted positions 0 and 1
+
+
+def test_quantised_boxes_zero_extent_axis_and_n_below_two():
+    sc = _two_leaf_scene((1.0, 2.0, 3.0), (2.0, 2.0, 3.0), 0.0, 0.0)   # radii 0: y and z have no extent at all
+    rec, _ = oracle.quantise_child_boxes(sc)
+    assert rec[0, 1] == 0 and rec[0, 2] == 0 and rec[0, 4] == 0 and rec[0, 5] == 0
+    assert (rec[0, 0] & 0xffff, rec[0, 0] >> 16) == (0, 0) and (rec[0, 3] & 0xffff, rec[0, 3] >> 16) == (65535, 65535)
+    one = dict(N=1, sphere_sorted=np.zeros((1, 4), np.float32), lo=np.zeros(3), hi=np.zeros(3), aabbs=np.zeros((1, 6), np.float32),
+               children=np.zeros((0, 2), np.int32))
+    assert oracle.quantise_child_boxes(one)[0].shape == (0, 8)
+
+
+@pytest.mark.parametrize("seed,fill,r_scale", [(1, 0.7, 1.0), (2, 0.3, 2.5), (3, 1.0, 0.5)])
+def test_quantised_boxes_contain_the_exact_ones_and_commute_with_the_union(seed, fill, r_scale):
+    W, H = 96, 54
+    color, depth, cam = synth.random_frame(W, H, seed, fill=fill)
+    sc = oracle.build_scene(color, depth, cam, W, H, r_scale)
+    n = sc["N"]
+    rec, frame = oracle.quantise_child_boxes(sc)
+    # (a) decoded in float64: never smaller than the exact box, at most one code step larger per plane
+    fr = frame.astype(np.float64)
+    qlo = fr[0:3] - fr[6]
+    step = ((fr[3:6] + fr[6]) - qlo) / 65535.0
+    w = rec[:, 0:6].reshape(-1, 2, 3)
+    lo, hi = qlo + (w & 0xffff) * step, qlo + (w >> 16) * step
+    want = sc["aabbs"][sc["children"]].astype(np.float64)
+    eps = 1e-6 * np.abs(want).max()
+    assert np.all(lo <= want[:, :, 0:3] + eps) and np.all(hi >= want[:, :, 3:6] - eps)
+    assert np.all(lo >= want[:, :, 0:3] - step - eps) and np.all(hi <= want[:, :, 3:6] + step + eps)
+    # (b) quantisation is monotone, so it commutes with the union: the code box of an internal child equals the
+    # min / max of the code boxes stored in that child's own record (what a bottom-up build on codes relies on)
+    ql, qh = (w & 0xffff).astype(np.int64), (w >> 16).astype(np.int64)
+    ch = sc["children"]
+    for j in range(n - 1):
+        for side in range(2):
+            c = int(ch[j, side])
+            if c < n - 1:
+                assert np.array_equal(ql[j, side], ql[c].min(axis=0)) and np.array_equal(qh[j, side], qh[c].max(axis=0))
+    # (c) links: every node and every leaf is referenced exactly once
+    links = rec[:, 6:8].reshape(-1)
+    leaves = np.sort(links[links >= 0x80000000] & 0x7fffffff)
+    inner = np.sort(links[links < 0x80000000])
+    assert np.array_equal(leaves, np.arange(n)) and np.array_equal(inner, np.arange(1, n - 1))
