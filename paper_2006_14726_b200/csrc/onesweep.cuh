@@ -76,7 +76,7 @@ struct SortSmem {
   uint32_t vstage[SORT_THREADS * SORT_MAX_ITEMS];  // values in tile-sorted order
   uint64_t stage2[SORT_THREADS * SORT_MAX_ITEMS];  // window buffer B
   uint32_t vstage2[SORT_THREADS * SORT_MAX_ITEMS];
-  int win[2];                                       // bounds of the current window
+  uint64_t mbar;                                    // mbarrier of the window phase's bulk copies
 };
 constexpr int WIN_MAX = SORT_THREADS * SORT_MAX_ITEMS;   // capacity of a window (4096 elements)
 
@@ -387,24 +387,65 @@ static_assert(WIN_MAX <= (1 << 24), "comparison key = the key bits below the buc
 
 constexpr int WIN_EXTRA = SPLATS_WIN_EXTRA;           // a window is loaded with this many elements beyond its nominal end
 
+// ---- bulk asynchronous copy global -> shared (cp.async.bulk, sm_90+): one thread asks the copy engine for a
+// contiguous range; completion is counted in bytes on an mbarrier that every thread of the block waits on.
+// Source, destination and size must be multiples of 16 bytes.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_addr(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@!p bra WAIT_%=;\n\t}"
+      :: "r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+
 __device__ __forceinline__ void window_phase(SortSmem& s, uint64_t* key, uint32_t* val, FrameState* st, uint32_t n, const int WIN_BSHIFT) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint32_t* heads = s.tile_off;   // one bit per loaded element: a bucket starts here (128 words)
   // nominal window size: what the capacity allows, a quarter of it for small frames (more windows than blocks)
   const uint32_t T = n > (uint32_t)gridDim.x * (WIN_MAX / 4) ? WIN_MAX - WIN_EXTRA : WIN_MAX / 4;
   const uint32_t nwin = (n + T - 1) / T;
+  if (tid == 0) mbar_init(&s.mbar, 1u);
+  uint32_t phase = 0;
+  __syncthreads();
   for (uint32_t k = blockIdx.x; k < nwin; k += gridDim.x) {
     // ---- load [k T, (k + 1) T + WIN_EXTRA) in one go; the window proper, [B(k T), B((k + 1) T)), is found in it.
     // The loaded range overlaps the neighbouring windows, which other blocks may be writing at the same time.
     // That is harmless: outside its own window a block looks at the bucket bits of a key only (to find the heads),
     // and a neighbour only permutes keys inside buckets, so those bits are the same before, during and after its
     // writes (64-bit stores: a key is seen old or new, never torn); the windows proper are disjoint.
-    const uint32_t g0 = k * T, gend = min(n, g0 + T + WIN_EXTRA), cnt = gend - g0;
-    for (uint32_t i = tid; i < cnt; i += SORT_THREADS) {
-      s.stage[i] = __ldcg(key + g0 + i);
-      s.vstage[i] = __ldcg(val + g0 + i);
+    // Keys and values come as two bulk asynchronous copies (up to 32 + 16 KiB; g0 is a multiple of 4 elements, so
+    // both ranges are 16-byte aligned); the up to three elements behind the last multiple of four are loaded by hand.
+    const uint32_t g0 = k * T, gend = min(n, g0 + T + WIN_EXTRA), cnt = gend - g0, cnt4 = cnt & ~3u;
+    if (tid == 0 && cnt4) {
+      // the staging buffers were read and written through the generic proxy (previous window, earlier passes), the
+      // global arrays by other blocks before the grid barrier: order all of that before the async proxy's accesses
+      asm volatile("fence.proxy.async;" ::: "memory");
+      mbar_expect_tx(&s.mbar, cnt4 * 12u);
+      bulk_g2s(s.stage, key + g0, cnt4 * 8u, &s.mbar);
+      bulk_g2s(s.vstage, val + g0, cnt4 * 4u, &s.mbar);
+    }
+    if (tid < (int)(cnt - cnt4)) {
+      s.stage[cnt4 + tid] = __ldcg(key + g0 + cnt4 + tid);
+      s.vstage[cnt4 + tid] = __ldcg(val + g0 + cnt4 + tid);
     }
     const uint64_t kprev = g0 > 0 ? __ldcg(key + g0 - 1) : 0ull;
+    if (cnt4) {
+      mbar_wait(&s.mbar, phase);
+      phase ^= 1u;
+    }
     __syncthreads();
     // bucket heads as a bit map (chunk c = elements 32 c .. 32 c + 31 of the loaded range)
     const uint32_t nchunk = (cnt + 31) >> 5;
