@@ -132,7 +132,10 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const QBox
 }
 
 template <class Gather>
-__global__ void __launch_bounds__(TT_THREADS)
+#ifndef SPLATS_TT_BLOCKS
+#define SPLATS_TT_BLOCKS 1
+#endif
+__global__ void __launch_bounds__(TT_THREADS, SPLATS_TT_BLOCKS)
 tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
                  float4* __restrict__ sphere, float4* __restrict__ rgba, uint32_t* __restrict__ ids_out, uint4* pyr,
                  QNode* __restrict__ qnodes, int4* __restrict__ queue, uint8_t* __restrict__ tile_min,
