@@ -27,12 +27,6 @@ constexpr int KBUF = SPLATS_KBUF;
 #endif
 constexpr int SSTACK = SPLATS_SSTACK;  // deeper entries live in local memory; 8 leaves more of the SM's 256 KB to L1 (4 .. 16 measured: within 1 %)
 constexpr int LSTACK = 96 - SSTACK;  // SSTACK + LSTACK >= 63 key bits + 32 index bits + 1
-#ifndef SPLATS_TICKET_AHEAD
-#define SPLATS_TICKET_AHEAD 0
-#endif
-#ifndef SPLATS_PREFETCH
-#define SPLATS_PREFETCH 0
-#endif
 #ifndef SPLATS_POSTPONE
 #define SPLATS_POSTPONE 0
 #endif
@@ -213,14 +207,7 @@ render_kernel(RenderParams prm) {
   const int nwarps = gridDim.x * (RENDER_THREADS / 32);
   if (blockIdx.x == 0 && tid == 0) atomicAdd(prm.traced, (unsigned long long)ntiles * 32ull);
   int tile = blockIdx.x * (RENDER_THREADS / 32) + warp;
-#if SPLATS_TICKET_AHEAD
-  // the ticket for the next tile is taken before this one is traced: the atomic's round trip hides behind the traversal
-  unsigned nxt = 0;
-  for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, nxt, 0)) {
-  if (lane == 0) nxt = atomicAdd(prm.sched, 1u);
-#else
   for (; tile < ntiles + nfill; tile = nwarps + (int)__shfl_sync(0xffffffffu, lane == 0 ? atomicAdd(prm.sched, 1u) : 0u, 0)) {
-#endif
   if (tile >= ntiles) {
     const int px0 = rx0 * 8, px1 = rx1 * 8, py0 = ry0 * 4, py1 = ry1 * 4;
     const int base = (tile - ntiles) * FILL_PX;
@@ -299,13 +286,6 @@ render_kernel(RenderParams prm) {
         // ---- internal nodes: both child boxes come with the node (one 32-byte load)
         while ((int)node >= 0) {
           const u8x rec = ldg_u8(prm.qnodes + node);
-#if SPLATS_PREFETCH
-          // both child records are known before the slab arithmetic: start fetching them into L1
-          if ((int)rec.v[6] >= 0) asm volatile("prefetch.global.L1 [%0];" :: "l"(prm.qnodes + rec.v[6]));
-#if SPLATS_PREFETCH > 1
-          if ((int)rec.v[7] >= 0) asm volatile("prefetch.global.L1 [%0];" :: "l"(prm.qnodes + rec.v[7]));
-#endif
-#endif
           STAT_ADD(0, 1);
           STAT_MAX(5, sp);
 #define QPLANE(w, sel) __uint_as_float(__byte_perm((w), 0x4B000000u, (sel)))
