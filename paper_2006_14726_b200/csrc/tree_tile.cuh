@@ -133,7 +133,7 @@ __device__ __forceinline__ int tile_report(TileSmem& s, int p, int q, const QBox
 
 template <class Gather>
 #ifndef SPLATS_TT_BLOCKS
-#define SPLATS_TT_BLOCKS 1
+#define SPLATS_TT_BLOCKS 5   // resident blocks per SM the register allocation aims at (48 registers; 4 .. 6 measured)
 #endif
 __global__ void __launch_bounds__(TT_THREADS, SPLATS_TT_BLOCKS)
 tree_tile_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ perm, const Gather src, FrameState* st,
